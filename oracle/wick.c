@@ -117,34 +117,41 @@ int wick_fourpt(int L, const double* S_u, const double* S_d, const double* S_s,
     const cplx* S[3] = {(const cplx*)S_u, (const cplx*)S_d, (const cplx*)S_s};
     cplx* F = (cplx*)F_out;
     memset(F, 0, sizeof(cplx) * (size_t)nr * nspin);
-#pragma omp parallel for collapse(2) schedule(dynamic)
-    for (int ir = 0; ir < nr; ir++)
-        for (int is = 0; is < nspin; is++) {
-            int r = rlist[ir];
-            int rx = r % L, ry = (r / L) % L, rz = r / (L * L);
-            cplx acc = 0.0;
-            for (int X = 0; X < V; X++) {
-                int x0 = X % L, y0 = (X / L) % L, z0 = X / (L * L);
-                int xs = ((x0 + rx) % L) + L * (((y0 + ry) % L) + L * ((z0 + rz) % L));
-                const cplx* Sx[3] = {S[0] + (size_t)xs * 144, S[1] + (size_t)xs * 144, S[2] + (size_t)xs * 144};
-                const cplx* Sy[3] = {S[0] + (size_t)X * 144, S[1] + (size_t)X * 144, S[2] + (size_t)X * 144};
-                for (int t1 = 0; t1 < nterm[0]; t1++)
-                    for (int t2 = 0; t2 < nterm[1]; t2++)
-                        for (int t3 = 0; t3 < nterm[2]; t3++)
-                            for (int t4 = 0; t4 < nterm[3]; t4++) {
-                                int f[6], h[6];
-                                for (int m = 0; m < 3; m++) {
-                                    f[m] = flav[(0 * 3 + t1) * 3 + m];
-                                    f[3 + m] = flav[(1 * 3 + t2) * 3 + m];
-                                    h[m] = flav[(2 * 3 + t3) * 3 + m];
-                                    h[3 + m] = flav[(3 * 3 + t4) * 3 + m];
-                                }
-                                double k = coef[0 * 3 + t1] * coef[1 * 3 + t2] * coef[2 * 3 + t3] * coef[3 * 3 + t4];
-                                acc += k * pair_term(Sx, Sy, f, h, spins[is * 4 + 0], spins[is * 4 + 1],
-                                                     spins[is * 4 + 2], spins[is * 4 + 3]);
-                            }
-            }
-            F[(size_t)ir * nspin + is] = acc;
-        }
+    /* one work item per (r, spin combination, X): a flat loop so that a single (r, spin) request
+     * still uses every core */
+    const long nitem = (long)nr * nspin * V;
+#pragma omp parallel for schedule(dynamic)
+    for (long item = 0; item < nitem; item++) {
+        int X = (int)(item % V);
+        int is = (int)((item / V) % nspin);
+        int ir = (int)(item / ((long)V * nspin));
+        int r = rlist[ir];
+        int rx = r % L, ry = (r / L) % L, rz = r / (L * L);
+        int x0 = X % L, y0 = (X / L) % L, z0 = X / (L * L);
+        int xs = ((x0 + rx) % L) + L * (((y0 + ry) % L) + L * ((z0 + rz) % L));
+        const cplx* Sx[3] = {S[0] + (size_t)xs * 144, S[1] + (size_t)xs * 144, S[2] + (size_t)xs * 144};
+        const cplx* Sy[3] = {S[0] + (size_t)X * 144, S[1] + (size_t)X * 144, S[2] + (size_t)X * 144};
+        cplx acc = 0.0;
+        for (int t1 = 0; t1 < nterm[0]; t1++)
+            for (int t2 = 0; t2 < nterm[1]; t2++)
+                for (int t3 = 0; t3 < nterm[2]; t3++)
+                    for (int t4 = 0; t4 < nterm[3]; t4++) {
+                        int f[6], h[6];
+                        for (int m = 0; m < 3; m++) {
+                            f[m] = flav[(0 * 3 + t1) * 3 + m];
+                            f[3 + m] = flav[(1 * 3 + t2) * 3 + m];
+                            h[m] = flav[(2 * 3 + t3) * 3 + m];
+                            h[3 + m] = flav[(3 * 3 + t4) * 3 + m];
+                        }
+                        double k = coef[0 * 3 + t1] * coef[1 * 3 + t2] * coef[2 * 3 + t3] * coef[3 * 3 + t4];
+                        acc += k * pair_term(Sx, Sy, f, h, spins[is * 4 + 0], spins[is * 4 + 1],
+                                             spins[is * 4 + 2], spins[is * 4 + 3]);
+                    }
+        double* dst = (double*)&F[(size_t)ir * nspin + is];
+#pragma omp atomic
+        dst[0] += creal(acc);
+#pragma omp atomic
+        dst[1] += cimag(acc);
+    }
     return 0;
 }
