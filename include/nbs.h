@@ -1,0 +1,170 @@
+/*
+ * nbs.h -- C ABI of the B200-native hot path of the HAL QCD effective baryon block algorithm
+ * (H. Nemura, arXiv:1604.07983; citations are PAPER.md:<line>, section / equation).
+ *
+ * What the library computes (eq. 2.1; eq. 2.4; eq. 2.6):
+ * for one time slice t and each requested channel <B1 B2 | B3 B4>
+ *
+ *   F[ch][a1][a2][a3][a4][r] = sum_X  sum_P sigma_P [B1_a1](X+r; xi'_P1 xi'_P2 xi'_P3) [B2_a2](X; xi'_P4 xi'_P5 xi'_P6)
+ *                               x eps eps (C g5)(C g5) delta delta                           (eq. 2.4)
+ *
+ * from the u, d, s wall-source quark propagators on that slice, via (i) normal baryon blocks
+ * (eq. 2.5 / 4.1), FFT, (ii)+(iii) effective blocks and their product (eqs. 4.2, 4.3), inverse
+ * FFT (eq. 2.6).  Everything runs in hand-written sm_100a CUDA kernels in complex128; there is no
+ * CPU fallback: every entry point fails with NBS_ECUDA if no CUDA device is usable.
+ *
+ * Conventions (readings A1-A17):
+ *   xi = colour + 3*spin (12 values);  site index x + L*(y + L*z);  periodic space;
+ *   propagator S_f[site][sink xi][source xi'] complex128 (re, im interleaved), row-major 12x12;
+ *   C gamma_5 = [[0,1,0,0],[-1,0,0,0],[0,0,0,1],[0,0,-1,0]];
+ *   r = position of B1 minus position of B2;  spin index ((a1*4+a2)*4+a3)*4+a4.
+ *
+ * Threading: a context is not thread-safe; different contexts are independent.
+ * Errors: every function returns 0 (NBS_OK) or a negative NBS_E* code; nothing throws across the
+ * ABI; nbs_last_error() gives a human-readable message for the last failure on a context.
+ */
+#ifndef NBS_H_
+#define NBS_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nbs_ctx nbs_ctx;
+
+/* Interpolating fields of eqs. 2.2-2.3. */
+enum {
+    NBS_P = 0,       /* p       =  eps (u Cg5 d) u */
+    NBS_N = 1,       /* n       = -eps (u Cg5 d) d */
+    NBS_LAMBDA = 2,  /* Lambda  = (X_u + X_d - 2 X_s)/sqrt 6 */
+    NBS_SIGMA_P = 3, /* Sigma+  = -eps (u Cg5 s) u */
+    NBS_SIGMA_0 = 4, /* Sigma0  = (X_u - X_d)/sqrt 2 */
+    NBS_SIGMA_M = 5, /* Sigma-  = -eps (d Cg5 s) d */
+    NBS_XI_0 = 6,    /* Xi0     =  eps (u Cg5 s) s */
+    NBS_XI_M = 7,    /* Xi-     = -eps (d Cg5 s) s */
+    NBS_XU = 8,      /* X_u     =  eps (d Cg5 s) u   (eq. 2.3; e.g. <p Lambda pbar Xubar>, eq. 2.7) */
+    NBS_XD = 9,      /* X_d     =  eps (s Cg5 u) d */
+    NBS_XS = 10,     /* X_s     =  eps (u Cg5 d) s */
+    NBS_NUM_BARYONS = 11
+};
+
+/* One channel <B1 B2 | B3 B4>: sink baryons b1 (at X+r), b2 (at X); source baryons b3, b4. */
+typedef struct {
+    int b1, b2, b3, b4;
+} nbs_channel;
+
+enum {
+    NBS_OK = 0,
+    NBS_EINVAL = -1,  /* bad argument: L, T, baryon id, channel violating flavour conservation, range */
+    NBS_ENOMEM = -2,  /* workspace does not fit in device memory / the given budget */
+    NBS_ESTATE = -3,  /* call order: slice t not loaded, context destroyed, ... */
+    NBS_ECUDA = -4    /* CUDA runtime error (sticky for the context; see nbs_last_error) */
+};
+
+enum {
+    NBS_MEM_DEVICE = 0, /* pointer is device memory on the context's device */
+    NBS_MEM_HOST = 1    /* pointer is host memory (pinned for asynchronous copies) */
+};
+
+/*
+ * nbs_create -- build the diagram tables (the paper's CPU "diagramatical classification", SoA
+ * tables copied to the device before the kernels) and allocate the workspace.
+ *   out       : receives the context (library-owned; free with nbs_destroy).
+ *   L, T      : spatial extent (2 <= L <= 64, FFT path: any L; radix-2 fast path for powers of 2)
+ *               and number of time slices (labels only: slices are independent).
+ *   ch, nch   : channel list (host memory, copied).  ch == NULL selects the standard 52 channels
+ *               "from NN to Xi-Xi" in the order of DESIGN.md reading A10.
+ *   device    : CUDA device ordinal.
+ *   workspace_budget_bytes : upper bound for library-owned device memory (0 = no bound).
+ * Errors: NBS_EINVAL (bad L/T/id, or a channel whose sink and source flavour content differ for
+ * every elementary source term: F would vanish identically), NBS_ENOMEM, NBS_ECUDA.
+ */
+int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int device,
+               size_t workspace_budget_bytes);
+
+/*
+ * nbs_load_propagators -- hand the u, d, s propagators of time slice t to the library
+ * ("Assuming that the quark propagators are already solved").
+ *   u, d, s : each [L^3][12][12] complex128 (layout above).  Pointer equality (d == u, s == u)
+ *             is allowed and means the same array.
+ *   memloc  : NBS_MEM_DEVICE -> borrowed, must stay valid until the matching nbs_correlator(t)
+ *             has completed on its stream;  NBS_MEM_HOST -> copied asynchronously on `stream`
+ *             into library-owned device memory (the caller may reuse the host buffer after the
+ *             stream has passed this point).
+ *   stream  : a cudaStream_t (NULL = default stream).
+ * Only one slice is held at a time per slot; the library keeps 2 slots (t % 2) so that two
+ * slices can be in flight on two streams (cudaStream overlap).
+ */
+int nbs_load_propagators(nbs_ctx* ctx, int t, const void* u, const void* d, const void* s, int memloc,
+                         void* stream);
+
+/*
+ * nbs_correlator -- the hot path for slice t, channels [ch_begin, ch_end):
+ *   (i)  normal baryon blocks, eq. 4.1, forward FFT,
+ *   (ii) effective blocks, eq. 4.2, fused with
+ *   (iii) their product summed over the shared index and the diagrams, eq. 4.3,
+ *   inverse FFT, eq. 2.6.
+ * Writes F[ch - ch_begin][a1][a2][a3][a4][r] (complex128, r fastest) to `out`.
+ *   out, out_bytes, memloc : caller-owned buffer of at least (ch_end-ch_begin)*256*L^3*16 bytes;
+ *             NBS_MEM_DEVICE (written by the kernels) or NBS_MEM_HOST (device result copied back
+ *             asynchronously on `stream`).
+ * Asynchronous on `stream`: synchronise the stream before reading `out`.
+ * Errors: NBS_ESTATE (slice t not loaded), NBS_EINVAL (range / size), NBS_ECUDA.
+ */
+int nbs_correlator(nbs_ctx* ctx, int t, int ch_begin, int ch_end, void* out, size_t out_bytes, int memloc,
+                   void* stream);
+
+/* nbs_destroy -- synchronise the device, free tables and workspace.  NULL is a no-op. */
+void nbs_destroy(nbs_ctx* ctx);
+
+/* Helpers. */
+const char* nbs_last_error(const nbs_ctx* ctx); /* never NULL; ctx == NULL -> last nbs_create error */
+size_t nbs_workspace_bytes(const nbs_ctx* ctx); /* library-owned device bytes */
+int nbs_num_channels(const nbs_ctx* ctx);
+int nbs_channel_info(const nbs_ctx* ctx, int i, nbs_channel* out);
+
+/*
+ * Table statistics of the host generator (row a0 of DESIGN.md; pins: 52 channels, 3456 literal
+ * and 370 = 1+9+144+144+36+36 effective terms for <p Lambda pbar Xubar>).
+ * These run on the host only (no CUDA call) so they work on a machine without a GPU.
+ *   nbs_std_channels : writes the standard 52 channels to `out` (capacity `cap`), returns 52.
+ *   nbs_diagram_stats: for one channel, returns the number of diagrams (coset representatives
+ *             summed over elementary source terms) and writes up to `cap` shared-index sizes K_d
+ *             to `K` (in enumeration order: source terms major, permutations lexicographic) and
+ *             signs sigma_P to `sign`; *literal_terms receives diagrams * (N_c! N_alpha)^2.
+ *             Returns NBS_EINVAL for an invalid channel.
+ */
+int nbs_std_channels(nbs_channel* out, int cap);
+int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long long* literal_terms);
+
+/*
+ * Stage-level entry points (used by the parity tests and by bench.py's per-stage timing).
+ *   nbs_blocks_x : eq. 4.1 only: writes the x-space normal block of baryon `baryon` for the
+ *             loaded slice t to device buffer out[site][alpha][xi1][xi2][xi3] (complex128).
+ *   nbs_model_flops : the algorithmic flop count per lattice site for the context's channel list
+ *             (complex multiply-add = 8 flops): blocks, fft (forward+inverse), product
+ *             (256 * sum_d K_d over the channels' diagrams), as doubles.
+ */
+int nbs_blocks_x(nbs_ctx* ctx, int t, int baryon, void* out_dev, size_t out_bytes, void* stream);
+int nbs_model_flops(const nbs_ctx* ctx, double* blocks, double* fft, double* product);
+
+/*
+ *   nbs_exec_flops : flops per site the product kernels actually execute (8 * 256 * sum of K_d over
+ *             the DISTINCT elementary correlators: source Lambda / Sigma0 terms shared between
+ *             channels of one sink pair are evaluated once).  <= the `product` model count.
+ *   nbs_fft3d : rows a2 / a5 alone (eq. 2.6): in-place 3-D transform of a device
+ *             array data[site][R] complex128, every one of the R components independently.
+ *             inverse == 0: sum_x f(x) exp(-i q.x);  inverse != 0: L^-3 sum_q f(q) exp(+i q.r).
+ *   nbs_kernel_launches : number of CUDA kernels this context has launched so far (bench.py's
+ *             `gpu_launches`).
+ */
+int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);
+int nbs_fft3d(nbs_ctx* ctx, void* data_dev, size_t R, int inverse, void* stream);
+long long nbs_kernel_launches(const nbs_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBS_H_ */

@@ -1,0 +1,393 @@
+// C-ABI entry points (include/nbs.h).  Host orchestration only; all arithmetic is in the kernels.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "nbs_kernels.cuh"
+#include "nbs_tables.hpp"
+
+using namespace nbs;
+
+namespace {
+
+std::string g_create_error = "";
+
+constexpr int NSLOTS_MAX = 2; // time slices in flight (cudaStream overlap)
+
+struct Slice {
+    int t = -1;
+    const double2* S[3] = {nullptr, nullptr, nullptr}; // u, d, s (device)
+    double2* own[3] = {nullptr, nullptr, nullptr};     // library-owned copies for host input
+    double2* B = nullptr;  // [V][R] normal blocks, x-space then momentum space (in place)
+    double2* E = nullptr;  // [V][nelem][256]
+    double2* Ft = nullptr; // [V][nch][256]
+};
+
+} // namespace
+
+struct nbs_ctx {
+    int L = 0, T = 0, device = 0;
+    size_t V = 0;
+    Plan plan;
+    std::string err = "";
+    bool cuda_failed = false;
+    size_t workspace = 0;
+    int nslices = 0;
+    Slice slice[NSLOTS_MAX];
+    size_t R = 0; // block row length (complex) = nbaryons * 6912
+    // device tables
+    PairRec* d_pairs = nullptr;
+    ElemRec* d_elems = nullptr;
+    DiagramRec* d_diagrams = nullptr;
+    uint16_t* d_gather = nullptr;
+    int* d_term_begin = nullptr;
+    ChanTermRec* d_terms = nullptr;
+    int* d_baryon_of_slot = nullptr;
+    int* d_one_baryon = nullptr; // scratch for nbs_blocks_x
+    BlockRec* d_brec = nullptr;
+    BTermRec* d_bterm = nullptr;
+    double2* d_tw = nullptr;
+    unsigned dq_mask = 0;
+    unsigned dq_mask_of[NBS_NUM_BARYONS] = {};
+    std::vector<void*> allocs;
+    long long launches = 0;
+};
+
+namespace {
+
+int fail(nbs_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg; else g_create_error = msg;
+    return code;
+}
+int cuda_fail(nbs_ctx* c, cudaError_t e, const char* what) {
+    if (c) c->cuda_failed = true;
+    return fail(c, NBS_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(c, call)                                            \
+    do {                                                       \
+        cudaError_t e_ = (call);                               \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); \
+    } while (0)
+
+template <typename Tp>
+int upload(nbs_ctx* c, Tp*& dst, const std::vector<Tp>& src) {
+    size_t bytes = std::max<size_t>(src.size(), 1) * sizeof(Tp);
+    void* p = nullptr;
+    CU(c, cudaMalloc(&p, bytes));
+    c->allocs.push_back(p);
+    c->workspace += bytes;
+    if (!src.empty()) CU(c, cudaMemcpy(p, src.data(), src.size() * sizeof(Tp), cudaMemcpyHostToDevice));
+    dst = (Tp*)p;
+    return NBS_OK;
+}
+int dev_alloc(nbs_ctx* c, double2*& dst, size_t ncomplex) {
+    void* p = nullptr;
+    CU(c, cudaMalloc(&p, ncomplex * sizeof(double2)));
+    c->allocs.push_back(p);
+    c->workspace += ncomplex * sizeof(double2);
+    dst = (double2*)p;
+    return NBS_OK;
+}
+
+template <bool INV>
+int launch_fft_axis(nbs_ctx* c, double2* data, size_t R, int axis, double scale, cudaStream_t st) {
+    const int L = c->L;
+    dim3 grid((unsigned)((R + FFT_THREADS - 1) / FFT_THREADS), (unsigned)(L * L));
+    switch (L) {
+    case 2: k_fft_axis_pow2<2, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
+    case 4: k_fft_axis_pow2<4, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
+    case 8: k_fft_axis_pow2<8, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
+    case 16: k_fft_axis_pow2<16, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
+    case 32: k_fft_axis_pow2<32, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
+    default: k_fft_axis_generic<INV><<<grid, FFT_THREADS, 0, st>>>(data, R, L, axis, c->d_tw, scale); break;
+    }
+    CU(c, cudaGetLastError());
+    ++c->launches;
+    return NBS_OK;
+}
+
+int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st) {
+    for (int axis = 0; axis < 3; ++axis) {
+        int rc = inverse ? launch_fft_axis<true>(c, data, R, axis, 1.0 / (double)c->L, st)
+                         : launch_fft_axis<false>(c, data, R, axis, 1.0, st);
+        if (rc) return rc;
+    }
+    return NBS_OK;
+}
+
+int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, int nslots, unsigned dq_mask, double2* out,
+                  size_t row_stride, cudaStream_t st) {
+    size_t smem = (3 * 144 + 9 * 432) * sizeof(double2);
+    k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, smem, st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask, c->d_brec,
+                                                           c->d_bterm, out, row_stride);
+    CU(c, cudaGetLastError());
+    ++c->launches;
+    return NBS_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int nbs_std_channels(nbs_channel* out, int cap) {
+    std::vector<nbs_channel> ch = standard_channels();
+    for (int i = 0; i < (int)ch.size() && i < cap; ++i) out[i] = ch[i];
+    return (int)ch.size();
+}
+
+int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long long* literal_terms) {
+    if (!ch) return NBS_EINVAL;
+    std::vector<DiagramInfo> d;
+    std::string err = channel_diagrams(*ch, d);
+    if (!err.empty()) { g_create_error = err; return NBS_EINVAL; }
+    for (int i = 0; i < (int)d.size() && i < cap; ++i) {
+        if (K) K[i] = d[i].K;
+        if (sign) sign[i] = d[i].sign;
+    }
+    if (literal_terms) *literal_terms = (long long)d.size() * 576; // (N_c! N_alpha)^B
+    return (int)d.size();
+}
+
+int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int device, size_t budget) {
+    if (!out) return fail(nullptr, NBS_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (L < 2 || L > FFT_MAXL) return fail(nullptr, NBS_EINVAL, "L must be in [2, 64]");
+    if (T < 1) return fail(nullptr, NBS_EINVAL, "T must be >= 1");
+    if (ch && nch < 1) return fail(nullptr, NBS_EINVAL, "nch must be >= 1");
+    std::vector<nbs_channel> chans = ch ? std::vector<nbs_channel>(ch, ch + nch) : standard_channels();
+    nbs_ctx* c = new nbs_ctx();
+    std::string err = build_plan(chans, c->plan);
+    if (!err.empty()) { delete c; return fail(nullptr, NBS_EINVAL, err); }
+    c->L = L; c->T = T; c->device = device;
+    c->V = (size_t)L * L * L;
+    c->R = c->plan.baryons.size() * (size_t)BLOCK_ELEMS;
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || device < 0 || device >= ndev) {
+        std::string msg = e != cudaSuccess ? std::string("no usable CUDA device: ") + cudaGetErrorString(e)
+                                           : "device ordinal out of range";
+        delete c;
+        return fail(nullptr, NBS_ECUDA, msg);
+    }
+#define CUC(call)                                                                 \
+    do {                                                                          \
+        int rc_ = (call);                                                         \
+        if (rc_ != NBS_OK) { g_create_error = c->err; nbs_destroy(c); return rc_; } \
+    } while (0)
+#define CUX(call)                                                                                        \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess) { g_create_error = std::string(#call) + ": " + cudaGetErrorString(e_); nbs_destroy(c); return NBS_ECUDA; } \
+    } while (0)
+    CUX(cudaSetDevice(device));
+
+    // block-construction descriptors for all baryon ids
+    std::vector<BlockRec> brec(NBS_NUM_BARYONS);
+    std::vector<BTermRec> bterm;
+    for (int b = 0; b < NBS_NUM_BARYONS; ++b) {
+        brec[b].term_begin = (int)bterm.size();
+        for (auto& t : block_terms(b)) {
+            BTermRec r;
+            r.coef = t.coef; r.dq = t.f0 * 3 + t.f1; r.f2 = t.f2;
+            r.p0 = t.perm[0]; r.p1 = t.perm[1]; r.p2 = t.perm[2]; r.pad = 0;
+            bterm.push_back(r);
+            c->dq_mask_of[b] |= 1u << r.dq;
+        }
+        brec[b].term_end = (int)bterm.size();
+    }
+    for (int b : c->plan.baryons) c->dq_mask |= c->dq_mask_of[b];
+    std::vector<double2> tw(L);
+    for (int m = 0; m < L; ++m) {
+        long double ang = -2.0L * 3.141592653589793238462643383279502884L * m / L;
+        tw[m] = make_double2((double)cosl(ang), (double)sinl(ang));
+    }
+    CUC(upload(c, c->d_pairs, c->plan.pairs));
+    CUC(upload(c, c->d_elems, c->plan.elems));
+    CUC(upload(c, c->d_diagrams, c->plan.diagrams));
+    CUC(upload(c, c->d_gather, c->plan.gather));
+    CUC(upload(c, c->d_term_begin, c->plan.chan_term_begin));
+    CUC(upload(c, c->d_terms, c->plan.chan_terms));
+    CUC(upload(c, c->d_baryon_of_slot, c->plan.baryons));
+    CUC(upload(c, c->d_one_baryon, std::vector<int>(NBS_NUM_BARYONS, 0)));
+    {
+        std::vector<int> ids(NBS_NUM_BARYONS);
+        for (int b = 0; b < NBS_NUM_BARYONS; ++b) ids[b] = b;
+        CUX(cudaMemcpy(c->d_one_baryon, ids.data(), ids.size() * sizeof(int), cudaMemcpyHostToDevice));
+    }
+    CUC(upload(c, c->d_brec, brec));
+    CUC(upload(c, c->d_bterm, bterm));
+    CUC(upload(c, c->d_tw, tw));
+
+    // workspace: per slice in flight, blocks + elementary correlators + channel correlators
+    size_t nelem = c->plan.elems.size(), nchan = c->plan.channels.size();
+    size_t per_slice = c->V * (c->R + (nelem + nchan) * 256) * sizeof(double2);
+    size_t free_b = 0, total_b = 0;
+    CUX(cudaMemGetInfo(&free_b, &total_b));
+    size_t avail = (size_t)(0.92 * (double)free_b);
+    if (budget && budget < avail + c->workspace) avail = budget > c->workspace ? budget - c->workspace : 0;
+    c->nslices = (T >= 2 && 2 * per_slice <= avail) ? 2 : 1;
+    if (per_slice > avail) {
+        g_create_error = "workspace of " + std::to_string(per_slice) + " bytes per time slice does not fit (" +
+                         std::to_string(avail) + " available)";
+        nbs_destroy(c);
+        return NBS_ENOMEM;
+    }
+    for (int i = 0; i < c->nslices; ++i) {
+        CUC(dev_alloc(c, c->slice[i].B, c->V * c->R));
+        CUC(dev_alloc(c, c->slice[i].E, c->V * nelem * 256));
+        CUC(dev_alloc(c, c->slice[i].Ft, c->V * nchan * 256));
+    }
+    CUX(cudaFuncSetAttribute(k_product_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
+    CUX(cudaFuncSetAttribute(k_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)((3 * 144 + 9 * 432) * sizeof(double2))));
+    *out = c;
+    return NBS_OK;
+#undef CUC
+#undef CUX
+}
+
+int nbs_load_propagators(nbs_ctx* c, int t, const void* u, const void* d, const void* s, int memloc, void* stream) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    if (t < 0 || t >= c->T || !u || !d || !s) return fail(c, NBS_EINVAL, "bad slice index or NULL propagator");
+    if (memloc != NBS_MEM_DEVICE && memloc != NBS_MEM_HOST) return fail(c, NBS_EINVAL, "bad memloc");
+    CU(c, cudaSetDevice(c->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    Slice& sl = c->slice[t % c->nslices];
+    const void* src[3] = {u, d, s};
+    if (memloc == NBS_MEM_DEVICE) {
+        for (int f = 0; f < 3; ++f) sl.S[f] = (const double2*)src[f];
+    } else {
+        size_t n = c->V * 144;
+        for (int f = 0; f < 3; ++f) {
+            int alias = -1;
+            for (int g = 0; g < f; ++g)
+                if (src[g] == src[f]) alias = g;
+            if (alias >= 0) { sl.S[f] = sl.S[alias]; continue; }
+            if (!sl.own[f]) {
+                int rc = dev_alloc(c, sl.own[f], n);
+                if (rc) return rc;
+            }
+            CU(c, cudaMemcpyAsync(sl.own[f], src[f], n * sizeof(double2), cudaMemcpyHostToDevice, st));
+            sl.S[f] = sl.own[f];
+        }
+    }
+    sl.t = t;
+    return NBS_OK;
+}
+
+int nbs_blocks_x(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes, void* stream) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    if (baryon < 0 || baryon >= NBS_NUM_BARYONS || !out_dev) return fail(c, NBS_EINVAL, "bad baryon id or NULL output");
+    if (t < 0 || t >= c->T) return fail(c, NBS_EINVAL, "bad slice index");
+    Slice& sl = c->slice[t % c->nslices];
+    if (sl.t != t) return fail(c, NBS_ESTATE, "time slice not loaded");
+    if (out_bytes < c->V * BLOCK_ELEMS * sizeof(double2)) return fail(c, NBS_EINVAL, "output buffer too small");
+    CU(c, cudaSetDevice(c->device));
+    return launch_blocks(c, sl, c->d_one_baryon + baryon, 1, c->dq_mask_of[baryon], (double2*)out_dev, BLOCK_ELEMS,
+                         (cudaStream_t)stream);
+}
+
+int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_t out_bytes, int memloc, void* stream) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    const int nch = (int)c->plan.channels.size();
+    if (t < 0 || t >= c->T) return fail(c, NBS_EINVAL, "bad slice index");
+    if (ch_begin < 0 || ch_end > nch || ch_begin >= ch_end || !out) return fail(c, NBS_EINVAL, "bad channel range or NULL output");
+    if (memloc != NBS_MEM_DEVICE && memloc != NBS_MEM_HOST) return fail(c, NBS_EINVAL, "bad memloc");
+    const size_t nout = (size_t)(ch_end - ch_begin);
+    const size_t need = nout * 256 * c->V * sizeof(double2);
+    if (out_bytes < need) return fail(c, NBS_EINVAL, "output buffer too small");
+    Slice& sl = c->slice[t % c->nslices];
+    if (sl.t != t) return fail(c, NBS_ESTATE, "time slice not loaded");
+    CU(c, cudaSetDevice(c->device));
+    cudaStream_t st = (cudaStream_t)stream;
+
+    // (i) normal baryon blocks, then forward FFT in place
+    int rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
+    if (rc) return rc;
+    rc = fft3d(c, sl.B, c->R, false, st);
+    if (rc) return rc;
+    // (ii)+(iii) effective blocks and their products -> elementary correlators
+    const int nelem = (int)c->plan.elems.size();
+    dim3 grid((unsigned)c->V, (unsigned)c->plan.pairs.size());
+    k_product_v1<<<grid, PROD_THREADS, PROD_SMEM, st>>>(sl.B, c->R, c->L, c->d_pairs, c->d_elems, c->d_diagrams,
+                                                        c->d_gather, sl.E, nelem);
+    CU(c, cudaGetLastError());
+    ++c->launches;
+    k_combine<<<(unsigned)c->V, 256, 0, st>>>(sl.E, nelem, c->d_term_begin, c->d_terms, ch_begin, (int)nout, sl.Ft);
+    CU(c, cudaGetLastError());
+    ++c->launches;
+    // inverse FFT and final layout F[ch][a1 a2 a3 a4][r]
+    rc = fft3d(c, sl.Ft, nout * 256, true, st);
+    if (rc) return rc;
+    double2* dst = (double2*)out;
+    if (memloc == NBS_MEM_HOST) dst = sl.E; // E is free again: use it as the device staging buffer
+    if (memloc == NBS_MEM_HOST && (size_t)nelem < nout) return fail(c, NBS_EINVAL, "host output needs nelem >= channels");
+    dim3 tg((unsigned)((c->V + 31) / 32), (unsigned)((nout * 256 + 31) / 32));
+    k_transpose_out<<<tg, 256, 0, st>>>(sl.Ft, c->V, nout * 256, dst);
+    CU(c, cudaGetLastError());
+    ++c->launches;
+    if (memloc == NBS_MEM_HOST) CU(c, cudaMemcpyAsync(out, dst, need, cudaMemcpyDeviceToHost, st));
+    return NBS_OK;
+}
+
+void nbs_destroy(nbs_ctx* c) {
+    if (!c) return;
+    if (cudaSetDevice(c->device) == cudaSuccess) {
+        cudaDeviceSynchronize();
+        for (void* p : c->allocs) cudaFree(p);
+    }
+    delete c;
+}
+
+const char* nbs_last_error(const nbs_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+size_t nbs_workspace_bytes(const nbs_ctx* c) { return c ? c->workspace : 0; }
+int nbs_num_channels(const nbs_ctx* c) { return c ? (int)c->plan.channels.size() : NBS_EINVAL; }
+int nbs_channel_info(const nbs_ctx* c, int i, nbs_channel* out) {
+    if (!c || !out || i < 0 || i >= (int)c->plan.channels.size()) return NBS_EINVAL;
+    *out = c->plan.channels[i];
+    return NBS_OK;
+}
+
+int nbs_model_flops(const nbs_ctx* c, double* blocks, double* fft, double* product) {
+    if (!c) return NBS_EINVAL;
+    // complex multiply-add = 8 flops.  Blocks: per distinct (f0 f1 f2) tensor 432*8 + 6912*3 cMAC.
+    std::vector<int> seen;
+    for (int b : c->plan.baryons)
+        for (auto& t : block_terms(b)) {
+            int key = (t.f0 * 3 + t.f1) * 3 + t.f2;
+            bool have = false;
+            for (int k : seen) have = have || (k == key);
+            if (!have) seen.push_back(key);
+        }
+    if (blocks) *blocks = 8.0 * seen.size() * (432.0 * 8 + 6912.0 * 3);
+    double lg = std::log2((double)c->V);
+    if (fft) *fft = 5.0 * lg * ((double)c->R + 256.0 * c->plan.channels.size());
+    if (product) *product = 8.0 * 256.0 * c->plan.sumK_std;
+    return NBS_OK;
+}
+
+int nbs_exec_flops(const nbs_ctx* c, double* product_executed) {
+    if (!c) return NBS_EINVAL;
+    if (product_executed) *product_executed = 8.0 * 256.0 * c->plan.sumK_exec;
+    return NBS_OK;
+}
+
+int nbs_fft3d(nbs_ctx* c, void* data_dev, size_t R, int inverse, void* stream) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    if (!data_dev || R == 0) return fail(c, NBS_EINVAL, "NULL data or R == 0");
+    CU(c, cudaSetDevice(c->device));
+    return fft3d(c, (double2*)data_dev, R, inverse != 0, (cudaStream_t)stream);
+}
+
+long long nbs_kernel_launches(const nbs_ctx* c) { return c ? c->launches : 0; }
+
+} // extern "C"

@@ -1,0 +1,315 @@
+// sm_100a CUDA kernels of the hot path (rows a1-a5 of DESIGN.md).  Complex128 throughout.
+//
+// Data layout in HBM ("site-major"): every stage keeps all components of one lattice site (or
+// momentum q) contiguous:
+//   blocks  B[site][slot][alpha][xi1 xi2 xi3]   (row length R = nslots * 6912 complex)
+//   E       [q][elem][256]                       elementary correlators
+//   Ft      [q][ch][256]                         channel correlators in momentum space
+// so that (a) the block kernel writes one site's 110 KB per baryon fully coalesced, (b) the FFT
+// runs one 1-D transform per thread with lanes on consecutive components (coalesced, no shared
+// memory), and (c) the product kernel stages B~1(q), B~2(-q) with contiguous bulk reads.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "nbs_tables.hpp"
+
+namespace nbs {
+
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ void cfma(double2& acc, double2 a, double2 b) {
+    acc.x = fma(a.x, b.x, acc.x);
+    acc.x = fma(-a.y, b.y, acc.x);
+    acc.y = fma(a.x, b.y, acc.y);
+    acc.y = fma(a.y, b.x, acc.y);
+}
+
+// ---------------------------------------------------------------------------------------------
+// (i) NormalBaryonBlocks, eq. 4.1.  One CTA per lattice site.
+//   phase 1: diquarks D^{f0f1}_c(i,j) = sum_{ab, beta gamma} eps_abc (C g5)_{beta gamma}
+//            S_f0[(a,beta), i] S_f1[(b,gamma), j]                       -> shared memory
+//   phase 2: block[a][xi0 xi1 xi2] = sum_terms coef sum_c D_c(xi_p0, xi_p1) S_f2[(c,a), xi_p2]
+//            written straight to HBM, consecutive threads -> consecutive components.
+// ---------------------------------------------------------------------------------------------
+struct BTermRec {
+    double coef;
+    int dq, f2;
+    int p0, p1, p2, pad;
+};
+struct BlockRec {
+    int term_begin, term_end;
+};
+
+constexpr int BLOCKS_THREADS = 256;
+
+__global__ void __launch_bounds__(BLOCKS_THREADS)
+k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const double2* __restrict__ Ss,
+         const int* __restrict__ baryon_of_slot, int nslots, unsigned dq_mask,
+         const BlockRec* __restrict__ brec, const BTermRec* __restrict__ bterm,
+         double2* __restrict__ out, size_t row_stride) {
+    extern __shared__ double2 smem[];
+    double2* sS = smem;            // [3][144]
+    double2* sD = smem + 3 * 144;  // [9][3][144]
+    const size_t site = blockIdx.x;
+    const int tid = threadIdx.x;
+    for (int i = tid; i < 144; i += BLOCKS_THREADS) {
+        sS[i] = Su[site * 144 + i];
+        sS[144 + i] = Sd[site * 144 + i];
+        sS[288 + i] = Ss[site * 144 + i];
+    }
+    __syncthreads();
+    for (int idx = tid; idx < 9 * 432; idx += BLOCKS_THREADS) {
+        int dq = idx / 432;
+        if (!((dq_mask >> dq) & 1u)) continue;
+        int rem = idx - dq * 432;
+        int c = rem / 144, i = (rem / 12) % 12, j = rem % 12;
+        const double2* S0 = sS + (dq / 3) * 144;
+        const double2* S1 = sS + (dq % 3) * 144;
+        int a = (c + 1) % 3, b = (c + 2) % 3;
+        double2 acc = make_double2(0.0, 0.0), neg = make_double2(0.0, 0.0);
+        // (C g5)_{01} = +1, (C g5)_{10} = -1, (C g5)_{23} = +1, (C g5)_{32} = -1
+#pragma unroll
+        for (int pr = 0; pr < 2; ++pr) {
+            int be = 2 * pr, ga = 2 * pr + 1;
+            cfma(acc, S0[(a + 3 * be) * 12 + i], S1[(b + 3 * ga) * 12 + j]); // +eps +cg5
+            cfma(neg, S0[(a + 3 * ga) * 12 + i], S1[(b + 3 * be) * 12 + j]); // +eps -cg5
+            cfma(neg, S0[(b + 3 * be) * 12 + i], S1[(a + 3 * ga) * 12 + j]); // -eps +cg5
+            cfma(acc, S0[(b + 3 * ga) * 12 + i], S1[(a + 3 * be) * 12 + j]); // -eps -cg5
+        }
+        sD[idx] = csub(acc, neg);
+    }
+    __syncthreads();
+    double2* orow = out + site * row_stride;
+    const int total = nslots * BLOCK_ELEMS;
+    for (int idx = tid; idx < total; idx += BLOCKS_THREADS) {
+        int slot = idx / BLOCK_ELEMS;
+        int rem = idx - slot * BLOCK_ELEMS;
+        int al = rem / NTRIPLE, t = rem - al * NTRIPLE;
+        int xi[3] = {t / 144, (t / 12) % 12, t % 12};
+        BlockRec br = brec[baryon_of_slot[slot]];
+        double2 val = make_double2(0.0, 0.0);
+        for (int it = br.term_begin; it < br.term_end; ++it) {
+            BTermRec bt = bterm[it];
+            const double2* Dq = sD + bt.dq * 432 + xi[bt.p0] * 12 + xi[bt.p1];
+            const double2* S2 = sS + bt.f2 * 144 + (3 * al) * 12 + xi[bt.p2];
+            double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) cfma(acc, Dq[c * 144], S2[c * 12]);
+            val.x = fma(bt.coef, acc.x, val.x);
+            val.y = fma(bt.coef, acc.y, val.y);
+        }
+        orow[idx] = val;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// 1-D FFT along one lattice axis, one transform per thread, lanes on consecutive components
+// (rows a2 and a5; eq. 2.6).  Forward: sum_x f(x) exp(-i q x); inverse: exp(+i q x)
+// times `scale`.  tw[m] = exp(-2 pi i m / L).
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
+__host__ __device__ constexpr int bitrev(int i, int bits) {
+    int r = 0;
+    for (int b = 0; b < bits; ++b) r |= ((i >> b) & 1) << (bits - 1 - b);
+    return r;
+}
+
+template <int L, bool INV>
+__device__ __forceinline__ void fft_inreg(double2 (&a)[L], const double2* __restrict__ tw) {
+    constexpr int LOG = ilog2(L);
+#pragma unroll
+    for (int i = 0; i < L; ++i) {
+        const int j = bitrev(i, LOG);
+        if (i < j) { double2 tmp = a[i]; a[i] = a[j]; a[j] = tmp; }
+    }
+#pragma unroll
+    for (int len = 2; len <= L; len <<= 1) {
+#pragma unroll
+        for (int i = 0; i < L; i += len) {
+#pragma unroll
+            for (int k = 0; k < len / 2; ++k) {
+                double2 u = a[i + k], v = a[i + k + len / 2];
+                if (k != 0) {
+                    double2 w = __ldg(tw + k * (L / len));
+                    if (INV) w.y = -w.y;
+                    v = cmul(v, w);
+                }
+                a[i + k] = cadd(u, v);
+                a[i + k + len / 2] = csub(u, v);
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ void line_geometry(int L, int axis, int line, size_t& s0, size_t& st) {
+    int u = line % L, v = line / L;
+    if (axis == 0) { s0 = (size_t)L * (u + (size_t)L * v); st = 1; }
+    else if (axis == 1) { s0 = u + (size_t)L * L * v; st = L; }
+    else { s0 = u + (size_t)L * v; st = (size_t)L * L; }
+}
+
+constexpr int FFT_THREADS = 128;
+
+template <int L, bool INV>
+__global__ void __launch_bounds__(FFT_THREADS)
+k_fft_axis_pow2(double2* __restrict__ data, size_t R, int axis, const double2* __restrict__ tw, double scale) {
+    size_t r = (size_t)blockIdx.x * FFT_THREADS + threadIdx.x;
+    if (r >= R) return;
+    size_t s0, st;
+    line_geometry(L, axis, blockIdx.y, s0, st);
+    double2 a[L];
+#pragma unroll
+    for (int j = 0; j < L; ++j) a[j] = data[(s0 + j * st) * R + r];
+    fft_inreg<L, INV>(a, tw);
+#pragma unroll
+    for (int j = 0; j < L; ++j) {
+        double2 v = a[j];
+        if (INV) { v.x *= scale; v.y *= scale; }
+        data[(s0 + j * st) * R + r] = v;
+    }
+}
+
+constexpr int FFT_MAXL = 64;
+
+// Any L (direct O(L^2) DFT); used for lattice sizes that are not powers of two.
+template <bool INV>
+__global__ void __launch_bounds__(FFT_THREADS)
+k_fft_axis_generic(double2* __restrict__ data, size_t R, int L, int axis, const double2* __restrict__ tw, double scale) {
+    size_t r = (size_t)blockIdx.x * FFT_THREADS + threadIdx.x;
+    if (r >= R) return;
+    size_t s0, st;
+    line_geometry(L, axis, blockIdx.y, s0, st);
+    double2 a[FFT_MAXL], b[FFT_MAXL];
+    for (int j = 0; j < L; ++j) a[j] = data[(s0 + j * st) * R + r];
+    for (int k = 0; k < L; ++k) {
+        double2 acc = make_double2(0.0, 0.0);
+        int m = 0;
+        for (int j = 0; j < L; ++j) {
+            double2 w = __ldg(tw + m);
+            if (INV) w.y = -w.y;
+            cfma(acc, a[j], w);
+            m += k;
+            if (m >= L) m -= L;
+        }
+        b[k] = acc;
+    }
+    for (int j = 0; j < L; ++j) {
+        double2 v = b[j];
+        if (INV) { v.x *= scale; v.y *= scale; }
+        data[(s0 + j * st) * R + r] = v;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// (ii)+(iii) EffectiveBaryonBlocks fused into MultiplicationEffectiveBlocks, eqs. 4.2-4.3
+// (PAPER.md:104-115).  One CTA per (momentum q, sink pair): B~1(q) and B~2(-q) (2 x 110 KB) are
+// staged once in shared memory and every diagram of every elementary correlator of the pair is
+// evaluated from there; the effective blocks exist only as gathered operands, never in memory.
+// v1: one thread per output spin combination (a1 a2 a3 a4), table-driven signed gathers.
+// ---------------------------------------------------------------------------------------------
+constexpr int PROD_THREADS = 256;
+constexpr size_t PROD_SMEM = 2 * (size_t)BLOCK_ELEMS * sizeof(double2);
+
+__device__ __forceinline__ size_t minus_q(int L, size_t q) {
+    int x = (int)(q % L), y = (int)((q / L) % L), z = (int)(q / ((size_t)L * L));
+    x = x ? L - x : 0; y = y ? L - y : 0; z = z ? L - z : 0;
+    return x + (size_t)L * (y + (size_t)L * z);
+}
+
+__global__ void __launch_bounds__(PROD_THREADS)
+k_product_v1(const double2* __restrict__ Bq, size_t R, int L, const PairRec* __restrict__ pairs,
+             const ElemRec* __restrict__ elems, const DiagramRec* __restrict__ diagrams,
+             const uint16_t* __restrict__ gather, double2* __restrict__ E, int nelem) {
+    extern __shared__ double2 smem[];
+    double2* s1 = smem;
+    double2* s2 = smem + BLOCK_ELEMS;
+    const size_t q = blockIdx.x;
+    const PairRec pr = pairs[blockIdx.y];
+    const int tid = threadIdx.x;
+    {
+        const double2* g1 = Bq + q * R + (size_t)pr.slot1 * BLOCK_ELEMS;
+        const double2* g2 = Bq + minus_q(L, q) * R + (size_t)pr.slot2 * BLOCK_ELEMS;
+        for (int i = tid; i < BLOCK_ELEMS; i += PROD_THREADS) {
+            s1[i] = g1[i];
+            s2[i] = g2[i];
+        }
+    }
+    __syncthreads();
+    const int a1 = tid >> 6, a2 = (tid >> 4) & 3, a3 = (tid >> 2) & 3, a4 = tid & 3;
+    const double2* base1 = s1 + a1 * NTRIPLE;
+    const double2* base2 = s2 + a2 * NTRIPLE;
+    for (int e = pr.elem_begin; e < pr.elem_end; ++e) {
+        const ElemRec er = elems[e];
+        double2 acc = make_double2(0.0, 0.0);
+        for (int d = er.diag_begin; d < er.diag_end; ++d) {
+            const DiagramRec dr = diagrams[d];
+            int c1, c2;
+            switch (dr.mask1) {
+            case 3: c1 = a3 * 4 + a4; c2 = 0; break;
+            case 1: c1 = a3; c2 = a4; break;
+            case 2: c1 = a4; c2 = a3; break;
+            default: c1 = 0; c2 = a3 * 4 + a4; break;
+            }
+            const int K = dr.K, n1 = dr.n1, n2 = dr.n2;
+            const uint16_t* p1 = gather + dr.off1 + (size_t)c1 * K * n1;
+            const uint16_t* p2 = gather + dr.off2 + (size_t)c2 * K * n2;
+            for (int k = 0; k < K; ++k) {
+                double2 x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
+                for (int j = 0; j < n1; ++j) {
+                    unsigned g = p1[k * n1 + j];
+                    double2 v = base1[g & 0x7ff];
+                    x = (g & 0x8000) ? csub(x, v) : cadd(x, v);
+                }
+                for (int j = 0; j < n2; ++j) {
+                    unsigned g = p2[k * n2 + j];
+                    double2 v = base2[g & 0x7ff];
+                    y = (g & 0x8000) ? csub(y, v) : cadd(y, v);
+                }
+                cfma(acc, x, y);
+            }
+        }
+        E[(q * nelem + e) * 256 + tid] = acc;
+    }
+}
+
+// Channel correlator = sum over its elementary source terms (Lambda, Sigma0 expanded into
+// X_u, X_d, X_s; eqs. 2.2-2.3): Ft[q][ch][o] = sum_terms coef * E[q][elem][o].
+__global__ void __launch_bounds__(256)
+k_combine(const double2* __restrict__ E, int nelem, const int* __restrict__ term_begin,
+          const ChanTermRec* __restrict__ terms, int ch_begin, int nch_out, double2* __restrict__ Ft) {
+    const size_t q = blockIdx.x;
+    const int o = threadIdx.x;
+    for (int c = 0; c < nch_out; ++c) {
+        double2 acc = make_double2(0.0, 0.0);
+        for (int it = term_begin[ch_begin + c]; it < term_begin[ch_begin + c + 1]; ++it) {
+            ChanTermRec t = terms[it];
+            double2 v = E[(q * nelem + t.elem) * 256 + o];
+            acc.x = fma(t.coef, v.x, acc.x);
+            acc.y = fma(t.coef, v.y, acc.y);
+        }
+        Ft[(q * nch_out + c) * 256 + o] = acc;
+    }
+}
+
+// Final layout change: Fr[r][comp] (site-major) -> out[comp][r] (r fastest), 32x32 tiles.
+__global__ void __launch_bounds__(256)
+k_transpose_out(const double2* __restrict__ Fr, size_t V, size_t ncomp, double2* __restrict__ out) {
+    __shared__ double2 tile[32][33];
+    const size_t r0 = (size_t)blockIdx.x * 32, c0 = (size_t)blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int i = ty; i < 32; i += 8) {
+        size_t r = r0 + i, c = c0 + tx;
+        if (r < V && c < ncomp) tile[i][tx] = Fr[r * ncomp + c];
+    }
+    __syncthreads();
+    for (int i = ty; i < 32; i += 8) {
+        size_t c = c0 + i, r = r0 + tx;
+        if (r < V && c < ncomp) out[c * V + r] = tile[tx][i];
+    }
+}
+
+} // namespace nbs

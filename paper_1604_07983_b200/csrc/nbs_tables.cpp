@@ -1,0 +1,407 @@
+// Host table generator: channels -> sink pairs -> elementary correlators -> diagrams -> gather tables.
+// Follows PAPER.md:45 (eq. 2.4), :57 (coset count), :67 (effective-block term count), :104-115
+// (eqs. 4.2, 4.3) and the readings A1-A10 of DESIGN.md.  No code shared with oracle/.
+#include "nbs_tables.hpp"
+
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <map>
+
+namespace nbs {
+
+namespace {
+
+enum { U = 0, D = 1, S = 2 };
+
+const double kS6 = 1.0 / std::sqrt(6.0);
+const double kS2 = 1.0 / std::sqrt(2.0);
+
+// eqs. 2.2-2.3 verbatim.  Block slot order: the operator's own field order for the octet members
+// made of one elementary operator, (u, d, s) for Lambda, Sigma0 and the X's.
+const BaryonDef kBaryons[NBS_NUM_BARYONS] = {
+    /* p   */ {{U, D, U}, 1, {{+1.0, {U, D, U}}}},
+    /* n   */ {{U, D, D}, 1, {{-1.0, {U, D, D}}}},
+    /* L   */ {{U, D, S}, 3, {{kS6, {D, S, U}}, {kS6, {S, U, D}}, {-2.0 * kS6, {U, D, S}}}},
+    /* S+  */ {{U, S, U}, 1, {{-1.0, {U, S, U}}}},
+    /* S0  */ {{U, D, S}, 2, {{kS2, {D, S, U}}, {-kS2, {S, U, D}}}},
+    /* S-  */ {{D, S, D}, 1, {{-1.0, {D, S, D}}}},
+    /* X0  */ {{U, S, S}, 1, {{+1.0, {U, S, S}}}},
+    /* X-  */ {{D, S, S}, 1, {{-1.0, {D, S, S}}}},
+    /* Xu  */ {{U, D, S}, 1, {{+1.0, {D, S, U}}}},
+    /* Xd  */ {{U, D, S}, 1, {{+1.0, {S, U, D}}}},
+    /* Xs  */ {{U, D, S}, 1, {{+1.0, {U, D, S}}}},
+};
+
+int parity(const int* p, int n) {
+    int inv = 0;
+    for (int i = 0; i < n; ++i)
+        for (int j = i + 1; j < n; ++j)
+            if (p[i] > p[j]) ++inv;
+    return (inv & 1) ? -1 : 1;
+}
+
+// Non-zeros of W[xi1 xi2 xi3; a] = eps_{c1c2c3} (C g5)_{a1a2} delta_{a3 a}  (reading A1 for C g5).
+struct WEntry {
+    int xi[3];
+    int c[3];
+    int a; // a3 = carried spin
+    int sign;
+};
+std::vector<WEntry> w_nonzeros() {
+    static const int cg5[4][3] = {{0, 1, +1}, {1, 0, -1}, {2, 3, +1}, {3, 2, -1}}; // (a1, a2, value)
+    std::vector<WEntry> out;
+    int c[3] = {0, 1, 2};
+    do {
+        int eps = parity(c, 3);
+        for (auto& g : cg5)
+            for (int a = 0; a < 4; ++a) {
+                WEntry e;
+                e.c[0] = c[0]; e.c[1] = c[1]; e.c[2] = c[2];
+                e.xi[0] = c[0] + 3 * g[0];
+                e.xi[1] = c[1] + 3 * g[1];
+                e.xi[2] = c[2] + 3 * a;
+                e.a = a;
+                e.sign = eps * g[2];
+                out.push_back(e);
+            }
+    } while (std::next_permutation(c, c + 3));
+    return out;
+}
+
+// The factor of W that belongs to the sink baryon holding source positions `mask` (bit p-1 set
+// <=> position p).  W = sum_shared factor(mask) * factor(7 ^ mask).
+struct FactorEntry {
+    int xi[3];  // value for each position held (-1 otherwise)
+    int shared; // value of the shared index
+    int carry;  // carried source spin (0 if this side does not hold position 3)
+    int sign;
+};
+struct Factor {
+    int nshared, ncarry;
+    std::vector<FactorEntry> e;
+};
+Factor make_factor(int mask) {
+    static const std::vector<WEntry> wnz = w_nonzeros();
+    Factor f;
+    f.ncarry = (mask & 4) ? 4 : 1;
+    auto blank = [] { FactorEntry e; e.xi[0] = e.xi[1] = e.xi[2] = -1; e.shared = 0; e.carry = 0; e.sign = 1; return e; };
+    switch (mask) {
+    case 0:
+        f.nshared = 1;
+        f.e.push_back(blank());
+        break;
+    case 7: // whole source baryon on this side: full W, nothing shared
+        f.nshared = 1;
+        for (auto& w : wnz) {
+            FactorEntry e = blank();
+            e.xi[0] = w.xi[0]; e.xi[1] = w.xi[1]; e.xi[2] = w.xi[2];
+            e.carry = w.a; e.sign = w.sign;
+            f.e.push_back(e);
+        }
+        break;
+    case 3: // the C g5 pair {1,2}: eps_{c1 c2 c} (C g5)_{a1 a2}, open colour c
+        f.nshared = 3;
+        for (auto& w : wnz) {
+            if (w.a != 0) continue; // the delta on a3 belongs to the other side
+            FactorEntry e = blank();
+            e.xi[0] = w.xi[0]; e.xi[1] = w.xi[1];
+            e.shared = w.c[2]; e.sign = w.sign;
+            f.e.push_back(e);
+        }
+        break;
+    case 4: // quark 3 alone: read at xi3 = (c, a), carries a
+        f.nshared = 3;
+        for (int c = 0; c < 3; ++c)
+            for (int a = 0; a < 4; ++a) {
+                FactorEntry e = blank();
+                e.xi[2] = c + 3 * a; e.shared = c; e.carry = a;
+                f.e.push_back(e);
+            }
+        break;
+    case 5: // {1,3}: W with the partner index xi2 left open
+    case 6: // {2,3}: W with the partner index xi1 left open
+    {
+        int open = (mask == 5) ? 1 : 0;
+        f.nshared = NXI;
+        for (auto& w : wnz) {
+            FactorEntry e = blank();
+            for (int p = 0; p < 3; ++p)
+                if (p != open) e.xi[p] = w.xi[p];
+            e.shared = w.xi[open]; e.carry = w.a; e.sign = w.sign;
+            f.e.push_back(e);
+        }
+        break;
+    }
+    case 1: // lone C g5 partner: raw read at the shared index
+    case 2: {
+        int pos = (mask == 1) ? 0 : 1;
+        f.nshared = NXI;
+        for (int s = 0; s < NXI; ++s) {
+            FactorEntry e = blank();
+            e.xi[pos] = s; e.shared = s;
+            f.e.push_back(e);
+        }
+        break;
+    }
+    }
+    return f;
+}
+const Factor& factor(int mask) {
+    static const std::array<Factor, 8> all = [] {
+        std::array<Factor, 8> a;
+        for (int m = 0; m < 8; ++m) a[m] = make_factor(m);
+        return a;
+    }();
+    return all[mask];
+}
+
+// Gather table of one side of one diagram (eq. 4.2): slots[m] = source quark (0..5) in slot m.
+struct SideTable {
+    int C, K, n;
+    int carries; // bit0: a3, bit1: a4
+    std::vector<uint16_t> g;
+};
+SideTable make_side(const int* slots, int overall_sign) {
+    int mask[2] = {0, 0};
+    for (int m = 0; m < 3; ++m) mask[slots[m] / 3] |= 1 << (slots[m] % 3);
+    const Factor& f0 = factor(mask[0]);
+    const Factor& f1 = factor(mask[1]);
+    SideTable t;
+    t.C = f0.ncarry * f1.ncarry;
+    t.K = f0.nshared * f1.nshared;
+    t.carries = ((mask[0] & 4) ? 1 : 0) | ((mask[1] & 4) ? 2 : 0);
+    size_t nent = (size_t)t.C * t.K;
+    t.n = (int)(f0.e.size() * f1.e.size() / nent);
+    std::vector<int> fill(nent, 0);
+    t.g.assign(nent * t.n, 0);
+    for (auto& e0 : f0.e)
+        for (auto& e1 : f1.e) {
+            int xi[3];
+            for (int m = 0; m < 3; ++m) {
+                int q = slots[m];
+                xi[m] = (q / 3 == 0 ? e0 : e1).xi[q % 3];
+            }
+            int tri = (xi[0] * NXI + xi[1]) * NXI + xi[2];
+            int c = e0.carry * f1.ncarry + e1.carry;
+            int k = e0.shared * f1.nshared + e1.shared;
+            int sign = e0.sign * e1.sign * overall_sign;
+            size_t ent = (size_t)c * t.K + k;
+            t.g[ent * t.n + fill[ent]++] = (uint16_t)(tri | (sign < 0 ? 0x8000 : 0));
+        }
+    return t;
+}
+
+struct RawDiagram {
+    int P[6];
+    int sign;
+    double coef;
+    int h[6]; // flavours of the six source quarks
+};
+
+std::string enumerate(const nbs_channel& ch, std::vector<RawDiagram>& out) {
+    const int ids[4] = {ch.b1, ch.b2, ch.b3, ch.b4};
+    for (int id : ids)
+        if (id < 0 || id >= NBS_NUM_BARYONS) return "unknown baryon id";
+    const BaryonDef &B1 = kBaryons[ch.b1], &B2 = kBaryons[ch.b2], &B3 = kBaryons[ch.b3], &B4 = kBaryons[ch.b4];
+    int g[6];
+    for (int j = 0; j < 3; ++j) { g[j] = B1.slot[j]; g[3 + j] = B2.slot[j]; }
+    for (int i3 = 0; i3 < B3.nterm; ++i3)
+        for (int i4 = 0; i4 < B4.nterm; ++i4) {
+            RawDiagram d;
+            for (int j = 0; j < 3; ++j) { d.h[j] = B3.term[i3].f[j]; d.h[3 + j] = B4.term[i4].f[j]; }
+            d.coef = B3.term[i3].coef * B4.term[i4].coef;
+            int P[6] = {0, 1, 2, 3, 4, 5};
+            do {
+                bool ok = true;
+                for (int j = 0; j < 6 && ok; ++j) ok = (g[j] == d.h[P[j]]);
+                // one representative per coset modulo exchange of same-flavour slots inside one
+                // sink baryon (the block is antisymmetric there): the paper's 2^{N_L+N_S0-B}
+                for (int base = 0; base < 6 && ok; base += 3)
+                    for (int j = base; j < base + 3 && ok; ++j)
+                        for (int k = j + 1; k < base + 3 && ok; ++k)
+                            if (g[j] == g[k] && P[j] > P[k]) ok = false;
+                if (!ok) continue;
+                for (int j = 0; j < 6; ++j) d.P[j] = P[j];
+                d.sign = parity(P, 6);
+                out.push_back(d);
+            } while (std::next_permutation(P, P + 6));
+        }
+    if (out.empty()) return "channel violates flavour conservation (F vanishes identically)";
+    return "";
+}
+
+int diagram_K(const int* P) {
+    int mask[2] = {0, 0};
+    for (int m = 0; m < 3; ++m) mask[P[m] / 3] |= 1 << (P[m] % 3);
+    return factor(mask[0]).nshared * factor(mask[1]).nshared;
+}
+
+} // namespace
+
+const BaryonDef& baryon_def(int id) { return kBaryons[id]; }
+
+std::vector<BlockTerm> block_terms(int baryon) {
+    const BaryonDef& B = kBaryons[baryon];
+    std::vector<BlockTerm> out;
+    for (int i = 0; i < B.nterm; ++i) {
+        int sig[3] = {0, 1, 2};
+        do { // Wick pairings: field j -> slot sig[j] of the same flavour, sign sgn(sig)
+            bool ok = true;
+            for (int j = 0; j < 3; ++j) ok = ok && (B.term[i].f[j] == B.slot[sig[j]]);
+            if (!ok) continue;
+            BlockTerm t;
+            t.coef = B.term[i].coef * parity(sig, 3);
+            t.f0 = B.term[i].f[0]; t.f1 = B.term[i].f[1]; t.f2 = B.term[i].f[2];
+            for (int j = 0; j < 3; ++j) t.perm[j] = sig[j];
+            out.push_back(t);
+        } while (std::next_permutation(sig, sig + 3));
+    }
+    return out;
+}
+
+std::vector<nbs_channel> standard_channels() {
+    // Reading A10: sectors of fixed strangeness and charge, all sink x source pairs inside a
+    // sector except the four isospin-forbidden LL <-> S0L and S0S0 <-> S0L.
+    typedef std::pair<int, int> St;
+    const std::vector<std::vector<St>> sectors = {
+        {{NBS_P, NBS_N}},
+        {{NBS_P, NBS_LAMBDA}, {NBS_SIGMA_P, NBS_N}, {NBS_SIGMA_0, NBS_P}},
+        {{NBS_LAMBDA, NBS_LAMBDA}, {NBS_P, NBS_XI_M}, {NBS_N, NBS_XI_0}, {NBS_SIGMA_P, NBS_SIGMA_M},
+         {NBS_SIGMA_0, NBS_SIGMA_0}, {NBS_SIGMA_0, NBS_LAMBDA}},
+        {{NBS_XI_M, NBS_LAMBDA}, {NBS_SIGMA_M, NBS_XI_0}, {NBS_SIGMA_0, NBS_XI_M}},
+        {{NBS_XI_M, NBS_XI_0}},
+    };
+    const St LL{NBS_LAMBDA, NBS_LAMBDA}, S0L{NBS_SIGMA_0, NBS_LAMBDA}, S0S0{NBS_SIGMA_0, NBS_SIGMA_0};
+    std::vector<nbs_channel> out;
+    for (auto& sec : sectors)
+        for (auto& snk : sec)
+            for (auto& src : sec) {
+                bool forbidden = (snk == S0L && (src == LL || src == S0S0)) || (src == S0L && (snk == LL || snk == S0S0));
+                if (forbidden) continue;
+                out.push_back(nbs_channel{snk.first, snk.second, src.first, src.second});
+            }
+    return out;
+}
+
+std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& out) {
+    std::vector<RawDiagram> raw;
+    std::string err = enumerate(ch, raw);
+    if (!err.empty()) return err;
+    for (auto& d : raw) {
+        DiagramInfo di;
+        for (int j = 0; j < 6; ++j) di.P[j] = d.P[j];
+        di.sign = d.sign;
+        di.K = diagram_K(d.P);
+        out.push_back(di);
+    }
+    return "";
+}
+
+std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan) {
+    plan = Plan();
+    plan.channels = channels;
+    if (channels.empty()) return "empty channel list";
+
+    // sink pairs in order of first appearance; needed baryon blocks
+    std::map<std::pair<int, int>, int> pair_index;
+    std::vector<std::pair<int, int>> pair_list;
+    std::map<int, int> slot_of;
+    auto slot = [&](int b) {
+        auto it = slot_of.find(b);
+        if (it != slot_of.end()) return it->second;
+        int s = (int)plan.baryons.size();
+        plan.baryons.push_back(b);
+        slot_of[b] = s;
+        return s;
+    };
+    // elementary correlators per pair, keyed by the six source flavours
+    typedef std::array<int, 6> Key;
+    std::vector<std::map<Key, std::vector<RawDiagram>>> pair_elems;
+    std::vector<std::vector<Key>> pair_elem_order;
+    struct CT { int pair; Key key; double coef; };
+    std::vector<std::vector<CT>> chan_ct(channels.size());
+
+    for (size_t ic = 0; ic < channels.size(); ++ic) {
+        const nbs_channel& ch = channels[ic];
+        std::vector<RawDiagram> raw;
+        std::string err = enumerate(ch, raw);
+        if (!err.empty()) return "channel " + std::to_string(ic) + ": " + err;
+        auto pk = std::make_pair(ch.b1, ch.b2);
+        int ip;
+        if (!pair_index.count(pk)) {
+            ip = (int)pair_list.size();
+            pair_index[pk] = ip;
+            pair_list.push_back(pk);
+            pair_elems.emplace_back();
+            pair_elem_order.emplace_back();
+            slot(ch.b1); slot(ch.b2);
+        } else ip = pair_index[pk];
+        plan.chan_pair.push_back(ip);
+        std::map<Key, std::vector<RawDiagram>> mine;
+        std::vector<Key> order;
+        for (auto& d : raw) {
+            Key k; for (int j = 0; j < 6; ++j) k[j] = d.h[j];
+            if (!mine.count(k)) order.push_back(k);
+            mine[k].push_back(d);
+            plan.sumK_std += diagram_K(d.P);
+        }
+        for (auto& k : order) {
+            if (!pair_elems[ip].count(k)) {
+                pair_elems[ip][k] = mine[k];
+                pair_elem_order[ip].push_back(k);
+            }
+            chan_ct[ic].push_back(CT{ip, k, mine[k][0].coef});
+        }
+    }
+
+    // flatten: pairs -> elems -> diagrams -> gather tables (deduplicated by content)
+    std::map<std::vector<uint16_t>, uint32_t> dedupe;
+    auto intern = [&](const std::vector<uint16_t>& g) {
+        auto it = dedupe.find(g);
+        if (it != dedupe.end()) return it->second;
+        uint32_t off = (uint32_t)plan.gather.size();
+        plan.gather.insert(plan.gather.end(), g.begin(), g.end());
+        while (plan.gather.size() % 8) plan.gather.push_back(0); // 16-byte aligned tables
+        dedupe[g] = off;
+        return off;
+    };
+    std::vector<std::map<Key, int>> elem_id(pair_list.size());
+    for (size_t ip = 0; ip < pair_list.size(); ++ip) {
+        PairRec pr;
+        pr.slot1 = slot_of[pair_list[ip].first];
+        pr.slot2 = slot_of[pair_list[ip].second];
+        pr.elem_begin = (int)plan.elems.size();
+        for (auto& k : pair_elem_order[ip]) {
+            ElemRec er;
+            er.diag_begin = (int)plan.diagrams.size();
+            for (auto& d : pair_elems[ip][k]) {
+                SideTable s1 = make_side(d.P, d.sign); // sigma_P folded into side 1
+                SideTable s2 = make_side(d.P + 3, +1);
+                DiagramRec r;
+                r.off1 = intern(s1.g); r.off2 = intern(s2.g);
+                r.K = (uint16_t)s1.K;
+                r.n1 = (uint8_t)s1.n; r.n2 = (uint8_t)s2.n;
+                r.C1 = (uint8_t)s1.C; r.C2 = (uint8_t)s2.C;
+                r.mask1 = (uint8_t)s1.carries;
+                r.pad = 0;
+                if (s1.K != s2.K || (s1.carries ^ s2.carries) != 3) return "internal: inconsistent cut";
+                plan.diagrams.push_back(r);
+                plan.sumK_exec += s1.K;
+            }
+            er.diag_end = (int)plan.diagrams.size();
+            elem_id[ip][k] = (int)plan.elems.size();
+            plan.elems.push_back(er);
+        }
+        pr.elem_end = (int)plan.elems.size();
+        plan.pairs.push_back(pr);
+    }
+    plan.chan_term_begin.push_back(0);
+    for (size_t ic = 0; ic < channels.size(); ++ic) {
+        for (auto& ct : chan_ct[ic]) plan.chan_terms.push_back(ChanTermRec{elem_id[ct.pair][ct.key], ct.coef});
+        plan.chan_term_begin.push_back((int)plan.chan_terms.size());
+    }
+    return "";
+}
+
+} // namespace nbs

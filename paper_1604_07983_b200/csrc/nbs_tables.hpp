@@ -1,0 +1,88 @@
+// Host table generator (row a0 of DESIGN.md): the paper's CPU-side "diagramatical classification"
+// whose Structure-of-Arrays result is copied to the device before the kernels run
+// (PAPER.md:108, :115).  Pure host C++, no CUDA; shares no code with oracle/.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/nbs.h"
+
+namespace nbs {
+
+constexpr int NXI = 12;           // colour x spin
+constexpr int NTRIPLE = 1728;     // 12^3 source index triples of a normal block
+constexpr int BLOCK_ELEMS = 6912; // 4 sink spins x 12^3
+
+// One elementary operator  eps_abc (q_f0,a  C g5  q_f1,b) q_f2,c  with a real coefficient
+// (eqs. 2.2-2.3).  Flavours: 0 = u, 1 = d, 2 = s.
+struct ElemTerm {
+    double coef;
+    int f[3];
+};
+struct BaryonDef {
+    int slot[3]; // flavour of the three source quarks the block is contracted with (eq. 2.5)
+    int nterm;
+    ElemTerm term[3];
+};
+const BaryonDef& baryon_def(int id);
+
+// One term of a normal block (eq. 2.5):
+//   out[a][xi0,xi1,xi2] += coef * sum_c D^{f0 f1}_c(xi_{perm0}, xi_{perm1}) S_{f2}[(c,a), xi_{perm2}]
+struct BlockTerm {
+    double coef;
+    int f0, f1, f2;
+    int perm[3];
+};
+std::vector<BlockTerm> block_terms(int baryon);
+
+// Device-side records (plain old data, copied verbatim).
+struct DiagramRec {
+    uint32_t off1, off2; // offsets (in uint16 units) of the two gather tables
+    uint16_t K;          // size of the shared index xi~_d (1, 9, 36, 144)
+    uint8_t n1, n2;      // gather terms per effective-block entry, side 1 / side 2
+    uint8_t C1, C2;      // number of carried source-spin combinations, side 1 / side 2 (C1*C2 = 16)
+    uint8_t mask1;       // bit0: side 1 carries a3; bit1: side 1 carries a4
+    uint8_t pad;
+};
+struct ElemRec {
+    int diag_begin, diag_end; // range in the diagram array
+};
+struct PairRec {
+    int slot1, slot2;         // block slots (index into the context's list of needed baryons)
+    int elem_begin, elem_end; // range in the elementary-correlator array
+};
+struct ChanTermRec {
+    int elem; // global elementary-correlator index
+    double coef;
+};
+
+struct DiagramInfo { // host-side description (tests, statistics)
+    int P[6];
+    int sign;
+    int K;
+};
+
+struct Plan {
+    std::vector<nbs_channel> channels;
+    std::vector<int> baryons; // needed sink baryon ids, slot order
+    std::vector<PairRec> pairs;
+    std::vector<ElemRec> elems;
+    std::vector<DiagramRec> diagrams;
+    std::vector<uint16_t> gather; // bit 15: minus sign; bits 0-10: triple index t
+    std::vector<int> chan_term_begin; // size nch+1
+    std::vector<ChanTermRec> chan_terms;
+    std::vector<int> chan_pair; // pair index of each channel
+    double sumK_std = 0;        // sum over channels of sum_d K_d (the paper's count)
+    double sumK_exec = 0;       // sum over distinct elementary correlators
+};
+
+// Returns "" on success, else an error message (invalid id, flavour violation).
+std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan);
+
+// Diagrams of one channel in enumeration order (source terms major, permutations lexicographic).
+std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& out);
+
+std::vector<nbs_channel> standard_channels();
+
+} // namespace nbs

@@ -1,0 +1,223 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Bar (BASELINE.json north_star; reading A13): per channel,
+    max_{a1..a4, r} |F_gpu - F_oracle|  <=  1e-10 * max_{a1..a4, r} |F_oracle|.
+"""
+import numpy as np
+import pytest
+
+from paper_1604_07983_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests need a B200")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def nbs():
+    from paper_1604_07983_b200 import nbs as m
+    return m
+
+
+def props(L, seed=21, t=0, masses=(0.20, 0.21, 0.30), same=()):
+    S = {f: synth.propagator(seed, i, t, L, masses[i]) for i, f in enumerate("uds")}
+    for a, b in same:
+        S[a] = S[b]
+    return S
+
+
+def to_dev(torch, S):
+    cache = {}
+    out = {}
+    for f in "uds":
+        key = id(S[f])
+        if key not in cache:
+            cache[key] = torch.from_numpy(S[f]).cuda()
+        out[f] = cache[key]
+    return out
+
+
+def assert_parity(F_gpu, F_or, chans, scale=None):
+    F_gpu = np.asarray(F_gpu)
+    assert F_gpu.shape == F_or.shape
+    for i, ch in enumerate(chans):
+        ref = np.abs(F_or[i]).max() if scale is None else scale
+        assert ref > 0
+        err = np.abs(F_gpu[i] - F_or[i]).max() / ref
+        assert err <= RTOL, (i, ch, err)
+
+
+def run_gpu(torch, nbs, L, S, chans=None, t=0, T=1):
+    with nbs.Nbs(L, T, chans) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(t, d["u"], d["d"], d["s"])
+        F = ctx.correlator(t)
+        torch.cuda.synchronize()
+        return F.cpu().numpy()
+
+
+# ------------------------------------------------------------------------------ row a1: blocks
+@pytest.mark.parametrize("L", [2, 3])
+def test_normal_blocks_match_oracle(torch_cuda, nbs, oracle, L):
+    """eq. 2.5 / 4.1 for all eleven interpolating fields, u != d != s."""
+    S = props(L, seed=5)
+    with nbs.Nbs(L, 1, [("p", "n", "p", "n")]) as ctx:
+        d = to_dev(torch_cuda, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        for name in oracle.BARYONS:
+            got = ctx.blocks_x(0, name).cpu().numpy()
+            ref = oracle.block(S, name)
+            assert np.abs(got - ref).max() <= RTOL * np.abs(ref).max(), name
+
+
+# ------------------------------------------------------------------------------ rows a2, a5: FFT
+@pytest.mark.parametrize("L", [2, 4, 6, 8, 12, 16, 32])
+def test_fft3d_matches_numpy(torch_cuda, nbs, L):
+    """B~(q) = sum_x B(x) exp(-i q.x) and its inverse (eq. 2.6), ragged component count."""
+    torch = torch_cuda
+    R = 37 if L < 32 else 5
+    rng = np.random.default_rng(L)
+    a = rng.standard_normal((L, L, L, R)) + 1j * rng.standard_normal((L, L, L, R))  # [z][y][x][R]
+    with nbs.Nbs(L, 1, [("p", "n", "p", "n")]) as ctx:
+        x = torch.from_numpy(a.reshape(L ** 3, R).copy()).cuda()
+        ctx.fft3d(x)
+        ref = np.fft.fftn(a, axes=(0, 1, 2)).reshape(L ** 3, R)
+        assert np.abs(x.cpu().numpy() - ref).max() <= 1e-12 * np.abs(ref).max()
+        ctx.fft3d(x, inverse=True)
+        assert np.abs(x.cpu().numpy() - a.reshape(L ** 3, R)).max() <= 1e-13 * np.abs(a).max()
+
+
+# ------------------------------------------------------------------------------ whole path
+def test_config0_4cubed_NN(torch_cuda, nbs, oracle):
+    """BASELINE.json configs[0]: 4^3 x 1, NN channel, u = d, seed 0.  Against tier B (all r) and
+    against tier A, eq. 2.4 with the direct X-sum, at a few r."""
+    cfg = synth.CONFIGS[0]
+    S = synth.config_slice(cfg, 0)
+    assert S["d"] is S["u"]
+    ch = [("p", "n", "p", "n")]
+    F = run_gpu(torch_cuda, nbs, 4, S, ch)
+    B = oracle.all_blocks(S, ["p", "n"])
+    assert_parity(F, oracle.correlator_fft(4, B, ch), ch)
+    rs = [0, 1, 7, 63]
+    Fd = oracle.correlator_direct(4, B, ch[0], rs=rs)
+    assert np.abs(F[0][..., rs] - Fd[..., rs]).max() <= RTOL * np.abs(Fd).max()
+
+
+def test_all_52_channels_4cubed(torch_cuda, nbs, oracle):
+    """All 52 channels, non-degenerate u, d, s (the flavour structure of configs[2])."""
+    S = props(4, seed=3)
+    chans = oracle.channels52()
+    F = run_gpu(torch_cuda, nbs, 4, S)
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(4, B, chans), chans)
+
+
+def test_all_52_channels_time_slice_scale(torch_cuda, nbs, oracle):
+    """Late time slice: entries ~ exp(-m t), F ~ 1e-28; the bar is relative per channel (A13)."""
+    S = props(2, seed=3, t=63)
+    chans = oracle.channels52()
+    F = run_gpu(torch_cuda, nbs, 2, S, t=63, T=64)
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    Fo = oracle.correlator_fft(2, B, chans)
+    assert np.abs(Fo).max() < 1e-25
+    assert_parity(F, Fo, chans)
+
+
+@pytest.mark.parametrize("L", [3, 6])
+def test_non_power_of_two_lattice(torch_cuda, nbs, oracle, L):
+    """Ragged sizes: L = 3, 6 take the mixed-radix / generic FFT path."""
+    S = props(L, seed=9, same=(("d", "u"),))
+    chans = [("p", "n", "p", "n"), ("p", "L", "S0", "p"), ("L", "L", "S0", "S0"), ("Xm", "X0", "Xm", "X0")]
+    F = run_gpu(torch_cuda, nbs, L, S, chans)
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
+
+
+def test_user_channels_elementary_and_identical(torch_cuda, nbs, oracle):
+    """Channels outside the 52: <p Lambda | p X_u> (eq. 2.7), pp, nn, Sigma+ Xi0."""
+    S = props(2, seed=13)
+    chans = [("p", "L", "p", "Xu"), ("p", "p", "p", "p"), ("n", "n", "n", "n"), ("Sp", "X0", "Sp", "X0"),
+             ("Xu", "Xs", "Xd", "Xs")]
+    F = run_gpu(torch_cuda, nbs, 2, S, chans)
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(2, B, chans), chans)
+
+
+def test_vanishing_channel_uses_pair_scale(torch_cuda, nbs, oracle):
+    """u = d: the isospin-forbidden Lambda Lambda <- Sigma0 Lambda vanishes; the GPU result must be
+    zero on the scale of the other channels of the same sink pair (reading A13)."""
+    S = props(2, seed=4, same=(("d", "u"),))
+    chans = [("L", "L", "L", "L"), ("L", "L", "S0", "L")]
+    F = run_gpu(torch_cuda, nbs, 2, S, chans)
+    scale = np.abs(F[0]).max()
+    assert np.abs(F[1]).max() <= 1e-10 * scale
+
+
+def test_channel_range_and_host_buffers(torch_cuda, nbs):
+    """nbs_correlator's channel range, and host-memory input / output, give the same numbers."""
+    torch = torch_cuda
+    L = 4
+    S = props(L, seed=8)
+    full = run_gpu(torch, nbs, L, S)
+    with nbs.Nbs(L, 1) as ctx:
+        ctx.load(0, S["u"], S["d"], S["s"])  # numpy arrays: NBS_MEM_HOST
+        part = ctx.correlator(0, 7, 19)
+        host = np.empty((5, 4, 4, 4, 4, L ** 3), dtype=np.complex128)
+        ctx.correlator(0, 47, 52, out=host)
+        torch.cuda.synchronize()
+    assert np.array_equal(part.cpu().numpy(), full[7:19])
+    assert np.array_equal(host, full[47:52])
+
+
+def test_two_slices_in_flight_on_two_streams(torch_cuda, nbs):
+    """Row a6: slices t and t+1 pipelined on two CUDA streams equal the serial results bit for bit."""
+    torch = torch_cuda
+    L = 4
+    chans = [("p", "n", "p", "n"), ("L", "L", "L", "L"), ("Xm", "L", "S0", "Xm")]
+    Ss = [props(L, seed=30, t=t) for t in range(4)]
+    serial = [run_gpu(torch, nbs, L, Ss[t], chans, t=t, T=4) for t in range(4)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    with nbs.Nbs(L, 4, chans) as ctx:
+        outs = []
+        devs = [to_dev(torch, S) for S in Ss]
+        torch.cuda.synchronize()
+        for t in range(4):
+            st = streams[t % 2]
+            ctx.load(t, devs[t]["u"], devs[t]["d"], devs[t]["s"], stream=st)
+            outs.append(ctx.correlator(t, stream=st))
+        torch.cuda.synchronize()
+        for t in range(4):
+            assert np.array_equal(outs[t].cpu().numpy(), serial[t]), t
+
+
+def test_errors(torch_cuda, nbs):
+    with pytest.raises(nbs.NbsError) as e:
+        nbs.Nbs(1, 1)
+    assert e.value.code == nbs.NBS_EINVAL
+    with pytest.raises(nbs.NbsError) as e:
+        nbs.Nbs(4, 1, [("p", "n", "p", "p")])
+    assert e.value.code == nbs.NBS_EINVAL
+    with nbs.Nbs(2, 2) as ctx:
+        with pytest.raises(nbs.NbsError) as e:
+            ctx.correlator(0)
+        assert e.value.code == nbs.NBS_ESTATE
+        S = to_dev(torch_cuda, props(2))
+        ctx.load(0, S["u"], S["d"], S["s"])
+        with pytest.raises(nbs.NbsError) as e:
+            ctx.correlator(0, 5, 5)
+        assert e.value.code == nbs.NBS_EINVAL
+        with pytest.raises(nbs.NbsError) as e:
+            ctx.correlator(0, 0, 53)
+        assert e.value.code == nbs.NBS_EINVAL
+        small = torch_cuda.empty(10, dtype=torch_cuda.complex128, device="cuda")
+        with pytest.raises(nbs.NbsError) as e:
+            ctx.correlator(0, 0, 52, out=small)
+        assert e.value.code == nbs.NBS_EINVAL
