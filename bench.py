@@ -1,0 +1,298 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement (BASELINE.json `metric`): 52-channel NBS correlator
+time-slices/s at 32^3 x 64 in FP64 on one B200, with the dominant kernel's roofline fraction.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+A "step" is one pass of the whole hot path (blocks -> FFT -> effective blocks x product -> inverse
+FFT -> F[52][256][V]) over one time slice of synthetic propagators of BASELINE.json configs[2]
+(32^3 x 64, u != d != s, Gaussian entries x exp(-m t), seed 3).  N > 1: "replicas only" -- time
+slices are independent (T-parallel), every rank runs its own slices, no collective on
+the data path; `value` = slices of all ranks / max-over-ranks time.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "nbs_correlator_time_slices_per_s_52ch_32c64_fp64"
+UNIT = "time-slices/s"
+FP64_PEAK_TFLOPS = 37.2  # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz; the
+#                          in-tree probe measured 37.1 (DMMA) / 33.7 (DFMA) TFLOP/s on this pool
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (2 = 32^3 x 64)")
+    ap.add_argument("--lattice", type=int, default=0, help="override L (debugging only; invalidates the metric)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--oracle-sample-L", type=int, default=5)
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([s.strip() for s in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_leg(sample_L: int, cfg_index: int, steps: int, warmup: int) -> dict:
+    """Time the CPU oracle (tier B, eq. 2.6 path) on a bounded sample of the workload: the same
+    flavour recipe and all 52 channels on a sample_L^3 sub-lattice; its cost is per lattice site
+    (blocks per x, products per q; numpy's FFT is negligible), so slices/s at L^3 = sites/s / L^3."""
+    import numpy as np
+    from oracle import nbs_oracle as O
+    from paper_1604_07983_b200 import synth
+    cfg = synth.CONFIGS[cfg_index]
+    chans = O.channels52()
+    V_full = cfg["L"] ** 3
+    times = []
+    for i in range(warmup + steps):
+        S = synth.config_slice(cfg, i % cfg["T"], L=sample_L)
+        t0 = time.perf_counter()
+        B = O.all_blocks(S, O.sink_names(chans))
+        F = O.correlator_fft(sample_L, B, chans)
+        dt = time.perf_counter() - t0
+        assert np.isfinite(F).all()
+        if i >= warmup:
+            times.append(dt)
+    per_step = sum(times) / len(times)
+    sites_per_s = sample_L ** 3 / per_step
+    try:
+        import threadpoolctl
+        cores = max([p["num_threads"] for p in threadpoolctl.threadpool_info()] + [1])
+    except Exception:
+        cores = 1
+    return {"value": sites_per_s / V_full, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{sample_L}^3 sites of one slice (same flavour recipe, all 52 channels), "
+                      f"{per_step:.1f} s per sample, scaled by {sample_L ** 3}/{V_full} sites",
+            "ms_per_step": per_step * 1e3 * V_full / sample_L ** 3, "host_cpus": os.cpu_count()}
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from paper_1604_07983_b200 import synth
+    cfg = dict(synth.CONFIGS[args.config])
+    L = args.lattice or cfg["L"]
+    V = L ** 3
+    workload = f"BASELINE.json configs[{args.config}]: {L}^3 x {cfg['T']}, 52 channels, complex128, {cfg['name']}"
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        steps, warm = max(1, min(args.steps, 3)), min(args.warmup, 1)
+        leg = oracle_leg(args.oracle_sample_L, args.config, steps, warm)
+        line = {"impl": "reference", "metric": METRIC, "value": leg["value"], "unit": UNIT, "n_gpus": args.gpus,
+                "steps": steps, "warmup": warm, "ms_per_step": leg["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload},
+                "cpu_baseline": {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample")},
+                "e2e": {"value": leg["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line))
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1604_07983_b200 import nbs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    K, W = args.steps, max(args.warmup, 3)
+    T = cfg["T"]
+    npool = min(4, K + W)
+    # this rank's time slices: T-parallel replicas (t = rank, rank + world, ...)
+    pool_t = [(rank + i * world) % T for i in range(npool)]
+    host = []
+    for t in pool_t:
+        S = synth.config_slice(cfg, t, L=L)
+        pinned = {}
+        for f in "uds":
+            spec = cfg["flavours"][f]
+            if isinstance(spec, str):
+                pinned[f] = pinned[spec]
+            else:
+                buf = torch.empty((V, 12, 12), dtype=torch.complex128).pin_memory()
+                buf.copy_(torch.from_numpy(S[f]))
+                pinned[f] = buf
+        host.append(pinned)
+    resident = []
+    for h in host:
+        d = {}
+        for f in "uds":
+            spec = cfg["flavours"][f]
+            d[f] = d[spec] if isinstance(spec, str) else h[f].to(dev)
+        resident.append(d)
+
+    ctx = nbs.Nbs(L, T, None, device=local)
+    nch = ctx.nch
+    flops = ctx.model_flops()
+    out_dev = torch.empty((nch, 256, V), dtype=torch.complex128, device=dev)
+    stream = torch.cuda.Stream(device=dev)
+
+    def step_resident(i):
+        t = pool_t[i % npool]
+        r = resident[i % npool]
+        ctx.load(t, r["u"], r["d"], r["s"], stream=stream)
+        ctx.correlator(t, out=out_dev, stream=stream)
+
+    # ---------------- device-resident leg (value, roofline) ----------------
+    for i in range(W):
+        step_resident(i)
+    torch.cuda.synchronize()
+    ctx.set_timing(True)
+    ctx.stage_times(reset=True)
+    launches0 = ctx.kernel_launches()
+    sampler = ClockSampler(local)
+    barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(K):
+        step_resident(W + i)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    stage = ctx.stage_times(reset=True)
+    ctx.set_timing(False)
+    launches = ctx.kernel_launches() - launches0
+    checksum = float(out_dev.view(torch.float64).abs().max().item())
+    assert np.isfinite(checksum) and checksum > 0
+
+    # ---------------- end-to-end leg: host buffers through the C ABI ----------------
+    e2e = None
+    if not args.no_e2e:
+        out_host = torch.empty((nch, 256, V), dtype=torch.complex128).pin_memory()
+
+        def step_e2e(i):
+            t = pool_t[i % npool]
+            h = host[i % npool]
+            ctx.load(t, h["u"], h["d"], h["s"], stream=stream)      # H2D inside the library
+            ctx.correlator(t, out=out_host, stream=stream)          # D2H of F inside the library
+        step_e2e(0)
+        torch.cuda.synchronize()
+        barrier()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        Ke = max(1, min(K, 4))
+        f0.record(stream)
+        for i in range(Ke):
+            step_e2e(1 + i)
+        f1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        ms_e2e = f0.elapsed_time(f1)
+        nflav = len({id(v) for v in host[0].values()})
+        e2e = {"ms": ms_e2e, "steps": Ke, "h2d": nflav * V * 144 * 16, "d2h": nch * 256 * V * 16}
+        assert np.isfinite(out_host.view(torch.float64)[:1024]).all()
+
+    # ---------------- max over ranks ----------------
+    if world > 1:
+        tmax = torch.tensor([ms, e2e["ms"] if e2e else 0.0], dtype=torch.float64, device=dev)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms = float(tmax[0]);
+        if e2e:
+            e2e["ms"] = float(tmax[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = world * K / (ms * 1e-3)
+    prod_ms, prod_calls = stage["product"]
+    prod_avg_s = prod_ms * 1e-3 / max(prod_calls, 1)
+    alg_flops = flops["product"] * V  # 256 * sum_d K_d cMAC x 8 flop per q, standard count
+    achieved = alg_flops / prod_avg_s / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload, "channels": nch, "lattice": [L, L, L, T],
+                   "l2_policy": "inputs (226 MB) and intermediates (tens of GB per slice) exceed the 126 MB L2",
+                   "parallelism": "replicas only (T-parallel), no collective" if world > 1 else "1 GPU",
+                   "channel_sites_per_s": value * nch * V},
+        "clocks": clocks,
+        "gpu_launches": int(launches),
+        "stages_ms_per_step": {k: v[0] / max(v[1], 1) for k, v in stage.items()},
+        "roofline": {"bound": "alu", "kernel": "product (effective blocks x product, eqs. 4.2-4.3)",
+                     "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+                     "peak_source": "derived FP64 pipe peak 148 SM x 64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
+                     "flops_per_launch_algorithmic": alg_flops,
+                     "flops_per_launch_executed": flops["product_executed"] * V,
+                     "kernel_ms": prod_avg_s * 1e3},
+    }
+    if e2e:
+        line["e2e"] = {"value": world * e2e["steps"] / (e2e["ms"] * 1e-3), "unit": UNIT,
+                       "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
+    if world == 1 and not args.no_cpu_baseline:
+        leg = oracle_leg(args.oracle_sample_L, args.config, 1, 0)
+        line["cpu_baseline"] = {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    ctx.close()
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

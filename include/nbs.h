@@ -160,6 +160,24 @@ int nbs_model_flops(const nbs_ctx* ctx, double* blocks, double* fft, double* pro
  *   nbs_kernel_launches : number of CUDA kernels this context has launched so far (bench.py's
  *             `gpu_launches`).
  */
+/*
+ * Per-stage device timing (bench.py's roofline figures).  When enabled, nbs_correlator brackets
+ * each stage with a pair of CUDA events recorded on the stream the kernels are launched on;
+ * nbs_stage_times synchronises those events, adds their elapsed times to per-stage totals, writes
+ * total milliseconds and number of timed stage executions for the NBS_NUM_STAGES stages
+ * (either pointer may be NULL), and, if reset != 0, clears the totals.
+ */
+enum {
+    NBS_STAGE_BLOCKS = 0,   /* (i) normal baryon blocks, eq. 4.1 */
+    NBS_STAGE_FFT_FWD = 1,  /* forward FFT of the block components */
+    NBS_STAGE_PRODUCT = 2,  /* (ii)+(iii) effective blocks and their product, eqs. 4.2-4.3 */
+    NBS_STAGE_FFT_INV = 3,  /* inverse FFT, eq. 2.6 */
+    NBS_STAGE_OUTPUT = 4,   /* final layout F[ch][a1..a4][r] */
+    NBS_NUM_STAGES = 5
+};
+int nbs_set_timing(nbs_ctx* ctx, int enable);
+int nbs_stage_times(nbs_ctx* ctx, double* ms, long long* calls, int reset);
+
 int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);
 int nbs_fft3d(nbs_ctx* ctx, void* data_dev, size_t R, int inverse, void* stream);
 long long nbs_kernel_launches(const nbs_ctx* ctx);

@@ -55,6 +55,13 @@ struct nbs_ctx {
     unsigned dq_mask_of[NBS_NUM_BARYONS] = {};
     std::vector<void*> allocs;
     long long launches = 0;
+    // optional per-stage device timing (nbs_set_timing): events recorded on the launching stream
+    bool timing = false;
+    struct Pending { int stage; cudaEvent_t a, b; };
+    std::vector<Pending> pending;
+    std::vector<cudaEvent_t> event_pool;
+    double stage_ms[NBS_NUM_STAGES] = {};
+    long long stage_calls[NBS_NUM_STAGES] = {};
 };
 
 namespace {
@@ -72,6 +79,26 @@ int cuda_fail(nbs_ctx* c, cudaError_t e, const char* what) {
         cudaError_t e_ = (call);                               \
         if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); \
     } while (0)
+
+struct StageTimer { // brackets the launches of one stage with two events on `st`
+    nbs_ctx* c; int stage; cudaStream_t st; cudaEvent_t a = nullptr, b = nullptr;
+    static cudaEvent_t get(nbs_ctx* c) {
+        if (!c->event_pool.empty()) { cudaEvent_t e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
+        cudaEvent_t e = nullptr;
+        cudaEventCreate(&e);
+        return e;
+    }
+    StageTimer(nbs_ctx* c_, int stage_, cudaStream_t st_) : c(c_), stage(stage_), st(st_) {
+        if (!c->timing) return;
+        a = get(c); b = get(c);
+        cudaEventRecord(a, st);
+    }
+    ~StageTimer() {
+        if (!a) return;
+        cudaEventRecord(b, st);
+        c->pending.push_back({stage, a, b});
+    }
+};
 
 template <typename Tp>
 int upload(nbs_ctx* c, Tp*& dst, const std::vector<Tp>& src) {
@@ -310,31 +337,74 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     cudaStream_t st = (cudaStream_t)stream;
 
     // (i) normal baryon blocks, then forward FFT in place
-    int rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
-    if (rc) return rc;
-    rc = fft3d(c, sl.B, c->R, false, st);
-    if (rc) return rc;
-    // (ii)+(iii) effective blocks and their products -> elementary correlators
+    int rc;
+    {
+        StageTimer tm(c, NBS_STAGE_BLOCKS, st);
+        rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
+        if (rc) return rc;
+    }
+    {
+        StageTimer tm(c, NBS_STAGE_FFT_FWD, st);
+        rc = fft3d(c, sl.B, c->R, false, st);
+        if (rc) return rc;
+    }
+    // (ii)+(iii) effective blocks and their products -> elementary correlators -> channels
     const int nelem = (int)c->plan.elems.size();
-    dim3 grid((unsigned)c->V, (unsigned)c->plan.pairs.size());
-    k_product_v1<<<grid, PROD_THREADS, PROD_SMEM, st>>>(sl.B, c->R, c->L, c->d_pairs, c->d_elems, c->d_diagrams,
-                                                        c->d_gather, sl.E, nelem);
-    CU(c, cudaGetLastError());
-    ++c->launches;
-    k_combine<<<(unsigned)c->V, 256, 0, st>>>(sl.E, nelem, c->d_term_begin, c->d_terms, ch_begin, (int)nout, sl.Ft);
-    CU(c, cudaGetLastError());
-    ++c->launches;
+    {
+        StageTimer tm(c, NBS_STAGE_PRODUCT, st);
+        dim3 grid((unsigned)c->V, (unsigned)c->plan.pairs.size());
+        k_product_v1<<<grid, PROD_THREADS, PROD_SMEM, st>>>(sl.B, c->R, c->L, c->d_pairs, c->d_elems, c->d_diagrams,
+                                                            c->d_gather, sl.E, nelem);
+        CU(c, cudaGetLastError());
+        ++c->launches;
+        k_combine<<<(unsigned)c->V, 256, 0, st>>>(sl.E, nelem, c->d_term_begin, c->d_terms, ch_begin, (int)nout, sl.Ft);
+        CU(c, cudaGetLastError());
+        ++c->launches;
+    }
     // inverse FFT and final layout F[ch][a1 a2 a3 a4][r]
-    rc = fft3d(c, sl.Ft, nout * 256, true, st);
-    if (rc) return rc;
+    {
+        StageTimer tm(c, NBS_STAGE_FFT_INV, st);
+        rc = fft3d(c, sl.Ft, nout * 256, true, st);
+        if (rc) return rc;
+    }
     double2* dst = (double2*)out;
     if (memloc == NBS_MEM_HOST) dst = sl.E; // E is free again: use it as the device staging buffer
     if (memloc == NBS_MEM_HOST && (size_t)nelem < nout) return fail(c, NBS_EINVAL, "host output needs nelem >= channels");
-    dim3 tg((unsigned)((c->V + 31) / 32), (unsigned)((nout * 256 + 31) / 32));
-    k_transpose_out<<<tg, 256, 0, st>>>(sl.Ft, c->V, nout * 256, dst);
-    CU(c, cudaGetLastError());
-    ++c->launches;
+    {
+        StageTimer tm(c, NBS_STAGE_OUTPUT, st);
+        dim3 tg((unsigned)((c->V + 31) / 32), (unsigned)((nout * 256 + 31) / 32));
+        k_transpose_out<<<tg, 256, 0, st>>>(sl.Ft, c->V, nout * 256, dst);
+        CU(c, cudaGetLastError());
+        ++c->launches;
+    }
     if (memloc == NBS_MEM_HOST) CU(c, cudaMemcpyAsync(out, dst, need, cudaMemcpyDeviceToHost, st));
+    return NBS_OK;
+}
+
+int nbs_set_timing(nbs_ctx* c, int enable) {
+    if (!c) return NBS_EINVAL;
+    c->timing = enable != 0;
+    return NBS_OK;
+}
+
+int nbs_stage_times(nbs_ctx* c, double* ms, long long* calls, int reset) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    for (auto& p : c->pending) {
+        CU(c, cudaEventSynchronize(p.b));
+        float t = 0.f;
+        CU(c, cudaEventElapsedTime(&t, p.a, p.b));
+        c->stage_ms[p.stage] += t;
+        c->stage_calls[p.stage] += 1;
+        c->event_pool.push_back(p.a);
+        c->event_pool.push_back(p.b);
+    }
+    c->pending.clear();
+    for (int i = 0; i < NBS_NUM_STAGES; ++i) {
+        if (ms) ms[i] = c->stage_ms[i];
+        if (calls) calls[i] = c->stage_calls[i];
+        if (reset) { c->stage_ms[i] = 0; c->stage_calls[i] = 0; }
+    }
     return NBS_OK;
 }
 
@@ -343,6 +413,8 @@ void nbs_destroy(nbs_ctx* c) {
     if (cudaSetDevice(c->device) == cudaSuccess) {
         cudaDeviceSynchronize();
         for (void* p : c->allocs) cudaFree(p);
+        for (auto& p : c->pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+        for (cudaEvent_t e : c->event_pool) cudaEventDestroy(e);
     }
     delete c;
 }
