@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "nbs_kernels.cuh"
+#include "nbs_product.cuh"
 #include "nbs_tables.hpp"
 
 using namespace nbs;
@@ -23,8 +24,9 @@ struct Slice {
     const double2* S[3] = {nullptr, nullptr, nullptr}; // u, d, s (device)
     double2* own[3] = {nullptr, nullptr, nullptr};     // library-owned copies for host input
     double2* B = nullptr;  // [V][R] normal blocks, x-space then momentum space (in place)
-    double2* E = nullptr;  // [V][nelem][256]
     double2* Ft = nullptr; // [V][nch][256]
+    double2* scratch = nullptr;            // [grid][max_pair_units][256] unit results (L2-resident)
+    unsigned long long* counter = nullptr; // work-item counter of the persistent product kernel
 };
 
 } // namespace
@@ -40,12 +42,14 @@ struct nbs_ctx {
     Slice slice[NSLOTS_MAX];
     size_t R = 0; // block row length (complex) = nbaryons * 6912
     // device tables
-    PairRec* d_pairs = nullptr;
-    ElemRec* d_elems = nullptr;
-    DiagramRec* d_diagrams = nullptr;
-    uint16_t* d_gather = nullptr;
-    int* d_term_begin = nullptr;
-    ChanTermRec* d_terms = nullptr;
+    Pair2Rec* d_pairs2 = nullptr;
+    Unit2Rec* d_units2 = nullptr;
+    Diag2Rec* d_diags2 = nullptr;
+    uint32_t* d_tab2 = nullptr;
+    int* d_sched = nullptr;
+    PairChanRec* d_pair_chans = nullptr;
+    int* d_qorder = nullptr;
+    int prod_grid = 0;
     int* d_baryon_of_slot = nullptr;
     int* d_one_baryon = nullptr; // scratch for nbs_blocks_x
     BlockRec* d_brec = nullptr;
@@ -233,12 +237,39 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         long double ang = -2.0L * 3.141592653589793238462643383279502884L * m / L;
         tw[m] = make_double2((double)cosl(ang), (double)sinl(ang));
     }
-    CUC(upload(c, c->d_pairs, c->plan.pairs));
-    CUC(upload(c, c->d_elems, c->plan.elems));
-    CUC(upload(c, c->d_diagrams, c->plan.diagrams));
-    CUC(upload(c, c->d_gather, c->plan.gather));
-    CUC(upload(c, c->d_term_begin, c->plan.chan_term_begin));
-    CUC(upload(c, c->d_terms, c->plan.chan_terms));
+    CUC(upload(c, c->d_pairs2, c->plan.pairs2));
+    CUC(upload(c, c->d_units2, c->plan.units2));
+    CUC(upload(c, c->d_diags2, c->plan.diags2));
+    CUC(upload(c, c->d_tab2, c->plan.tab2));
+    CUC(upload(c, c->d_sched, c->plan.sched));
+    CUC(upload(c, c->d_pair_chans, c->plan.pair_chans));
+    {
+        // momenta ordered so that q and -q are adjacent (their blocks are shared through L2)
+        std::vector<int> qorder;
+        std::vector<char> seen(c->V, 0);
+        auto neg = [&](size_t q) {
+            size_t x = q % L, y = (q / L) % L, z = q / ((size_t)L * L);
+            x = x ? L - x : 0; y = y ? L - y : 0; z = z ? L - z : 0;
+            return x + (size_t)L * (y + (size_t)L * z);
+        };
+        for (size_t q = 0; q < c->V; ++q) {
+            if (seen[q]) continue;
+            qorder.push_back((int)q); seen[q] = 1;
+            size_t m = neg(q);
+            if (!seen[m]) { qorder.push_back((int)m); seen[m] = 1; }
+        }
+        CUC(upload(c, c->d_qorder, qorder));
+    }
+    {
+        cudaDeviceProp prop;
+        CUX(cudaGetDeviceProperties(&prop, device));
+        if ((size_t)prop.sharedMemPerBlockOptin < PROD2_SMEM) {
+            g_create_error = "device has too little shared memory per block for the product kernel";
+            nbs_destroy(c);
+            return NBS_ECUDA;
+        }
+        c->prod_grid = prop.multiProcessorCount;
+    }
     CUC(upload(c, c->d_baryon_of_slot, c->plan.baryons));
     CUC(upload(c, c->d_one_baryon, std::vector<int>(NBS_NUM_BARYONS, 0)));
     {
@@ -251,8 +282,9 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     CUC(upload(c, c->d_tw, tw));
 
     // workspace: per slice in flight, blocks + elementary correlators + channel correlators
-    size_t nelem = c->plan.elems.size(), nchan = c->plan.channels.size();
-    size_t per_slice = c->V * (c->R + (nelem + nchan) * 256) * sizeof(double2);
+    size_t nchan = c->plan.channels.size();
+    size_t scratch_elems = (size_t)c->prod_grid * c->plan.max_pair_units * 256;
+    size_t per_slice = (c->V * (c->R + nchan * 256) + scratch_elems) * sizeof(double2);
     size_t free_b = 0, total_b = 0;
     CUX(cudaMemGetInfo(&free_b, &total_b));
     size_t avail = (size_t)(0.92 * (double)free_b);
@@ -266,10 +298,13 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     }
     for (int i = 0; i < c->nslices; ++i) {
         CUC(dev_alloc(c, c->slice[i].B, c->V * c->R));
-        CUC(dev_alloc(c, c->slice[i].E, c->V * nelem * 256));
         CUC(dev_alloc(c, c->slice[i].Ft, c->V * nchan * 256));
+        CUC(dev_alloc(c, c->slice[i].scratch, scratch_elems));
+        double2* cnt = nullptr;
+        CUC(dev_alloc(c, cnt, 1));
+        c->slice[i].counter = (unsigned long long*)cnt;
     }
-    CUX(cudaFuncSetAttribute(k_product_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
+    CUX(cudaFuncSetAttribute(k_product_v2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD2_SMEM));
     CUX(cudaFuncSetAttribute(k_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)((3 * 144 + 9 * 432) * sizeof(double2))));
     *out = c;
@@ -349,15 +384,21 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         if (rc) return rc;
     }
     // (ii)+(iii) effective blocks and their products -> elementary correlators -> channels
-    const int nelem = (int)c->plan.elems.size();
     {
         StageTimer tm(c, NBS_STAGE_PRODUCT, st);
-        dim3 grid((unsigned)c->V, (unsigned)c->plan.pairs.size());
-        k_product_v1<<<grid, PROD_THREADS, PROD_SMEM, st>>>(sl.B, c->R, c->L, c->d_pairs, c->d_elems, c->d_diagrams,
-                                                            c->d_gather, sl.E, nelem);
-        CU(c, cudaGetLastError());
-        ++c->launches;
-        k_combine<<<(unsigned)c->V, 256, 0, st>>>(sl.E, nelem, c->d_term_begin, c->d_terms, ch_begin, (int)nout, sl.Ft);
+        CU(c, cudaMemsetAsync(sl.counter, 0, sizeof(unsigned long long), st));
+        Prod2Args pa;
+        pa.Bq = sl.B; pa.R = c->R; pa.L = c->L;
+        pa.npairs = (int)c->plan.pairs2.size();
+        pa.nitems = (long long)c->V * pa.npairs;
+        pa.qorder = c->d_qorder;
+        pa.pairs = c->d_pairs2; pa.units = c->d_units2; pa.diags = c->d_diags2; pa.tab = c->d_tab2;
+        pa.sched = c->d_sched; pa.pair_chans = c->d_pair_chans;
+        pa.scratch = sl.scratch; pa.max_pair_units = c->plan.max_pair_units;
+        pa.Ft = sl.Ft; pa.ch_begin = ch_begin; pa.nch_out = (int)nout;
+        pa.counter = sl.counter;
+        unsigned grid = (unsigned)std::min<long long>(c->prod_grid, pa.nitems);
+        k_product_v2<<<grid, PROD2_THREADS, PROD2_SMEM, st>>>(pa);
         CU(c, cudaGetLastError());
         ++c->launches;
     }
@@ -368,8 +409,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         if (rc) return rc;
     }
     double2* dst = (double2*)out;
-    if (memloc == NBS_MEM_HOST) dst = sl.E; // E is free again: use it as the device staging buffer
-    if (memloc == NBS_MEM_HOST && (size_t)nelem < nout) return fail(c, NBS_EINVAL, "host output needs nelem >= channels");
+    if (memloc == NBS_MEM_HOST) dst = sl.B; // the block buffer is free again: device staging for the host copy
     {
         StageTimer tm(c, NBS_STAGE_OUTPUT, st);
         dim3 tg((unsigned)((c->V + 31) / 32), (unsigned)((nout * 256 + 31) / 32));

@@ -3,7 +3,6 @@
 // Data layout in HBM ("site-major"): every stage keeps all components of one lattice site (or
 // momentum q) contiguous:
 //   blocks  B[site][slot][alpha][xi1 xi2 xi3]   (row length R = nslots * 6912 complex)
-//   E       [q][elem][256]                       elementary correlators
 //   Ft      [q][ch][256]                         channel correlators in momentum space
 // so that (a) the block kernel writes one site's 110 KB per baryon fully coalesced, (b) the FFT
 // runs one 1-D transform per thread with lanes on consecutive components (coalesced, no shared
@@ -201,97 +200,6 @@ k_fft_axis_generic(double2* __restrict__ data, size_t R, int L, int axis, const 
         double2 v = b[j];
         if (INV) { v.x *= scale; v.y *= scale; }
         data[(s0 + j * st) * R + r] = v;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// (ii)+(iii) EffectiveBaryonBlocks fused into MultiplicationEffectiveBlocks, eqs. 4.2-4.3
-// (PAPER.md:104-115).  One CTA per (momentum q, sink pair): B~1(q) and B~2(-q) (2 x 110 KB) are
-// staged once in shared memory and every diagram of every elementary correlator of the pair is
-// evaluated from there; the effective blocks exist only as gathered operands, never in memory.
-// v1: one thread per output spin combination (a1 a2 a3 a4), table-driven signed gathers.
-// ---------------------------------------------------------------------------------------------
-constexpr int PROD_THREADS = 256;
-constexpr size_t PROD_SMEM = 2 * (size_t)BLOCK_ELEMS * sizeof(double2);
-
-__device__ __forceinline__ size_t minus_q(int L, size_t q) {
-    int x = (int)(q % L), y = (int)((q / L) % L), z = (int)(q / ((size_t)L * L));
-    x = x ? L - x : 0; y = y ? L - y : 0; z = z ? L - z : 0;
-    return x + (size_t)L * (y + (size_t)L * z);
-}
-
-__global__ void __launch_bounds__(PROD_THREADS)
-k_product_v1(const double2* __restrict__ Bq, size_t R, int L, const PairRec* __restrict__ pairs,
-             const ElemRec* __restrict__ elems, const DiagramRec* __restrict__ diagrams,
-             const uint16_t* __restrict__ gather, double2* __restrict__ E, int nelem) {
-    extern __shared__ double2 smem[];
-    double2* s1 = smem;
-    double2* s2 = smem + BLOCK_ELEMS;
-    const size_t q = blockIdx.x;
-    const PairRec pr = pairs[blockIdx.y];
-    const int tid = threadIdx.x;
-    {
-        const double2* g1 = Bq + q * R + (size_t)pr.slot1 * BLOCK_ELEMS;
-        const double2* g2 = Bq + minus_q(L, q) * R + (size_t)pr.slot2 * BLOCK_ELEMS;
-        for (int i = tid; i < BLOCK_ELEMS; i += PROD_THREADS) {
-            s1[i] = g1[i];
-            s2[i] = g2[i];
-        }
-    }
-    __syncthreads();
-    const int a1 = tid >> 6, a2 = (tid >> 4) & 3, a3 = (tid >> 2) & 3, a4 = tid & 3;
-    const double2* base1 = s1 + a1 * NTRIPLE;
-    const double2* base2 = s2 + a2 * NTRIPLE;
-    for (int e = pr.elem_begin; e < pr.elem_end; ++e) {
-        const ElemRec er = elems[e];
-        double2 acc = make_double2(0.0, 0.0);
-        for (int d = er.diag_begin; d < er.diag_end; ++d) {
-            const DiagramRec dr = diagrams[d];
-            int c1, c2;
-            switch (dr.mask1) {
-            case 3: c1 = a3 * 4 + a4; c2 = 0; break;
-            case 1: c1 = a3; c2 = a4; break;
-            case 2: c1 = a4; c2 = a3; break;
-            default: c1 = 0; c2 = a3 * 4 + a4; break;
-            }
-            const int K = dr.K, n1 = dr.n1, n2 = dr.n2;
-            const uint16_t* p1 = gather + dr.off1 + (size_t)c1 * K * n1;
-            const uint16_t* p2 = gather + dr.off2 + (size_t)c2 * K * n2;
-            for (int k = 0; k < K; ++k) {
-                double2 x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
-                for (int j = 0; j < n1; ++j) {
-                    unsigned g = p1[k * n1 + j];
-                    double2 v = base1[g & 0x7ff];
-                    x = (g & 0x8000) ? csub(x, v) : cadd(x, v);
-                }
-                for (int j = 0; j < n2; ++j) {
-                    unsigned g = p2[k * n2 + j];
-                    double2 v = base2[g & 0x7ff];
-                    y = (g & 0x8000) ? csub(y, v) : cadd(y, v);
-                }
-                cfma(acc, x, y);
-            }
-        }
-        E[(q * nelem + e) * 256 + tid] = acc;
-    }
-}
-
-// Channel correlator = sum over its elementary source terms (Lambda, Sigma0 expanded into
-// X_u, X_d, X_s; eqs. 2.2-2.3): Ft[q][ch][o] = sum_terms coef * E[q][elem][o].
-__global__ void __launch_bounds__(256)
-k_combine(const double2* __restrict__ E, int nelem, const int* __restrict__ term_begin,
-          const ChanTermRec* __restrict__ terms, int ch_begin, int nch_out, double2* __restrict__ Ft) {
-    const size_t q = blockIdx.x;
-    const int o = threadIdx.x;
-    for (int c = 0; c < nch_out; ++c) {
-        double2 acc = make_double2(0.0, 0.0);
-        for (int it = term_begin[ch_begin + c]; it < term_begin[ch_begin + c + 1]; ++it) {
-            ChanTermRec t = terms[it];
-            double2 v = E[(q * nelem + t.elem) * 256 + o];
-            acc.x = fma(t.coef, v.x, acc.x);
-            acc.y = fma(t.coef, v.y, acc.y);
-        }
-        Ft[(q * nch_out + c) * 256 + o] = acc;
     }
 }
 

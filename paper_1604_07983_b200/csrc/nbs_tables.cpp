@@ -401,6 +401,101 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan) {
         for (auto& ct : chan_ct[ic]) plan.chan_terms.push_back(ChanTermRec{elem_id[ct.pair][ct.key], ct.coef});
         plan.chan_term_begin.push_back((int)plan.chan_terms.size());
     }
+
+    // ---- v2 (DMMA) tables: pairs -> (<= MAX_PAIR_ELEMS elementary correlators) -> units -> diagrams
+    std::map<std::vector<uint32_t>, uint32_t> dedupe2;
+    auto intern2 = [&](const SideTable& t) {
+        // [c][k][term] u16  ->  [k][c][term/2] u32, k padded to a multiple of 4
+        const int Kp = (t.K + 3) / 4 * 4, nw = t.n / 2;
+        std::vector<uint32_t> w((size_t)Kp * t.C * nw, 0u);
+        for (int k = 0; k < t.K; ++k)
+            for (int c = 0; c < t.C; ++c)
+                for (int j = 0; j < nw; ++j) {
+                    size_t src = ((size_t)c * t.K + k) * t.n + 2 * j;
+                    w[((size_t)k * t.C + c) * nw + j] = (uint32_t)t.g[src] | ((uint32_t)t.g[src + 1] << 16);
+                }
+        auto it = dedupe2.find(w);
+        if (it != dedupe2.end()) return it->second;
+        uint32_t off = (uint32_t)plan.tab2.size();
+        plan.tab2.insert(plan.tab2.end(), w.begin(), w.end());
+        while (plan.tab2.size() % 4) plan.tab2.push_back(0); // 16-byte aligned tables
+        dedupe2[w] = off;
+        return off;
+    };
+    const int UNIT_COST_MAX = 160;
+    for (size_t ip = 0; ip < pair_list.size(); ++ip) {
+        const std::vector<Key>& order = pair_elem_order[ip];
+        // at most 15 distinct elementary source operators pairs share the flavour content of one sink pair
+        if (order.size() > (size_t)MAX_PAIR_ELEMS) return "internal: more than 16 elementary correlators for one sink pair";
+        {
+            const size_t e0 = 0, e1 = order.size();
+            Pair2Rec pr;
+            pr.slot1 = slot_of[pair_list[ip].first];
+            pr.slot2 = slot_of[pair_list[ip].second];
+            pr.unit_begin = (int)plan.units2.size();
+            pr.nelem = (int)(e1 - e0);
+            for (size_t e = e0; e < e1; ++e) {
+                pr.elem_unit_begin[e - e0] = (int)plan.units2.size() - pr.unit_begin;
+                for (int cls = 0; cls < 4; ++cls) {
+                    Unit2Rec u;
+                    u.cls = cls; u.cost = 0; u.diag_begin = (int)plan.diags2.size();
+                    auto flush = [&] {
+                        u.diag_end = (int)plan.diags2.size();
+                        if (u.diag_end > u.diag_begin) plan.units2.push_back(u);
+                        u.diag_begin = u.diag_end; u.cost = 0;
+                    };
+                    for (auto& d : pair_elems[ip][order[e]]) {
+                        SideTable s1 = make_side(d.P, d.sign); // sigma_P folded into side 1
+                        SideTable s2 = make_side(d.P + 3, +1);
+                        int c;
+                        if (s1.C == 4 && s2.C == 4) c = (s1.carries == 1) ? 0 : 1;
+                        else if (s1.C == 16 && s2.C == 1) c = 2;
+                        else if (s1.C == 1 && s2.C == 16) c = 3;
+                        else return "internal: unexpected carry split";
+                        if (c != cls) continue;
+                        if ((s1.n & 1) || (s2.n & 1)) return "internal: odd gather length";
+                        Diag2Rec r;
+                        const SideTable &A = (c == 3) ? s2 : s1, &B = (c == 3) ? s1 : s2;
+                        r.offA = intern2(A); r.offB = intern2(B);
+                        r.K = (uint16_t)s1.K; r.Kp = (uint16_t)((s1.K + 3) / 4 * 4);
+                        r.nA = (uint8_t)A.n; r.nB = (uint8_t)B.n; r.pad = 0;
+                        int cost = r.Kp * (c >= 2 ? 3 : 2) / 2 + 4;
+                        if (u.cost > 0 && u.cost + cost > UNIT_COST_MAX) flush();
+                        plan.diags2.push_back(r);
+                        u.cost += cost;
+                        plan.sumKp_exec += r.Kp;
+                    }
+                    flush();
+                }
+            }
+            pr.nunits = (int)plan.units2.size() - pr.unit_begin;
+            for (int e = pr.nelem; e <= MAX_PAIR_ELEMS; ++e) pr.elem_unit_begin[e] = pr.nunits;
+            plan.max_pair_units = std::max(plan.max_pair_units, pr.nunits);
+            // schedule: local unit indices by decreasing cost (warps take them in this order)
+            pr.sched_begin = (int)plan.sched.size();
+            std::vector<int> idx(pr.nunits);
+            for (int i = 0; i < pr.nunits; ++i) idx[i] = i;
+            std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
+                return plan.units2[pr.unit_begin + a].cost > plan.units2[pr.unit_begin + b].cost;
+            });
+            plan.sched.insert(plan.sched.end(), idx.begin(), idx.end());
+            // channels of this pair as dense coefficient rows over its elementary correlators
+            pr.chan_begin = (int)plan.pair_chans.size();
+            for (size_t ic = 0; ic < channels.size(); ++ic) {
+                if (plan.chan_pair[ic] != (int)ip) continue;
+                PairChanRec pc;
+                pc.ch = (int)ic; pc.pad = 0;
+                bool any = false;
+                for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = 0.0;
+                for (auto& ct : chan_ct[ic])
+                    for (size_t e = e0; e < e1; ++e)
+                        if (order[e] == ct.key) { pc.coef[e - e0] += ct.coef; any = true; }
+                if (any) plan.pair_chans.push_back(pc);
+            }
+            pr.nchan = (int)plan.pair_chans.size() - pr.chan_begin;
+            plan.pairs2.push_back(pr);
+        }
+    }
     return "";
 }
 

@@ -57,6 +57,38 @@ struct ChanTermRec {
     double coef;
 };
 
+// ---- v2 product kernel (DMMA) records ------------------------------------------------------
+// A "unit" is the work of one warp: a few diagrams of ONE elementary correlator that share one
+// accumulator layout (class).  Classes (which effective block carries a3 / a4):
+//   0: 16x16, B~1 carries a3, B~2 carries a4      1: 16x16, B~1 carries a4, B~2 carries a3
+//   2: 64x4,  B~1 carries a3 and a4               3: 4x64,  B~2 carries a3 and a4
+// Gather tables are u32 words holding two u16 entries (bit 15: minus sign, bits 0-10: source
+// triple xi1 xi2 xi3), laid out [k][c][term/2] with k padded to a multiple of 4 (Kp).
+constexpr int MAX_PAIR_ELEMS = 16;
+struct Diag2Rec {
+    uint32_t offA, offB; // word offsets: operand A (the M side) and operand B (the N side)
+    uint16_t K, Kp;
+    uint8_t nA, nB;      // gather terms per entry
+    uint16_t pad;
+};
+struct Unit2Rec {
+    int diag_begin, diag_end; // range in Plan::diags2
+    int cls;
+    int cost;
+};
+struct Pair2Rec {
+    int slot1, slot2;
+    int unit_begin, nunits;  // units grouped by elementary correlator (elem_unit_begin)
+    int sched_begin;         // Plan::sched[sched_begin + i]: local unit index, cost descending
+    int nelem;
+    int elem_unit_begin[MAX_PAIR_ELEMS + 1]; // local unit ranges per elementary correlator
+    int chan_begin, nchan;   // range in Plan::pair_chans
+};
+struct PairChanRec {
+    int ch, pad;
+    double coef[MAX_PAIR_ELEMS]; // channel = sum_e coef[e] * elementary correlator e (eqs. 2.2-2.3)
+};
+
 struct DiagramInfo { // host-side description (tests, statistics)
     int P[6];
     int sign;
@@ -75,6 +107,15 @@ struct Plan {
     std::vector<int> chan_pair; // pair index of each channel
     double sumK_std = 0;        // sum over channels of sum_d K_d (the paper's count)
     double sumK_exec = 0;       // sum over distinct elementary correlators
+    // v2 (DMMA) product kernel tables
+    std::vector<Pair2Rec> pairs2;
+    std::vector<Unit2Rec> units2;
+    std::vector<Diag2Rec> diags2;
+    std::vector<uint32_t> tab2;
+    std::vector<int> sched;
+    std::vector<PairChanRec> pair_chans;
+    int max_pair_units = 0;
+    double sumKp_exec = 0; // executed k-steps x 4 (padding included)
 };
 
 // Returns "" on success, else an error message (invalid id, flavour violation).
