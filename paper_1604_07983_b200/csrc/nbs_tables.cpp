@@ -162,7 +162,7 @@ struct SideTable {
     int carries; // bit0: a3, bit1: a4
     std::vector<uint16_t> g;
 };
-SideTable make_side(const int* slots, int overall_sign) {
+SideTable make_side(const int* slots, int overall_sign, bool smem_layout = false) {
     int mask[2] = {0, 0};
     for (int m = 0; m < 3; ++m) mask[slots[m] / 3] |= 1 << (slots[m] % 3);
     const Factor& f0 = factor(mask[0]);
@@ -182,9 +182,12 @@ SideTable make_side(const int* slots, int overall_sign) {
                 int q = slots[m];
                 xi[m] = (q / 3 == 0 ? e0 : e1).xi[q % 3];
             }
-            int tri = (xi[0] * NXI + xi[1]) * NXI + xi[2];
+            int tri = smem_layout ? sm_index(xi[0], xi[1], xi[2]) : (xi[0] * NXI + xi[1]) * NXI + xi[2];
             int c = e0.carry * f1.ncarry + e1.carry;
-            int k = e0.shared * f1.nshared + e1.shared;
+            // shared index: the larger factor runs fastest (12 is a multiple of the MMA k-step 4, so
+            // four consecutive k then differ in ONE colour-spin index: conflict-free gathers)
+            int k = (f0.nshared > f1.nshared) ? e1.shared * f0.nshared + e0.shared
+                                               : e0.shared * f1.nshared + e1.shared;
             int sign = e0.sign * e1.sign * overall_sign;
             size_t ent = (size_t)c * t.K + k;
             t.g[ent * t.n + fill[ent]++] = (uint16_t)(tri | (sign < 0 ? 0x8000 : 0));
@@ -298,7 +301,7 @@ std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& ou
     return "";
 }
 
-std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan) {
+std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps, int unit_cost_max) {
     plan = Plan();
     plan.channels = channels;
     if (channels.empty()) return "empty channel list";
@@ -422,7 +425,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan) {
         dedupe2[w] = off;
         return off;
     };
-    const int UNIT_COST_MAX = 160;
+    const int UNIT_SPLIT_STEPS = unit_split_steps, UNIT_COST_MAX = unit_cost_max; // cost: 2 per 16x16 step, 3 per 64x4 step
     for (size_t ip = 0; ip < pair_list.size(); ++ip) {
         const std::vector<Key>& order = pair_elem_order[ip];
         // at most 15 distinct elementary source operators pairs share the flavour content of one sink pair
@@ -445,8 +448,8 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan) {
                         u.diag_begin = u.diag_end; u.cost = 0;
                     };
                     for (auto& d : pair_elems[ip][order[e]]) {
-                        SideTable s1 = make_side(d.P, d.sign); // sigma_P folded into side 1
-                        SideTable s2 = make_side(d.P + 3, +1);
+                        SideTable s1 = make_side(d.P, d.sign, true); // sigma_P folded into side 1
+                        SideTable s2 = make_side(d.P + 3, +1, true);
                         int c;
                         if (s1.C == 4 && s2.C == 4) c = (s1.carries == 1) ? 0 : 1;
                         else if (s1.C == 16 && s2.C == 1) c = 2;
@@ -457,13 +460,21 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan) {
                         Diag2Rec r;
                         const SideTable &A = (c == 3) ? s2 : s1, &B = (c == 3) ? s1 : s2;
                         r.offA = intern2(A); r.offB = intern2(B);
-                        r.K = (uint16_t)s1.K; r.Kp = (uint16_t)((s1.K + 3) / 4 * 4);
-                        r.nA = (uint8_t)A.n; r.nB = (uint8_t)B.n; r.pad = 0;
-                        int cost = r.Kp * (c >= 2 ? 3 : 2) / 2 + 4;
-                        if (u.cost > 0 && u.cost + cost > UNIT_COST_MAX) flush();
-                        plan.diags2.push_back(r);
-                        u.cost += cost;
-                        plan.sumKp_exec += r.Kp;
+                        r.K = (uint16_t)s1.K;
+                        r.nA = (uint8_t)A.n; r.nB = (uint8_t)B.n;
+                        // split long diagrams into k-ranges so that a sink pair with few diagrams
+                        // still spreads over all warps of the CTA
+                        const int steps = (s1.K + 3) / 4;
+                        const int nchunk = (steps + UNIT_SPLIT_STEPS - 1) / UNIT_SPLIT_STEPS;
+                        for (int ic = 0; ic < nchunk; ++ic) {
+                            const int sb = steps * ic / nchunk, se = steps * (ic + 1) / nchunk;
+                            r.kbeg = (uint16_t)(4 * sb); r.kend = (uint16_t)(4 * se);
+                            const int cost = (se - sb) * (c >= 2 ? 3 : 2) + 2;
+                            if (u.cost > 0 && u.cost + cost > UNIT_COST_MAX) flush();
+                            plan.diags2.push_back(r);
+                            u.cost += cost;
+                            plan.sumKp_exec += 4 * (se - sb);
+                        }
                     }
                     flush();
                 }
@@ -496,6 +507,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan) {
             plan.pairs2.push_back(pr);
         }
     }
+    plan.tab2.insert(plan.tab2.end(), 256, 0u); // the kernel prefetches one k-step past a table's end
     return "";
 }
 

@@ -14,6 +14,16 @@ constexpr int NXI = 12;           // colour x spin
 constexpr int NTRIPLE = 1728;     // 12^3 source index triples of a normal block
 constexpr int BLOCK_ELEMS = 6912; // 4 sink spins x 12^3
 
+// Shared-memory layout of one sink-spin plane of a normal block in the product kernel: the source
+// triple (xi1, xi2, xi3) sits at xi1*145 + xi2*12 + (xi3 + xi2) mod 12.  With this skew four
+// consecutive values of any one xi fall into four different 16-byte bank groups modulo 4, and the
+// plane stride 1740 = 4 (mod 8) puts two adjacent planes into the two halves of the 8 bank groups:
+// the 8 lanes of a quarter warp (2 planes x 4 consecutive k) then gather without bank conflicts.
+constexpr int SM_STRIDE1 = 145;
+constexpr int SM_PLANE = 12 * SM_STRIDE1;  // 1740
+constexpr int SM_BLOCK = 4 * SM_PLANE;     // 6960 complex per staged block
+constexpr int sm_index(int xi1, int xi2, int xi3) { return xi1 * SM_STRIDE1 + xi2 * 12 + (xi3 + xi2) % 12; }
+
 // One elementary operator  eps_abc (q_f0,a  C g5  q_f1,b) q_f2,c  with a real coefficient
 // (eqs. 2.2-2.3).  Flavours: 0 = u, 1 = d, 2 = s.
 struct ElemTerm {
@@ -62,14 +72,14 @@ struct ChanTermRec {
 // accumulator layout (class).  Classes (which effective block carries a3 / a4):
 //   0: 16x16, B~1 carries a3, B~2 carries a4      1: 16x16, B~1 carries a4, B~2 carries a3
 //   2: 64x4,  B~1 carries a3 and a4               3: 4x64,  B~2 carries a3 and a4
-// Gather tables are u32 words holding two u16 entries (bit 15: minus sign, bits 0-10: source
-// triple xi1 xi2 xi3), laid out [k][c][term/2] with k padded to a multiple of 4 (Kp).
+// Gather tables are u32 words holding two u16 entries (bit 15: minus sign, bits 0-10: sm_index of the
+// source triple), laid out [k][c][term/2] with k padded to a multiple of 4 (Kp).
 constexpr int MAX_PAIR_ELEMS = 16;
 struct Diag2Rec {
     uint32_t offA, offB; // word offsets: operand A (the M side) and operand B (the N side)
-    uint16_t K, Kp;
+    uint16_t K;          // size of the shared index (1, 9, 36, 144)
+    uint16_t kbeg, kend; // this record covers k in [kbeg, kend), both multiples of 4 (kend may pass K: padding)
     uint8_t nA, nB;      // gather terms per entry
-    uint16_t pad;
 };
 struct Unit2Rec {
     int diag_begin, diag_end; // range in Plan::diags2
@@ -119,7 +129,8 @@ struct Plan {
 };
 
 // Returns "" on success, else an error message (invalid id, flavour violation).
-std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan);
+std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps = 18,
+                       int unit_cost_max = 40);
 
 // Diagrams of one channel in enumeration order (source terms major, permutations lexicographic).
 std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& out);
