@@ -11,6 +11,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+#include <utility>
+
 #include "nbs_tables.hpp"
 
 namespace nbs {
@@ -117,31 +120,50 @@ __host__ __device__ constexpr int bitrev(int i, int bits) {
     return r;
 }
 
+// cos / sin of 2 pi m / 32, m = 0..15, as compile-time constants (they reach the FP64 pipe through
+// the constant bank and cost no registers).  exp(-2 pi i k / len) = (tw32_cos, -tw32_sin)(k * 32 / len)
+// for every power-of-two len <= 32.
+__host__ __device__ constexpr double tw32_quarter(int m) { // cos(2 pi m / 32), 0 <= m <= 8
+    constexpr double C[9] = {1.0, 9.807852804032304491e-01, 9.238795325112867561e-01, 8.314696123025452371e-01,
+                             7.071067811865475244e-01, 5.555702330196022248e-01, 3.826834323650897717e-01,
+                             1.950903220161282679e-01, 0.0};
+    return C[m];
+}
+__host__ __device__ constexpr double tw32_cos(int m) { return m <= 8 ? tw32_quarter(m) : -tw32_quarter(16 - m); }
+__host__ __device__ constexpr double tw32_sin(int m) { return m <= 8 ? tw32_quarter(8 - m) : tw32_quarter(m - 8); }
+
+// Compile-time loop: every array index below is a constant, so the L points stay in registers
+// (a run-time-indexed double2[32] would be placed in local memory).
+template <int... Is, class F>
+__device__ __forceinline__ void static_for(std::integer_sequence<int, Is...>, F&& f) {
+    (f(std::integral_constant<int, Is>{}), ...);
+}
+
 template <int L, bool INV>
 __device__ __forceinline__ void fft_inreg(double2 (&a)[L], const double2* __restrict__ tw) {
     constexpr int LOG = ilog2(L);
-#pragma unroll
-    for (int i = 0; i < L; ++i) {
-        const int j = bitrev(i, LOG);
-        if (i < j) { double2 tmp = a[i]; a[i] = a[j]; a[j] = tmp; }
-    }
-#pragma unroll
-    for (int len = 2; len <= L; len <<= 1) {
-#pragma unroll
-        for (int i = 0; i < L; i += len) {
-#pragma unroll
-            for (int k = 0; k < len / 2; ++k) {
-                double2 u = a[i + k], v = a[i + k + len / 2];
-                if (k != 0) {
-                    double2 w = __ldg(tw + k * (L / len));
-                    if (INV) w.y = -w.y;
-                    v = cmul(v, w);
+    static_for(std::make_integer_sequence<int, L>{}, [&](auto ic) {
+        constexpr int i = decltype(ic)::value, j = bitrev(i, LOG);
+        if constexpr (i < j) { const double2 tmp = a[i]; a[i] = a[j]; a[j] = tmp; }
+    });
+    static_for(std::make_integer_sequence<int, LOG>{}, [&](auto sc) {
+        constexpr int len = 2 << decltype(sc)::value, half = len / 2;
+        static_for(std::make_integer_sequence<int, L / 2>{}, [&](auto bc) {
+            constexpr int b = decltype(bc)::value, k = b % half, i = (b / half) * len + k;
+            const double2 u = a[i];
+            double2 v = a[i + half];
+            if constexpr (k != 0) {
+                if constexpr (4 * k == len) { // w = -i (forward) or +i (inverse)
+                    v = INV ? make_double2(-v.y, v.x) : make_double2(v.y, -v.x);
+                } else {
+                    constexpr double wr = tw32_cos(k * (32 / len)), wi = -tw32_sin(k * (32 / len));
+                    v = cmul(v, make_double2(wr, INV ? -wi : wi));
                 }
-                a[i + k] = cadd(u, v);
-                a[i + k + len / 2] = csub(u, v);
             }
-        }
-    }
+            a[i] = cadd(u, v);
+            a[i + half] = csub(u, v);
+        });
+    });
 }
 
 __device__ __forceinline__ void line_geometry(int L, int axis, int line, size_t& s0, size_t& st) {
