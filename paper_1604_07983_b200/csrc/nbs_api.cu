@@ -25,7 +25,7 @@ struct Slice {
     double2* own[3] = {nullptr, nullptr, nullptr};     // library-owned copies for host input
     double2* B = nullptr;  // [V][R] normal blocks, x-space then momentum space (in place)
     double2* Ft = nullptr; // [V][nch][256]
-    double2* scratch = nullptr;            // [grid][max_pair_units][256] unit results (L2-resident)
+    double2* scratch = nullptr;            // [grid][2][max_pair_units][256] unit results
     unsigned long long* counter = nullptr; // work-item counter of the persistent product kernel
 };
 
@@ -40,13 +40,13 @@ struct nbs_ctx {
     size_t workspace = 0;
     int nslices = 0;
     Slice slice[NSLOTS_MAX];
-    size_t R = 0; // block row length (complex) = nbaryons * 6912
+    size_t R = 0; // block row length (complex) = nbaryons * SM_BLOCK (staged layout, nbs_tables.hpp)
     // device tables
-    Pair2Rec* d_pairs2 = nullptr;
-    Unit2Rec* d_units2 = nullptr;
-    Diag2Rec* d_diags2 = nullptr;
-    uint32_t* d_tab2 = nullptr;
-    int* d_sched = nullptr;
+    Pair3Rec* d_pairs3 = nullptr;
+    Unit3Rec* d_units3 = nullptr;
+    Diag3Rec* d_diags3 = nullptr;
+    uint2x* d_tab3 = nullptr;
+    ChainRec* d_chain = nullptr;
     PairChanRec* d_pair_chans = nullptr;
     int* d_qorder = nullptr;
     int prod_grid = 0;
@@ -151,10 +151,10 @@ int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st) {
 }
 
 int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, int nslots, unsigned dq_mask, double2* out,
-                  size_t row_stride, cudaStream_t st) {
+                  size_t row_stride, int staged, cudaStream_t st) {
     size_t smem = (3 * 144 + 9 * 432) * sizeof(double2);
     k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, smem, st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask, c->d_brec,
-                                                           c->d_bterm, out, row_stride);
+                                                           c->d_bterm, out, row_stride, staged);
     CU(c, cudaGetLastError());
     ++c->launches;
     return NBS_OK;
@@ -195,7 +195,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     if (!err.empty()) { delete c; return fail(nullptr, NBS_EINVAL, err); }
     c->L = L; c->T = T; c->device = device;
     c->V = (size_t)L * L * L;
-    c->R = c->plan.baryons.size() * (size_t)BLOCK_ELEMS;
+    c->R = c->plan.baryons.size() * (size_t)SM_BLOCK;
 
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -237,11 +237,11 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         long double ang = -2.0L * 3.141592653589793238462643383279502884L * m / L;
         tw[m] = make_double2((double)cosl(ang), (double)sinl(ang));
     }
-    CUC(upload(c, c->d_pairs2, c->plan.pairs2));
-    CUC(upload(c, c->d_units2, c->plan.units2));
-    CUC(upload(c, c->d_diags2, c->plan.diags2));
-    CUC(upload(c, c->d_tab2, c->plan.tab2));
-    CUC(upload(c, c->d_sched, c->plan.sched));
+    CUC(upload(c, c->d_pairs3, c->plan.pairs3));
+    CUC(upload(c, c->d_units3, c->plan.units3));
+    CUC(upload(c, c->d_diags3, c->plan.diags3));
+    CUC(upload(c, c->d_tab3, c->plan.tab3));
+    CUC(upload(c, c->d_chain, c->plan.chain));
     CUC(upload(c, c->d_pair_chans, c->plan.pair_chans));
     {
         // momenta ordered so that q and -q are adjacent (their blocks are shared through L2)
@@ -263,7 +263,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     {
         cudaDeviceProp prop;
         CUX(cudaGetDeviceProperties(&prop, device));
-        if ((size_t)prop.sharedMemPerBlockOptin < PROD2_SMEM) {
+        if ((size_t)prop.sharedMemPerBlockOptin < PROD_SMEM) {
             g_create_error = "device has too little shared memory per block for the product kernel";
             nbs_destroy(c);
             return NBS_ECUDA;
@@ -283,7 +283,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
 
     // workspace: per slice in flight, blocks + elementary correlators + channel correlators
     size_t nchan = c->plan.channels.size();
-    size_t scratch_elems = (size_t)c->prod_grid * c->plan.max_pair_units * 256;
+    size_t scratch_elems = (size_t)c->prod_grid * 2 * c->plan.max_pair_units * 256;
     size_t per_slice = (c->V * (c->R + nchan * 256) + scratch_elems) * sizeof(double2);
     size_t free_b = 0, total_b = 0;
     CUX(cudaMemGetInfo(&free_b, &total_b));
@@ -304,7 +304,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         CUC(dev_alloc(c, cnt, 1));
         c->slice[i].counter = (unsigned long long*)cnt;
     }
-    CUX(cudaFuncSetAttribute(k_product_v2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD2_SMEM));
+    CUX(cudaFuncSetAttribute(k_product, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
     CUX(cudaFuncSetAttribute(k_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)((3 * 144 + 9 * 432) * sizeof(double2))));
     *out = c;
@@ -352,7 +352,7 @@ int nbs_blocks_x(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes,
     if (sl.t != t) return fail(c, NBS_ESTATE, "time slice not loaded");
     if (out_bytes < c->V * BLOCK_ELEMS * sizeof(double2)) return fail(c, NBS_EINVAL, "output buffer too small");
     CU(c, cudaSetDevice(c->device));
-    return launch_blocks(c, sl, c->d_one_baryon + baryon, 1, c->dq_mask_of[baryon], (double2*)out_dev, BLOCK_ELEMS,
+    return launch_blocks(c, sl, c->d_one_baryon + baryon, 1, c->dq_mask_of[baryon], (double2*)out_dev, BLOCK_ELEMS, 0,
                          (cudaStream_t)stream);
 }
 
@@ -375,7 +375,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     int rc;
     {
         StageTimer tm(c, NBS_STAGE_BLOCKS, st);
-        rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
+        rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, 1, st);
         if (rc) return rc;
     }
     {
@@ -387,18 +387,19 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     {
         StageTimer tm(c, NBS_STAGE_PRODUCT, st);
         CU(c, cudaMemsetAsync(sl.counter, 0, sizeof(unsigned long long), st));
-        Prod2Args pa;
+        ProdArgs pa;
         pa.Bq = sl.B; pa.R = c->R; pa.L = c->L;
-        pa.npairs = (int)c->plan.pairs2.size();
-        pa.nitems = (long long)c->V * pa.npairs;
+        pa.npairs = (int)c->plan.pairs3.size();
+        pa.ntasks = (long long)c->V;
         pa.qorder = c->d_qorder;
-        pa.pairs = c->d_pairs2; pa.units = c->d_units2; pa.diags = c->d_diags2; pa.tab = c->d_tab2;
-        pa.sched = c->d_sched; pa.pair_chans = c->d_pair_chans;
+        pa.pairs = c->d_pairs3; pa.units = c->d_units3; pa.diags = c->d_diags3;
+        pa.tab = reinterpret_cast<const uint2*>(c->d_tab3);
+        pa.pair_chans = c->d_pair_chans; pa.chain = c->d_chain;
         pa.scratch = sl.scratch; pa.max_pair_units = c->plan.max_pair_units;
         pa.Ft = sl.Ft; pa.ch_begin = ch_begin; pa.nch_out = (int)nout;
         pa.counter = sl.counter;
-        unsigned grid = (unsigned)std::min<long long>(c->prod_grid, pa.nitems);
-        k_product_v2<<<grid, PROD2_THREADS, PROD2_SMEM, st>>>(pa);
+        unsigned grid = (unsigned)std::min<long long>(c->prod_grid, pa.ntasks);
+        k_product<<<grid, PROD_THREADS, PROD_SMEM, st>>>(pa);
         CU(c, cudaGetLastError());
         ++c->launches;
     }

@@ -2,7 +2,9 @@
 //
 // Data layout in HBM ("site-major"): every stage keeps all components of one lattice site (or
 // momentum q) contiguous:
-//   blocks  B[site][slot][alpha][xi1 xi2 xi3]   (row length R = nslots * 6912 complex)
+//   blocks  B[site][slot][staged block]         (row length R = nslots * 6960 complex; a staged block
+//                                               = 4 sink-spin planes in the padded, skewed layout
+//                                               of nbs_tables.hpp that the product kernel gathers from)
 //   Ft      [q][ch][256]                         channel correlators in momentum space
 // so that (a) the block kernel writes one site's 110 KB per baryon fully coalesced, (b) the FFT
 // runs one 1-D transform per thread with lanes on consecutive components (coalesced, no shared
@@ -52,7 +54,7 @@ __global__ void __launch_bounds__(BLOCKS_THREADS)
 k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const double2* __restrict__ Ss,
          const int* __restrict__ baryon_of_slot, int nslots, unsigned dq_mask,
          const BlockRec* __restrict__ brec, const BTermRec* __restrict__ bterm,
-         double2* __restrict__ out, size_t row_stride) {
+         double2* __restrict__ out, size_t row_stride, int staged) {
     extern __shared__ double2 smem[];
     double2* sS = smem;            // [3][144]
     double2* sD = smem + 3 * 144;  // [9][3][144]
@@ -86,12 +88,29 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
     }
     __syncthreads();
     double2* orow = out + site * row_stride;
-    const int total = nslots * BLOCK_ELEMS;
+    // staged != 0: every (site, slot) row is written in the padded, skewed layout the product
+    // kernel gathers from (nbs_tables.hpp: plane a at a*SM_PLANE, triple at sm_index, pads = 0), so
+    // that staging a block is a plain bulk copy.  staged == 0: [alpha][xi1][xi2][xi3] (nbs_blocks_x).
+    const int row_elems = staged ? SM_BLOCK : BLOCK_ELEMS;
+    const int total = nslots * row_elems;
     for (int idx = tid; idx < total; idx += BLOCKS_THREADS) {
-        int slot = idx / BLOCK_ELEMS;
-        int rem = idx - slot * BLOCK_ELEMS;
-        int al = rem / NTRIPLE, t = rem - al * NTRIPLE;
-        int xi[3] = {t / 144, (t / 12) % 12, t % 12};
+        int slot = idx / row_elems;
+        int rem = idx - slot * row_elems;
+        int al, xi[3];
+        if (staged) {
+            al = rem / SM_PLANE;
+            int w = rem - al * SM_PLANE;
+            xi[0] = w / SM_STRIDE1;
+            w -= xi[0] * SM_STRIDE1;
+            if (w == 144) { orow[idx] = make_double2(0.0, 0.0); continue; } // pad
+            xi[1] = w / 12;
+            int x3 = w - xi[1] * 12 - xi[1];
+            xi[2] = x3 < 0 ? x3 + 12 : x3;
+        } else {
+            al = rem / NTRIPLE;
+            int t = rem - al * NTRIPLE;
+            xi[0] = t / 144; xi[1] = (t / 12) % 12; xi[2] = t % 12;
+        }
         BlockRec br = brec[baryon_of_slot[slot]];
         double2 val = make_double2(0.0, 0.0);
         for (int it = br.term_begin; it < br.term_end; ++it) {

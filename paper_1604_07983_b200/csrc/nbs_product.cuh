@@ -1,81 +1,103 @@
 // (ii)+(iii) EffectiveBaryonBlocks fused into MultiplicationEffectiveBlocks, eqs. 4.2-4.3
-// (PAPER.md:104-115), on the FP64 tensor pipe (DMMA.8x8x4, the native FP64 MMA of sm_100a).
+// (PAPER.md:104-115), on the FP64 tensor path (DMMA.8x8x4, the native FP64 MMA of sm_100a).
 //
 // Per diagram d the sum over the shared index xi~_d is a small complex GEMM (eq. 4.3)
 //     out[m][n] += sum_k  eff1[m][k] * eff2[n][k],   m = (a1, carried spins), n = (a2, carried spins)
-// of shape 16 x 16 x K or 64 x 4 x K (K = 1, 9, 36, 144).  One warp owns a whole
-// diagram: every effective-block entry (a signed sum of 2, 8 or 24 normal-block entries, eq. 4.2)
-// is gathered from shared memory exactly once, straight into the lane that holds it as an MMA
-// fragment, and is then used by 8 output columns through the tensor pipe.  The effective blocks
-// never exist in memory.
+// of shape 16 x 16 x K or 64 x 4 x K (K = 1, 9, 36, 144).  One warp owns a "unit"
+// (a few diagrams, or a k-range of one): every effective-block entry (eq. 4.2: a difference of two
+// sums of 1, 4 or 12 normal-block entries) is gathered from shared memory exactly once, straight
+// into the lane that holds it as an MMA fragment, and is then used by 8 output columns through the
+// tensor path.  The effective blocks never exist in memory.
 //
-// Persistent kernel, one CTA per SM.  A CTA takes work items (momentum q, sink pair) from a global
-// counter; items are ordered so that q and -q are adjacent (B~1(q), B~2(-q) and B~1(-q), B~2(q) of
-// the 14 sink pairs then hit L2).  For an item the CTA stages B~1(q) and B~2(-q) (2 x 110 KB) in
-// shared memory; its warps take "units" (a few diagrams of one elementary correlator with one
-// accumulator layout) from a shared-memory counter, accumulate them in registers and write each
-// unit's 256 spin components to an L2-resident scratch; finally the CTA sums units per elementary
-// correlator and writes the channel correlators (eqs. 2.2-2.3 coefficients) in a fixed order, so
-// the result is bitwise reproducible.
+// Persistent, warp-specialised kernel, one CTA per SM:
+//   * 10 compute warps.  A CTA takes a momentum q from a global counter and walks the sink pairs in
+//     "chain" order (consecutive pairs share B~1(q) or B~2(-q), so only ~15 instead of 28 blocks
+//     are staged per q).  The q-space normal blocks are stored in HBM in exactly the padded,
+//     bank-conflict-free layout the gathers want, so staging is one thread issuing bulk
+//     asynchronous copies (cp.async.bulk, completion on an mbarrier).  Warps take units from a
+//     shared-memory counter, accumulate in registers and write each unit's 256 spin components to
+//     a double-buffered per-CTA scratch.
+//   * 2 epilogue warps.  While the compute warps work on item i+1 they sum the unit results of
+//     item i per elementary correlator in a fixed order (bitwise reproducible) and write the
+//     channel correlators (coefficients of eqs. 2.2-2.3).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <cstddef>
 
 #include "nbs_tables.hpp"
 
 namespace nbs {
 
-constexpr int PROD2_WARPS = 8;
-constexpr int PROD2_THREADS = PROD2_WARPS * 32;
-constexpr size_t PROD2_SMEM = 2 * (size_t)SM_BLOCK * sizeof(double2) + 256;
+constexpr int PROD_CWARPS = 10, PROD_EWARPS = 2;
+constexpr int PROD_CTHREADS = PROD_CWARPS * 32, PROD_ETHREADS = PROD_EWARPS * 32;
+constexpr int PROD_THREADS = PROD_CTHREADS + PROD_ETHREADS;
+constexpr uint32_t PLANE_BYTES = SM_PLANE * 16u;  // 27 840
+constexpr uint32_t BLOCK_BYTES = SM_BLOCK * 16u;  // 111 360
+// shared-memory map (bytes)
+constexpr uint32_t SMO_S1 = 0, SMO_S2 = BLOCK_BYTES, SMO_UNITS = 2 * BLOCK_BYTES;
+constexpr uint32_t SMO_CTRL = SMO_UNITS + MAX_PAIR_UNITS * 16u;
+constexpr size_t PROD_SMEM = SMO_CTRL + 128;
+static_assert(sizeof(Unit3Rec) == 16 && sizeof(Diag3Rec) == 16, "record sizes");
+static_assert(PROD_SMEM <= 232448, "shared memory budget of one SM");
 
+struct ProdCtrl { // at SMO_CTRL
+    unsigned long long mbar1, mbar2; // completion of the bulk copies into s1 / s2
+    int next_unit;                   // work counter of the current item
+    int pad;
+    long long qtask[2];              // prefetched momentum-task indices (alternating slots)
+    int meta_q[2], meta_pair[2];     // item descriptors handed to the epilogue warps
+};
+
+// ---- PTX helpers ----------------------------------------------------------------------------
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
         : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
-
-__device__ __forceinline__ double flip(double v, unsigned s) { // s = 0 or 0x80000000: v or -v
-    return __hiloint2double(__double2hiint(v) ^ (int)s, __double2loint(v));
+__device__ __forceinline__ double dneg(double v) {
+    return __hiloint2double(__double2hiint(v) ^ (int)0x80000000u, __double2loint(v));
 }
-__device__ __forceinline__ double2 flip2(double2 v, unsigned s) { return make_double2(flip(v.x, s), flip(v.y, s)); }
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, uint32_t parity) {
+    const uint32_t a = smem_u32(bar);
+    uint32_t ok = 0;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, void* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void named_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void named_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+enum { BAR_COMPUTE = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4 };
 
-// One table word = two gather terms (bit 15 / 31: minus sign; low 11 bits: sm_index of the triple).
-// raw_load issues the shared-memory loads for NP sink-spin planes, raw_add folds them (signed) into
-// out: splitting the two lets the loads of the next k-step fly under the MMAs of the current one.
-template <int NP>
-__device__ __forceinline__ void raw_load(const double2* __restrict__ base, int stride, uint32_t w,
-                                         double2 (&u)[NP], double2 (&v)[NP]) {
-    const unsigned i0 = w & 0x7ffu, i1 = (w >> 16) & 0x7ffu;
+// ---- gathers (eq. 4.2) ----------------------------------------------------------------------
+// One table word = one (+, -) pair of byte offsets into a staged block.  ld_pair issues the
+// shared-memory loads for NP sink-spin planes (plane stride PS bytes), sub_pair folds them.
+template <int NP, uint32_t PS>
+__device__ __forceinline__ void ld_pair(const char* __restrict__ blk, uint2 w, double2 (&u)[NP], double2 (&v)[NP]) {
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
-        u[p] = base[p * stride + i0];
-        v[p] = base[p * stride + i1];
+        u[p] = *reinterpret_cast<const double2*>(blk + w.x + p * PS);
+        v[p] = *reinterpret_cast<const double2*>(blk + w.y + p * PS);
     }
 }
 template <int NP, bool FIRST>
-__device__ __forceinline__ void raw_add(uint32_t w, const double2 (&u)[NP], const double2 (&v)[NP],
-                                        double2 (&out)[NP]) {
-    const unsigned s0 = (w & 0x8000u) << 16, s1 = w & 0x80000000u;
+__device__ __forceinline__ void sub_pair(const double2 (&u)[NP], const double2 (&v)[NP], double2 (&out)[NP]) {
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
-        const double2 a = flip2(u[p], s0), b = flip2(v[p], s1);
-        if (FIRST) out[p] = make_double2(a.x + b.x, a.y + b.y);
-        else { out[p].x += a.x + b.x; out[p].y += a.y + b.y; }
-    }
-}
-
-// Signed gather of one effective-block entry (eq. 4.2) with a run-time number of table words.
-template <int NP>
-__device__ __forceinline__ void gather(const double2* __restrict__ base, int stride,
-                                       const uint32_t* __restrict__ words, int nw, double2 (&out)[NP]) {
-    double2 u[NP], v[NP];
-    uint32_t w = __ldg(words);
-    raw_load<NP>(base, stride, w, u, v);
-    raw_add<NP, true>(w, u, v, out);
-    for (int j = 1; j < nw; ++j) {
-        w = __ldg(words + j);
-        raw_load<NP>(base, stride, w, u, v);
-        raw_add<NP, false>(w, u, v, out);
+        if (FIRST) out[p] = make_double2(u[p].x - v[p].x, u[p].y - v[p].y);
+        else { out[p].x += u[p].x - v[p].x; out[p].y += u[p].y - v[p].y; }
     }
 }
 
@@ -86,7 +108,7 @@ struct AccSquare {
     double re[2][2][2], im[2][2][2];
 };
 __device__ __forceinline__ void mma_square(AccSquare& c, const double2 (&A)[2], const double2 (&B)[2]) {
-    const double nBy[2] = {flip(B[0].y, 0x80000000u), flip(B[1].y, 0x80000000u)};
+    const double nBy[2] = {dneg(B[0].y), dneg(B[1].y)};
 #pragma unroll
     for (int i = 0; i < 2; ++i)
 #pragma unroll
@@ -103,48 +125,62 @@ __device__ __forceinline__ void mma_square(AccSquare& c, const double2 (&A)[2], 
         }
 }
 
-__device__ __forceinline__ void run_unit_square(const Unit2Rec u, const Diag2Rec* __restrict__ diags,
-                                                const uint32_t* __restrict__ tab, const double2* s1,
-                                                const double2* s2, double2* __restrict__ out, int lane) {
-    const int r = lane >> 2, kk = lane & 3, c = r >> 1;
-    const double2* pA = s1 + (r & 1) * SM_PLANE;
-    const double2* pB = s2 + (r & 1) * SM_PLANE;
-    const double2 zero = make_double2(0.0, 0.0);
+__device__ __forceinline__ Diag3Rec load_diag(const Diag3Rec* __restrict__ p) {
+    const int4 v = __ldg(reinterpret_cast<const int4*>(p));
+    Diag3Rec d;
+    d.offA = (uint32_t)v.x; d.offB = (uint32_t)v.y;
+    d.sbeg = (uint16_t)((uint32_t)v.z & 0xffffu); d.send = (uint16_t)((uint32_t)v.z >> 16);
+    d.nwA = (uint8_t)((uint32_t)v.w & 0xffu); d.nwB = (uint8_t)(((uint32_t)v.w >> 8) & 0xffu);
+    d.K = (uint16_t)((uint32_t)v.w >> 16);
+    return d;
+}
+
+__device__ __forceinline__ void run_unit_square(const Unit3Rec u, const Diag3Rec* __restrict__ diags,
+                                                const uint2* __restrict__ tab, const char* s1, const char* s2,
+                                                double2* __restrict__ out, int lane) {
+    const int r = lane >> 2, kk = lane & 3;
+    constexpr uint32_t PS = 2 * PLANE_BYTES;
     AccSquare acc = {};
     for (int d = u.diag_begin; d < u.diag_end; ++d) {
-        const Diag2Rec dr = diags[d];
-        if (dr.nA == 2 && dr.nB == 2) {
+        const Diag3Rec dr = load_diag(diags + d);
+        const int nsteps = dr.send - dr.sbeg;
+        if (dr.nwA == 1) {
             // software pipeline: table words two k-steps ahead, shared-memory gathers one ahead
-            const uint32_t* tA = tab + dr.offA + (dr.kbeg + kk) * 4 + c;
-            const uint32_t* tB = tab + dr.offB + (dr.kbeg + kk) * 4 + c;
-            uint32_t wa = __ldg(tA), wb = __ldg(tB);
+            const uint2* tA = tab + dr.offA + (dr.sbeg * 4 + kk) * 8 + r;
+            const uint2* tB = tab + dr.offB + (dr.sbeg * 4 + kk) * 8 + r;
+            uint2 wa = __ldg(tA), wb = __ldg(tB);
+            uint2 na = __ldg(tA + 32), nb = __ldg(tB + 32);
             double2 A[2], B[2], ua[2], va[2], ub[2], vb[2];
-            raw_load<2>(pA, 2 * SM_PLANE, wa, ua, va);
-            raw_load<2>(pB, 2 * SM_PLANE, wb, ub, vb);
-            uint32_t na = __ldg(tA + 16), nb = __ldg(tB + 16);
-            raw_add<2, true>(wa, ua, va, A);
-            raw_add<2, true>(wb, ub, vb, B);
-            if (dr.kbeg + kk >= dr.K) A[0] = A[1] = B[0] = B[1] = zero;
-            for (int k0 = dr.kbeg; k0 < dr.kend; k0 += 4) {
-                tA += 16; tB += 16;
+            ld_pair<2, PS>(s1, wa, ua, va);
+            ld_pair<2, PS>(s2, wb, ub, vb);
+            sub_pair<2, true>(ua, va, A);
+            sub_pair<2, true>(ub, vb, B);
+            for (int s = 0; s < nsteps; ++s) {
+                tA += 32; tB += 32;
                 wa = na; wb = nb;
-                raw_load<2>(pA, 2 * SM_PLANE, wa, ua, va);
-                raw_load<2>(pB, 2 * SM_PLANE, wb, ub, vb);
-                na = __ldg(tA + 16); nb = __ldg(tB + 16);
+                ld_pair<2, PS>(s1, wa, ua, va); // one step past the end reads a valid (unused) entry
+                ld_pair<2, PS>(s2, wb, ub, vb);
+                na = __ldg(tA + 32); nb = __ldg(tB + 32);
                 mma_square(acc, A, B);
-                raw_add<2, true>(wa, ua, va, A);
-                raw_add<2, true>(wb, ub, vb, B);
-                if (k0 + 4 + kk >= dr.K) A[0] = A[1] = B[0] = B[1] = zero;
+                sub_pair<2, true>(ua, va, A);
+                sub_pair<2, true>(ub, vb, B);
             }
         } else {
-            const int nwA = dr.nA >> 1, nwB = dr.nB >> 1;
-            const uint32_t* tA = tab + dr.offA + ((dr.kbeg + kk) * 4 + c) * nwA;
-            const uint32_t* tB = tab + dr.offB + ((dr.kbeg + kk) * 4 + c) * nwB;
-            for (int k0 = dr.kbeg; k0 < dr.kend; k0 += 4, tA += 16 * nwA, tB += 16 * nwB) {
-                double2 A[2], B[2];
-                gather<2>(pA, 2 * SM_PLANE, tA, nwA, A);
-                gather<2>(pB, 2 * SM_PLANE, tB, nwB, B);
-                if (k0 + kk >= dr.K) A[0] = A[1] = B[0] = B[1] = zero; // padded k: contributes nothing
+            const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry)
+            const uint2* tA = tab + dr.offA + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
+            const uint2* tB = tab + dr.offB + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
+            for (int s = 0; s < nsteps; ++s, tA += 32 * nw, tB += 32 * nw) {
+                double2 A[2], B[2], ua[2], va[2], ub[2], vb[2];
+                ld_pair<2, PS>(s1, __ldg(tA), ua, va);
+                ld_pair<2, PS>(s2, __ldg(tB), ub, vb);
+                sub_pair<2, true>(ua, va, A);
+                sub_pair<2, true>(ub, vb, B);
+                for (int j = 1; j < nw; ++j) {
+                    ld_pair<2, PS>(s1, __ldg(tA + j), ua, va);
+                    ld_pair<2, PS>(s2, __ldg(tB + j), ub, vb);
+                    sub_pair<2, false>(ua, va, A);
+                    sub_pair<2, false>(ub, vb, B);
+                }
                 mma_square(acc, A, B);
             }
         }
@@ -169,7 +205,7 @@ __device__ __forceinline__ void run_unit_square(const Unit2Rec u, const Diag2Rec
 //   C += Ar [Br | Bi];  C += Ai [-Bi | Br].
 __device__ __forceinline__ void mma_wide(double (&acc)[8][2], const double2 (&A)[4][2], double2 Bv, int hi) {
     const double b1 = hi ? Bv.y : Bv.x;
-    const double b2 = hi ? Bv.x : flip(Bv.y, 0x80000000u);
+    const double b2 = hi ? Bv.x : dneg(Bv.y);
 #pragma unroll
     for (int g = 0; g < 4; ++g)
 #pragma unroll
@@ -180,88 +216,59 @@ __device__ __forceinline__ void mma_wide(double (&acc)[8][2], const double2 (&A)
         for (int j = 0; j < 2; ++j) dmma884(acc[j * 4 + g][0], acc[j * 4 + g][1], A[g][j].y, b2);
 }
 
-__device__ __forceinline__ void run_unit_wide(const Unit2Rec u, const Diag2Rec* __restrict__ diags,
-                                              const uint32_t* __restrict__ tab, const double2* s1,
-                                              const double2* s2, double2* __restrict__ out, int lane) {
-    const int r = lane >> 2, kk = lane & 3, aY = r & 3, hi = r >> 2, cg = r >> 1;
-    const double2* pA = (u.cls == 2 ? s1 : s2) + (r & 1) * SM_PLANE;
-    const double2* pB = (u.cls == 2 ? s2 : s1) + aY * SM_PLANE;
-    const double2 zero = make_double2(0.0, 0.0);
+// Table words of one k-step of one lane: 4 A entries (g) and the 4 term pairs of the B entry.
+__device__ __forceinline__ void wide_loads_A(const char* sA, uint4 a01, uint4 a23, double2 (&ua)[4][2], double2 (&va)[4][2]) {
+    constexpr uint32_t PS = 2 * PLANE_BYTES;
+    ld_pair<2, PS>(sA, make_uint2(a01.x, a01.y), ua[0], va[0]);
+    ld_pair<2, PS>(sA, make_uint2(a01.z, a01.w), ua[1], va[1]);
+    ld_pair<2, PS>(sA, make_uint2(a23.x, a23.y), ua[2], va[2]);
+    ld_pair<2, PS>(sA, make_uint2(a23.z, a23.w), ua[3], va[3]);
+}
+__device__ __forceinline__ void wide_loads_B(const char* sB, uint4 b01, uint4 b23, double2 (&ub)[4][1], double2 (&vb)[4][1]) {
+    ld_pair<1, 0>(sB, make_uint2(b01.x, b01.y), ub[0], vb[0]);
+    ld_pair<1, 0>(sB, make_uint2(b01.z, b01.w), ub[1], vb[1]);
+    ld_pair<1, 0>(sB, make_uint2(b23.x, b23.y), ub[2], vb[2]);
+    ld_pair<1, 0>(sB, make_uint2(b23.z, b23.w), ub[3], vb[3]);
+}
+__device__ __forceinline__ void wide_fold_B(const double2 (&ub)[4][1], const double2 (&vb)[4][1], double2 (&Bv)[1]) {
+    sub_pair<1, true>(ub[0], vb[0], Bv);
+    sub_pair<1, false>(ub[1], vb[1], Bv);
+    sub_pair<1, false>(ub[2], vb[2], Bv);
+    sub_pair<1, false>(ub[3], vb[3], Bv);
+}
+
+__device__ __forceinline__ void run_unit_wide(const Unit3Rec u, const Diag3Rec* __restrict__ diags,
+                                              const uint2* __restrict__ tab, const char* s1, const char* s2,
+                                              double2* __restrict__ out, int lane) {
+    const int r = lane >> 2, kk = lane & 3, aY = r & 3, hi = r >> 2;
+    const char* sA = (u.cls == 2) ? s1 : s2;
+    const char* sB = (u.cls == 2) ? s2 : s1;
     double acc[8][2] = {};
     for (int d = u.diag_begin; d < u.diag_end; ++d) {
-        const Diag2Rec dr = diags[d];
-        if (dr.nA == 2 && dr.nB == 8) {
-            const uint32_t* tA = tab + dr.offA + (dr.kbeg + kk) * 16 + cg;
-            const uint4* tB = reinterpret_cast<const uint4*>(tab + dr.offB) + (dr.kbeg + kk);
-            uint32_t wa[4];
-            uint4 wb = __ldg(tB);
+        const Diag3Rec dr = load_diag(diags + d); // nwA == 1, nwB == 4 (checked by the table generator)
+        const int nsteps = dr.send - dr.sbeg;
+        // A table [k][r][g] (4 uint2 = 2 uint4 per lane), B table [k][aY][4 pairs] (2 uint4 per lane)
+        const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA) + ((dr.sbeg * 4 + kk) * 8 + r) * 2;
+        const uint4* tB = reinterpret_cast<const uint4*>(tab + dr.offB) + ((dr.sbeg * 4 + kk) * 4 + aY) * 2;
+        // software pipeline: table words one k-step ahead; the A gathers of step s+1 fly under the
+        // MMAs of step s, the (8-term) B gather of step s+1 is issued after them and folded at the
+        // top of step s+1 (keeps the live registers under the 168 available per thread)
+        double2 A[4][2], Bv[1], ua[4][2], va[4][2], ub[4][1], vb[4][1];
+        wide_loads_A(sA, __ldg(tA), __ldg(tA + 1), ua, va);
+        wide_loads_B(sB, __ldg(tB), __ldg(tB + 1), ub, vb);
+        uint4 na01 = __ldg(tA + 64), na23 = __ldg(tA + 65), nb01 = __ldg(tB + 32), nb23 = __ldg(tB + 33);
 #pragma unroll
-            for (int g = 0; g < 4; ++g) wa[g] = __ldg(tA + 4 * g);
-            double2 A[4][2], Bv[1], ua[4][2], va[4][2], ub[4][1], vb[4][1];
+        for (int g = 0; g < 4; ++g) sub_pair<2, true>(ua[g], va[g], A[g]);
+        for (int s = 0; s < nsteps; ++s) {
+            tA += 64; tB += 32;
+            wide_fold_B(ub, vb, Bv);
+            wide_loads_A(sA, na01, na23, ua, va); // one step past the end reads valid (unused) entries
+            na01 = __ldg(tA + 64); na23 = __ldg(tA + 65);
+            mma_wide(acc, A, Bv[0], hi);
 #pragma unroll
-            for (int g = 0; g < 4; ++g) raw_load<2>(pA, 2 * SM_PLANE, wa[g], ua[g], va[g]);
-            raw_load<1>(pB, 0, wb.x, ub[0], vb[0]);
-            raw_load<1>(pB, 0, wb.y, ub[1], vb[1]);
-            raw_load<1>(pB, 0, wb.z, ub[2], vb[2]);
-            raw_load<1>(pB, 0, wb.w, ub[3], vb[3]);
-            uint32_t na[4];
-            uint4 nb = __ldg(tB + 4);
-#pragma unroll
-            for (int g = 0; g < 4; ++g) na[g] = __ldg(tA + 64 + 4 * g);
-#pragma unroll
-            for (int g = 0; g < 4; ++g) raw_add<2, true>(wa[g], ua[g], va[g], A[g]);
-            raw_add<1, true>(wb.x, ub[0], vb[0], Bv);
-            raw_add<1, false>(wb.y, ub[1], vb[1], Bv);
-            raw_add<1, false>(wb.z, ub[2], vb[2], Bv);
-            raw_add<1, false>(wb.w, ub[3], vb[3], Bv);
-            if (dr.kbeg + kk >= dr.K) {
-#pragma unroll
-                for (int g = 0; g < 4; ++g) A[g][0] = A[g][1] = zero;
-                Bv[0] = zero;
-            }
-            for (int k0 = dr.kbeg; k0 < dr.kend; k0 += 4) {
-                tA += 64; tB += 4;
-#pragma unroll
-                for (int g = 0; g < 4; ++g) wa[g] = na[g];
-                wb = nb;
-#pragma unroll
-                for (int g = 0; g < 4; ++g) raw_load<2>(pA, 2 * SM_PLANE, wa[g], ua[g], va[g]);
-                raw_load<1>(pB, 0, wb.x, ub[0], vb[0]);
-                raw_load<1>(pB, 0, wb.y, ub[1], vb[1]);
-                raw_load<1>(pB, 0, wb.z, ub[2], vb[2]);
-                raw_load<1>(pB, 0, wb.w, ub[3], vb[3]);
-                nb = __ldg(tB + 4);
-#pragma unroll
-                for (int g = 0; g < 4; ++g) na[g] = __ldg(tA + 64 + 4 * g);
-                mma_wide(acc, A, Bv[0], hi);
-#pragma unroll
-                for (int g = 0; g < 4; ++g) raw_add<2, true>(wa[g], ua[g], va[g], A[g]);
-                raw_add<1, true>(wb.x, ub[0], vb[0], Bv);
-                raw_add<1, false>(wb.y, ub[1], vb[1], Bv);
-                raw_add<1, false>(wb.z, ub[2], vb[2], Bv);
-                raw_add<1, false>(wb.w, ub[3], vb[3], Bv);
-                if (k0 + 4 + kk >= dr.K) {
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) A[g][0] = A[g][1] = zero;
-                    Bv[0] = zero;
-                }
-            }
-        } else {
-            const int nwA = dr.nA >> 1, nwB = dr.nB >> 1;
-            const uint32_t* tA = tab + dr.offA + ((dr.kbeg + kk) * 16 + cg) * nwA;
-            const uint32_t* tB = tab + dr.offB + (dr.kbeg + kk) * nwB;
-            for (int k0 = dr.kbeg; k0 < dr.kend; k0 += 4, tA += 64 * nwA, tB += 4 * nwB) {
-                double2 A[4][2], Bv[1];
-#pragma unroll
-                for (int g = 0; g < 4; ++g) gather<2>(pA, 2 * SM_PLANE, tA + 4 * g * nwA, nwA, A[g]);
-                gather<1>(pB, 0, tB, nwB, Bv);
-                if (k0 + kk >= dr.K) {
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) A[g][0] = A[g][1] = zero;
-                    Bv[0] = zero;
-                }
-                mma_wide(acc, A, Bv[0], hi);
-            }
+            for (int g = 0; g < 4; ++g) sub_pair<2, true>(ua[g], va[g], A[g]);
+            wide_loads_B(sB, nb01, nb23, ub, vb);
+            nb01 = __ldg(tB + 32); nb23 = __ldg(tB + 33);
         }
     }
     double* o = reinterpret_cast<double*>(out);
@@ -278,117 +285,188 @@ __device__ __forceinline__ void run_unit_wide(const Unit2Rec u, const Diag2Rec* 
             }
 }
 
-struct Prod2Args {
-    const double2* Bq;   // [V][R] momentum-space normal blocks
-    size_t R;
+struct ProdArgs {
+    const double2* Bq;   // [V][R] momentum-space normal blocks, every (site, slot) row in the staged layout
+    size_t R;            // row length (complex) = nslots * SM_BLOCK
     int L;
     int npairs;
-    long long nitems;    // V * npairs
+    long long ntasks;    // V momentum tasks
     const int* qorder;   // [V] momenta with q and -q adjacent
-    const Pair2Rec* pairs;
-    const Unit2Rec* units;
-    const Diag2Rec* diags;
-    const uint32_t* tab;
-    const int* sched;
+    const Pair3Rec* pairs;
+    const Unit3Rec* units;
+    const Diag3Rec* diags;
+    const uint2* tab;
     const PairChanRec* pair_chans;
-    double2* scratch;    // [gridDim.x][max_pair_units][256]
+    const ChainRec* chain; // [npairs]
+    double2* scratch;    // [gridDim.x][2][max_pair_units][256]
     int max_pair_units;
     double2* Ft;         // [V][nch_out][256]
     int ch_begin, nch_out;
     unsigned long long* counter; // zeroed before the launch
 };
 
-__device__ __forceinline__ size_t minus_q2(int L, size_t q) {
+__device__ __forceinline__ size_t minus_q(int L, size_t q) {
     int x = (int)(q % L), y = (int)((q / L) % L), z = (int)(q / ((size_t)L * L));
     x = x ? L - x : 0; y = y ? L - y : 0; z = z ? L - z : 0;
     return x + (size_t)L * (y + (size_t)L * z);
 }
 
-// global block element i = a*1728 + (xi1*12 + xi2)*12 + xi3  ->  staged position (sm_index)
-__device__ __forceinline__ int staged_index(int i) {
-    const int a = i / NTRIPLE, t = i - a * NTRIPLE;
-    const int xi1 = t / 144, rem = t - xi1 * 144, xi2 = rem / 12, xi3 = rem - xi2 * 12;
-    int x3 = xi3 + xi2;
-    x3 = x3 >= 12 ? x3 - 12 : x3;
-    return a * SM_PLANE + xi1 * SM_STRIDE1 + xi2 * 12 + x3;
-}
-
-__global__ void __launch_bounds__(PROD2_THREADS, 1) k_product_v2(const Prod2Args a) {
-    extern __shared__ double2 smem[];
-    double2* s1 = smem;
-    double2* s2 = smem + SM_BLOCK;
-    Pair2Rec* s_pr = reinterpret_cast<Pair2Rec*>(smem + 2 * SM_BLOCK); // 100 bytes
-    long long* s_item = reinterpret_cast<long long*>(reinterpret_cast<char*>(s_pr) + 128);
-    int* s_next = reinterpret_cast<int*>(s_item + 1);
-    const int tid = threadIdx.x, lane = tid & 31;
-    double2* scr = a.scratch + (size_t)blockIdx.x * a.max_pair_units * 256;
-
-    for (;;) {
-        __syncthreads(); // previous item fully consumed (shared memory, scratch)
-        if (tid == 0) {
-            *s_item = (long long)atomicAdd(a.counter, 1ull);
-            *s_next = 0;
-        }
-        __syncthreads();
-        const long long item = *s_item;
-        if (item >= a.nitems) break;
-        const size_t q = (size_t)a.qorder[item / a.npairs];
-        const int ip = (int)(item % a.npairs);
-        if (tid < (int)(sizeof(Pair2Rec) / sizeof(int)))
-            reinterpret_cast<int*>(s_pr)[tid] = reinterpret_cast<const int*>(a.pairs + ip)[tid];
-        {
-            const double2* g1 = a.Bq + q * a.R + (size_t)a.pairs[ip].slot1 * BLOCK_ELEMS;
-            const double2* g2 = a.Bq + minus_q2(a.L, q) * a.R + (size_t)a.pairs[ip].slot2 * BLOCK_ELEMS;
-#pragma unroll 3
-            for (int i = tid; i < BLOCK_ELEMS; i += PROD2_THREADS) { // 6912 = 27 * 256
-                const int j = staged_index(i);
-                const double2 v1 = __ldcs(g1 + i), v2 = __ldcs(g2 + i);
-                s1[j] = v1;
-                s2[j] = v2;
+// Epilogue of one item: elementary correlators = sums of unit results (fixed order), channel
+// correlators = real combinations of them (eqs. 2.2-2.3) -> Ft[q][ch][256].
+__device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* __restrict__ pr, size_t q,
+                                             const double2* __restrict__ scr, int et) {
+    constexpr int CG = 4; // channels per pass over the unit results
+    const int nelem = pr->nelem, nchan = pr->nchan;
+    for (int c0 = 0; c0 < nchan; c0 += CG) {
+        double2 acc[CG][4];
+#pragma unroll
+        for (int c = 0; c < CG; ++c)
+#pragma unroll
+            for (int m = 0; m < 4; ++m) acc[c][m] = make_double2(0.0, 0.0);
+        for (int e = 0; e < nelem; ++e) {
+            double2 s[4];
+#pragma unroll
+            for (int m = 0; m < 4; ++m) s[m] = make_double2(0.0, 0.0);
+            const int ub = pr->elem_unit_begin[e], ue = pr->elem_unit_begin[e + 1];
+#pragma unroll 4
+            for (int ul = ub; ul < ue; ++ul) {
+#pragma unroll
+                for (int m = 0; m < 4; ++m) {
+                    const double2 v = __ldcg(scr + (size_t)ul * 256 + et + 64 * m);
+                    s[m].x += v.x;
+                    s[m].y += v.y;
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < CG; ++c) {
+                if (c0 + c < nchan) {
+                    const double k = __ldg(&a.pair_chans[pr->chan_begin + c0 + c].coef[e]);
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        acc[c][m].x = fma(k, s[m].x, acc[c][m].x);
+                        acc[c][m].y = fma(k, s[m].y, acc[c][m].y);
+                    }
+                }
             }
         }
-        __syncthreads();
-        const int nunits = s_pr->nunits;
-        const Unit2Rec* units = a.units + s_pr->unit_begin;
-        const int* sched = a.sched + s_pr->sched_begin;
+#pragma unroll
+        for (int c = 0; c < CG; ++c) {
+            if (c0 + c < nchan) {
+                const int ch = __ldg(&a.pair_chans[pr->chan_begin + c0 + c].ch) - a.ch_begin;
+                if (ch >= 0 && ch < a.nch_out) {
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) __stcs(a.Ft + (q * a.nch_out + ch) * 256 + et + 64 * m, acc[c][m]);
+                }
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
+    extern __shared__ __align__(128) char prod_smem[];
+    char* smem = prod_smem;
+    char* s1 = smem + SMO_S1;
+    char* s2 = smem + SMO_S2;
+    Unit3Rec* s_units = reinterpret_cast<Unit3Rec*>(smem + SMO_UNITS);
+    volatile ProdCtrl* ctl = reinterpret_cast<volatile ProdCtrl*>(smem + SMO_CTRL);
+    void* mbar1 = smem + SMO_CTRL + offsetof(ProdCtrl, mbar1);
+    void* mbar2 = smem + SMO_CTRL + offsetof(ProdCtrl, mbar2);
+    int* next_unit = reinterpret_cast<int*>(smem + SMO_CTRL + offsetof(ProdCtrl, next_unit));
+    const int tid = threadIdx.x;
+    const size_t scr_stride = (size_t)a.max_pair_units * 256;
+    double2* scr0 = a.scratch + (size_t)blockIdx.x * 2 * scr_stride;
+
+    if (tid == 0) {
+        mbar_init(mbar1, 1);
+        mbar_init(mbar2, 1);
+        ctl->qtask[0] = (long long)atomicAdd(a.counter, 1ull);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (tid >= PROD_CTHREADS) {
+        // ---------------- epilogue warps: combine item i while the compute warps run item i+1
+        const int et = tid - PROD_CTHREADS;
+        for (unsigned it = 0;; ++it) {
+            const int b = it & 1;
+            named_sync(BAR_FULL0 + b, PROD_THREADS);
+            const int ip = ctl->meta_pair[b];
+            if (ip < 0) break;
+            const size_t q = (size_t)ctl->meta_q[b];
+            combine_item(a, a.pairs + ip, q, scr0 + b * scr_stride, et);
+            named_arrive(BAR_EMPTY0 + b, PROD_THREADS);
+        }
+        return;
+    }
+
+    // ---------------- compute warps
+    const int lane = tid & 31;
+    uint32_t ph1 = 0, ph2 = 0; // phase parities of the two staging barriers
+    int pos = 0;               // position in the chain of sink pairs
+    unsigned ntask = 0;
+    long long qt = 0;
+    size_t q = 0, mq = 0;
+    for (unsigned it = 0;; ++it) {
+        const int b = it & 1;
+        named_sync(BAR_COMPUTE, PROD_CTHREADS); // the staged blocks and unit records of the previous item are consumed
+        if (pos == 0) {
+            qt = ctl->qtask[ntask & 1];
+            if (qt < a.ntasks) {
+                q = (size_t)__ldg(a.qorder + qt);
+                mq = minus_q(a.L, q);
+            }
+        }
+        if (it >= 2) named_sync(BAR_EMPTY0 + b, PROD_THREADS); // scratch buffer b and its descriptor are free again
+        if (qt >= a.ntasks) { // no work left: tell the epilogue warps and leave
+            if (tid == 0) ctl->meta_pair[b] = -1;
+            __threadfence_block();
+            named_arrive(BAR_FULL0 + b, PROD_THREADS);
+            break;
+        }
+        const int ip = __ldg(&a.chain[pos].pair);
+        const int load1 = __ldg(&a.chain[pos].load1), load2 = __ldg(&a.chain[pos].load2);
+        const Pair3Rec* pr = a.pairs + ip;
+        const int nunits = __ldg(&pr->nunits);
+        if (tid == 0) {
+            if (pos == 0) ctl->qtask[(ntask + 1) & 1] = (long long)atomicAdd(a.counter, 1ull); // next momentum task
+            *next_unit = 0;
+            ctl->meta_q[b] = (int)q;
+            ctl->meta_pair[b] = ip;
+            const uint32_t ubytes = (uint32_t)nunits * (uint32_t)sizeof(Unit3Rec);
+            const Unit3Rec* usrc = a.units + __ldg(&pr->unit_begin);
+            if (load1) {
+                const char* g1 = reinterpret_cast<const char*>(a.Bq + q * a.R + (size_t)__ldg(&pr->slot1) * SM_BLOCK);
+                mbar_expect_tx(mbar1, BLOCK_BYTES + ubytes);
+                bulk_g2s(s_units, usrc, ubytes, mbar1);
+#pragma unroll
+                for (int p = 0; p < 4; ++p) bulk_g2s(s1 + p * PLANE_BYTES, g1 + p * PLANE_BYTES, PLANE_BYTES, mbar1);
+            }
+            if (load2) {
+                const char* g2 = reinterpret_cast<const char*>(a.Bq + mq * a.R + (size_t)__ldg(&pr->slot2) * SM_BLOCK);
+                mbar_expect_tx(mbar2, BLOCK_BYTES + (load1 ? 0u : ubytes));
+                if (!load1) bulk_g2s(s_units, usrc, ubytes, mbar2);
+#pragma unroll
+                for (int p = 0; p < 4; ++p) bulk_g2s(s2 + p * PLANE_BYTES, g2 + p * PLANE_BYTES, PLANE_BYTES, mbar2);
+            }
+        }
+        if (load1) { mbar_wait(mbar1, ph1); ph1 ^= 1u; }
+        if (load2) { mbar_wait(mbar2, ph2); ph2 ^= 1u; }
+        double2* scr = scr0 + b * scr_stride;
         for (;;) {
             int i = 0;
-            if (lane == 0) i = atomicAdd(s_next, 1);
+            if (lane == 0) i = atomicAdd(next_unit, 1);
             i = __shfl_sync(0xffffffffu, i, 0);
             if (i >= nunits) break;
-            const int ul = sched[i];
-            const Unit2Rec u = units[ul];
-            double2* out = scr + (size_t)ul * 256;
+            const int4 uv = *reinterpret_cast<const int4*>(s_units + i);
+            Unit3Rec u;
+            u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
+            double2* out = scr + (size_t)u.slot * 256;
             if (u.cls < 2) run_unit_square(u, a.diags, a.tab, s1, s2, out, lane);
             else run_unit_wide(u, a.diags, a.tab, s1, s2, out, lane);
         }
-        __syncthreads(); // all units of this item are in the scratch
-        {
-            double2 es[MAX_PAIR_ELEMS];
-#pragma unroll
-            for (int e = 0; e < MAX_PAIR_ELEMS; ++e) {
-                es[e] = make_double2(0.0, 0.0);
-                if (e < s_pr->nelem)
-                    for (int ul = s_pr->elem_unit_begin[e]; ul < s_pr->elem_unit_begin[e + 1]; ++ul) {
-                        const double2 v = __ldcg(scr + (size_t)ul * 256 + tid);
-                        es[e].x += v.x;
-                        es[e].y += v.y;
-                    }
-            }
-            for (int c = 0; c < s_pr->nchan; ++c) {
-                const PairChanRec* pc = a.pair_chans + s_pr->chan_begin + c;
-                const int ch = pc->ch - a.ch_begin;
-                if (ch < 0 || ch >= a.nch_out) continue;
-                double2 acc = make_double2(0.0, 0.0);
-#pragma unroll
-                for (int e = 0; e < MAX_PAIR_ELEMS; ++e) {
-                    const double k = pc->coef[e];
-                    acc.x = fma(k, es[e].x, acc.x);
-                    acc.y = fma(k, es[e].y, acc.y);
-                }
-                __stcs(a.Ft + (q * a.nch_out + ch) * 256 + tid, acc);
-            }
-        }
+        __threadfence_block();
+        named_arrive(BAR_FULL0 + b, PROD_THREADS); // unit results of this item are in scratch buffer b
+        if (++pos == a.npairs) { pos = 0; ++ntask; }
     }
 }
 

@@ -405,109 +405,177 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         plan.chan_term_begin.push_back((int)plan.chan_terms.size());
     }
 
-    // ---- v2 (DMMA) tables: pairs -> (<= MAX_PAIR_ELEMS elementary correlators) -> units -> diagrams
-    std::map<std::vector<uint32_t>, uint32_t> dedupe2;
-    auto intern2 = [&](const SideTable& t) {
-        // [c][k][term] u16  ->  [k][c][term/2] u32, k padded to a multiple of 4
+    // ---- product kernel tables: pairs -> (<= MAX_PAIR_ELEMS elementary correlators) -> units -> diagrams
+    // layout: 0 = 16x16 side, 1 = 64x4 A side, 2 = 64x4 B side (see nbs_tables.hpp)
+    std::map<std::vector<uint32_t>, uint32_t> dedupe3;
+    std::string tab_err;
+    auto intern3 = [&](const SideTable& t, int layout) -> uint32_t {
         const int Kp = (t.K + 3) / 4 * 4, nw = t.n / 2;
-        std::vector<uint32_t> w((size_t)Kp * t.C * nw, 0u);
+        const int rows = (layout == 2) ? 4 : 8, G = (layout == 1) ? 4 : 1;
+        // padded k (k >= K): off+ == off- == 0.  One extra all-zero k-step closes every table: the
+        // kernel's software pipeline gathers one k-step past the end of a unit's range, and those
+        // (unused) gathers must not pick up offsets of a following table with another layout.
+        std::vector<uint32_t> w((size_t)(Kp + 4) * rows * G * nw * 2, 0u);
         for (int k = 0; k < t.K; ++k)
-            for (int c = 0; c < t.C; ++c)
-                for (int j = 0; j < nw; ++j) {
-                    size_t src = ((size_t)c * t.K + k) * t.n + 2 * j;
-                    w[((size_t)k * t.C + c) * nw + j] = (uint32_t)t.g[src] | ((uint32_t)t.g[src + 1] << 16);
+            for (int r = 0; r < rows; ++r)
+                for (int g = 0; g < G; ++g) {
+                    // carried index and sink-spin plane folded into the byte offset
+                    const int c = (layout == 0) ? (r >> 1) : (layout == 1) ? 4 * g + (r >> 1) : 0;
+                    const int plane = (layout == 2) ? r : (r & 1);
+                    std::vector<uint32_t> plus, minus;
+                    for (int j = 0; j < t.n; ++j) {
+                        const uint16_t e = t.g[((size_t)c * t.K + k) * t.n + j];
+                        const uint32_t off = (uint32_t)(plane * SM_PLANE + (e & 0x7fff)) * 16u;
+                        ((e & 0x8000) ? minus : plus).push_back(off);
+                    }
+                    if ((int)plus.size() != nw || (int)minus.size() != nw) { tab_err = "internal: unbalanced gather signs"; return 0; }
+                    for (int j = 0; j < nw; ++j) {
+                        const size_t o = ((((size_t)k * rows + r) * G + g) * nw + j) * 2;
+                        w[o] = plus[j]; w[o + 1] = minus[j];
+                    }
                 }
-        auto it = dedupe2.find(w);
-        if (it != dedupe2.end()) return it->second;
-        uint32_t off = (uint32_t)plan.tab2.size();
-        plan.tab2.insert(plan.tab2.end(), w.begin(), w.end());
-        while (plan.tab2.size() % 4) plan.tab2.push_back(0); // 16-byte aligned tables
-        dedupe2[w] = off;
+        w.push_back((uint32_t)layout); // same content in another layout is another table
+        auto it = dedupe3.find(w);
+        if (it != dedupe3.end()) return it->second;
+        w.pop_back();
+        const uint32_t off = (uint32_t)plan.tab3.size();
+        for (size_t i = 0; i < w.size(); i += 2) plan.tab3.push_back(uint2x{w[i], w[i + 1]});
+        while (plan.tab3.size() % 2) plan.tab3.push_back(uint2x{0, 0}); // 16-byte aligned tables
+        w.push_back((uint32_t)layout);
+        dedupe3[w] = off;
         return off;
     };
     const int UNIT_SPLIT_STEPS = unit_split_steps, UNIT_COST_MAX = unit_cost_max; // cost: 2 per 16x16 step, 3 per 64x4 step
     for (size_t ip = 0; ip < pair_list.size(); ++ip) {
         const std::vector<Key>& order = pair_elem_order[ip];
-        // at most 15 distinct elementary source operators pairs share the flavour content of one sink pair
+        // at most 15 distinct elementary source operator pairs share the flavour content of one sink pair
         if (order.size() > (size_t)MAX_PAIR_ELEMS) return "internal: more than 16 elementary correlators for one sink pair";
-        {
-            const size_t e0 = 0, e1 = order.size();
-            Pair2Rec pr;
-            pr.slot1 = slot_of[pair_list[ip].first];
-            pr.slot2 = slot_of[pair_list[ip].second];
-            pr.unit_begin = (int)plan.units2.size();
-            pr.nelem = (int)(e1 - e0);
-            for (size_t e = e0; e < e1; ++e) {
-                pr.elem_unit_begin[e - e0] = (int)plan.units2.size() - pr.unit_begin;
-                for (int cls = 0; cls < 4; ++cls) {
-                    Unit2Rec u;
-                    u.cls = cls; u.cost = 0; u.diag_begin = (int)plan.diags2.size();
-                    auto flush = [&] {
-                        u.diag_end = (int)plan.diags2.size();
-                        if (u.diag_end > u.diag_begin) plan.units2.push_back(u);
-                        u.diag_begin = u.diag_end; u.cost = 0;
-                    };
-                    for (auto& d : pair_elems[ip][order[e]]) {
-                        SideTable s1 = make_side(d.P, d.sign, true); // sigma_P folded into side 1
-                        SideTable s2 = make_side(d.P + 3, +1, true);
-                        int c;
-                        if (s1.C == 4 && s2.C == 4) c = (s1.carries == 1) ? 0 : 1;
-                        else if (s1.C == 16 && s2.C == 1) c = 2;
-                        else if (s1.C == 1 && s2.C == 16) c = 3;
-                        else return "internal: unexpected carry split";
-                        if (c != cls) continue;
-                        if ((s1.n & 1) || (s2.n & 1)) return "internal: odd gather length";
-                        Diag2Rec r;
-                        const SideTable &A = (c == 3) ? s2 : s1, &B = (c == 3) ? s1 : s2;
-                        r.offA = intern2(A); r.offB = intern2(B);
-                        r.K = (uint16_t)s1.K;
-                        r.nA = (uint8_t)A.n; r.nB = (uint8_t)B.n;
-                        // split long diagrams into k-ranges so that a sink pair with few diagrams
-                        // still spreads over all warps of the CTA
-                        const int steps = (s1.K + 3) / 4;
-                        const int nchunk = (steps + UNIT_SPLIT_STEPS - 1) / UNIT_SPLIT_STEPS;
-                        for (int ic = 0; ic < nchunk; ++ic) {
-                            const int sb = steps * ic / nchunk, se = steps * (ic + 1) / nchunk;
-                            r.kbeg = (uint16_t)(4 * sb); r.kend = (uint16_t)(4 * se);
-                            const int cost = (se - sb) * (c >= 2 ? 3 : 2) + 2;
-                            if (u.cost > 0 && u.cost + cost > UNIT_COST_MAX) flush();
-                            plan.diags2.push_back(r);
-                            u.cost += cost;
-                            plan.sumKp_exec += 4 * (se - sb);
-                        }
+        Pair3Rec pr;
+        pr.slot1 = slot_of[pair_list[ip].first];
+        pr.slot2 = slot_of[pair_list[ip].second];
+        pr.unit_begin = (int)plan.units3.size();
+        pr.nelem = (int)order.size();
+        std::vector<Unit3Rec> units;
+        std::vector<int> cost_of;
+        for (size_t e = 0; e < order.size(); ++e) {
+            pr.elem_unit_begin[e] = (int)units.size();
+            for (int cls = 0; cls < 4; ++cls) {
+                Unit3Rec u;
+                int ucost = 0;
+                u.cls = cls; u.diag_begin = (int)plan.diags3.size();
+                auto flush = [&] {
+                    u.diag_end = (int)plan.diags3.size();
+                    if (u.diag_end > u.diag_begin) { u.slot = (int)units.size(); units.push_back(u); cost_of.push_back(ucost); }
+                    u.diag_begin = u.diag_end; ucost = 0;
+                };
+                for (auto& d : pair_elems[ip][order[e]]) {
+                    SideTable s1 = make_side(d.P, d.sign, true); // sigma_P folded into side 1
+                    SideTable s2 = make_side(d.P + 3, +1, true);
+                    int c;
+                    if (s1.C == 4 && s2.C == 4) c = (s1.carries == 1) ? 0 : 1;
+                    else if (s1.C == 16 && s2.C == 1) c = 2;
+                    else if (s1.C == 1 && s2.C == 16) c = 3;
+                    else return "internal: unexpected carry split";
+                    if (c != cls) continue;
+                    if ((s1.n & 1) || (s2.n & 1)) return "internal: odd gather length";
+                    const SideTable &A = (c == 3) ? s2 : s1, &B = (c == 3) ? s1 : s2;
+                    if (c < 2 ? !(A.n == B.n && (A.n == 2 || A.n == 8 || A.n == 24)) : !(A.n == 2 && B.n == 8))
+                        return "internal: unexpected gather lengths";
+                    Diag3Rec r;
+                    r.offA = intern3(A, c < 2 ? 0 : 1); r.offB = intern3(B, c < 2 ? 0 : 2);
+                    if (!tab_err.empty()) return tab_err;
+                    r.K = (uint16_t)s1.K;
+                    r.nwA = (uint8_t)(A.n / 2); r.nwB = (uint8_t)(B.n / 2);
+                    // split long diagrams into k-ranges so that a sink pair with few diagrams
+                    // still spreads over all warps of the CTA
+                    const int steps = (s1.K + 3) / 4;
+                    const int nchunk = (steps + UNIT_SPLIT_STEPS - 1) / UNIT_SPLIT_STEPS;
+                    for (int ic = 0; ic < nchunk; ++ic) {
+                        const int sb = steps * ic / nchunk, se = steps * (ic + 1) / nchunk;
+                        r.sbeg = (uint16_t)sb; r.send = (uint16_t)se;
+                        const int cost = (se - sb) * (c >= 2 ? 3 : 2) * (c < 2 ? (int)r.nwA : 1) + 2;
+                        if (ucost > 0 && ucost + cost > UNIT_COST_MAX) flush();
+                        plan.diags3.push_back(r);
+                        ucost += cost;
+                        plan.sumKp_exec += 4 * (se - sb);
                     }
-                    flush();
                 }
+                flush();
             }
-            pr.nunits = (int)plan.units2.size() - pr.unit_begin;
-            for (int e = pr.nelem; e <= MAX_PAIR_ELEMS; ++e) pr.elem_unit_begin[e] = pr.nunits;
-            plan.max_pair_units = std::max(plan.max_pair_units, pr.nunits);
-            // schedule: local unit indices by decreasing cost (warps take them in this order)
-            pr.sched_begin = (int)plan.sched.size();
-            std::vector<int> idx(pr.nunits);
-            for (int i = 0; i < pr.nunits; ++i) idx[i] = i;
-            std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
-                return plan.units2[pr.unit_begin + a].cost > plan.units2[pr.unit_begin + b].cost;
-            });
-            plan.sched.insert(plan.sched.end(), idx.begin(), idx.end());
-            // channels of this pair as dense coefficient rows over its elementary correlators
-            pr.chan_begin = (int)plan.pair_chans.size();
-            for (size_t ic = 0; ic < channels.size(); ++ic) {
-                if (plan.chan_pair[ic] != (int)ip) continue;
-                PairChanRec pc;
-                pc.ch = (int)ic; pc.pad = 0;
-                bool any = false;
-                for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = 0.0;
-                for (auto& ct : chan_ct[ic])
-                    for (size_t e = e0; e < e1; ++e)
-                        if (order[e] == ct.key) { pc.coef[e - e0] += ct.coef; any = true; }
-                if (any) plan.pair_chans.push_back(pc);
+        }
+        pr.nunits = (int)units.size();
+        if (pr.nunits > MAX_PAIR_UNITS) return "internal: too many units for one sink pair";
+        for (int e = pr.nelem; e <= MAX_PAIR_ELEMS; ++e) pr.elem_unit_begin[e] = pr.nunits;
+        plan.max_pair_units = std::max(plan.max_pair_units, pr.nunits);
+        // schedule: units by decreasing cost (warps take them in this order)
+        std::vector<int> idx(pr.nunits);
+        for (int i = 0; i < pr.nunits; ++i) idx[i] = i;
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return cost_of[a] > cost_of[b]; });
+        for (int i : idx) plan.units3.push_back(units[i]);
+        // channels of this pair as dense coefficient rows over its elementary correlators
+        pr.chan_begin = (int)plan.pair_chans.size();
+        for (size_t ic = 0; ic < channels.size(); ++ic) {
+            if (plan.chan_pair[ic] != (int)ip) continue;
+            PairChanRec pc;
+            pc.ch = (int)ic; pc.pad = 0;
+            bool any = false;
+            for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = 0.0;
+            for (auto& ct : chan_ct[ic])
+                for (size_t e = 0; e < order.size(); ++e)
+                    if (order[e] == ct.key) { pc.coef[e] += ct.coef; any = true; }
+            if (any) plan.pair_chans.push_back(pc);
+        }
+        pr.nchan = (int)plan.pair_chans.size() - pr.chan_begin;
+        plan.pairs3.push_back(pr);
+    }
+    plan.tab3.insert(plan.tab3.end(), 1024, uint2x{0, 0}); // the kernel prefetches a few k-steps past a table's end
+
+    // ---- chain: order of the sink pairs inside one momentum task that reloads the fewest blocks
+    {
+        const int n = (int)plan.pairs3.size();
+        auto tcost = [&](int a, int b) {
+            return (plan.pairs3[a].slot1 != plan.pairs3[b].slot1) + (plan.pairs3[a].slot2 != plan.pairs3[b].slot2);
+        };
+        std::vector<int> best;
+        if (n <= 16) { // exact: shortest Hamiltonian path by subset DP
+            const int N = 1 << n, INF = 1 << 28;
+            std::vector<int> dp((size_t)N * n, INF), from((size_t)N * n, -1);
+            for (int i = 0; i < n; ++i) dp[((size_t)1 << i) * n + i] = 2;
+            for (int m = 1; m < N; ++m)
+                for (int i = 0; i < n; ++i) {
+                    const int cur = dp[(size_t)m * n + i];
+                    if (cur >= INF || !((m >> i) & 1)) continue;
+                    for (int j = 0; j < n; ++j) {
+                        if ((m >> j) & 1) continue;
+                        const int m2 = m | (1 << j), c = cur + tcost(i, j);
+                        if (c < dp[(size_t)m2 * n + j]) { dp[(size_t)m2 * n + j] = c; from[(size_t)m2 * n + j] = i; }
+                    }
+                }
+            int bi = 0;
+            for (int i = 1; i < n; ++i)
+                if (dp[(size_t)(N - 1) * n + i] < dp[(size_t)(N - 1) * n + bi]) bi = i;
+            int m = N - 1, i = bi;
+            while (i >= 0) { best.push_back(i); const int pi = from[(size_t)m * n + i]; m &= ~(1 << i); i = pi; }
+            std::reverse(best.begin(), best.end());
+        } else { // greedy nearest neighbour
+            std::vector<char> used(n, 0);
+            int cur = 0;
+            used[0] = 1; best.push_back(0);
+            for (int s = 1; s < n; ++s) {
+                int bj = -1;
+                for (int j = 0; j < n; ++j)
+                    if (!used[j] && (bj < 0 || tcost(cur, j) < tcost(cur, bj))) bj = j;
+                used[bj] = 1; best.push_back(bj); cur = bj;
             }
-            pr.nchan = (int)plan.pair_chans.size() - pr.chan_begin;
-            plan.pairs2.push_back(pr);
+        }
+        for (int s = 0; s < n; ++s) {
+            ChainRec cr;
+            cr.pair = best[s];
+            cr.load1 = (s == 0) || plan.pairs3[best[s]].slot1 != plan.pairs3[best[s - 1]].slot1;
+            cr.load2 = (s == 0) || plan.pairs3[best[s]].slot2 != plan.pairs3[best[s - 1]].slot2;
+            plan.chain.push_back(cr);
         }
     }
-    plan.tab2.insert(plan.tab2.end(), 256, 0u); // the kernel prefetches one k-step past a table's end
     return "";
 }
 

@@ -67,37 +67,53 @@ struct ChanTermRec {
     double coef;
 };
 
-// ---- v2 product kernel (DMMA) records ------------------------------------------------------
-// A "unit" is the work of one warp: a few diagrams of ONE elementary correlator that share one
-// accumulator layout (class).  Classes (which effective block carries a3 / a4):
+// ---- product kernel (DMMA) records ----------------------------------------------------------
+// A "unit" is the work of one warp: a few diagrams (or k-ranges of one diagram) of ONE elementary
+// correlator that share one accumulator layout (class).  Classes (which effective
+// block carries a3 / a4):
 //   0: 16x16, B~1 carries a3, B~2 carries a4      1: 16x16, B~1 carries a4, B~2 carries a3
 //   2: 64x4,  B~1 carries a3 and a4               3: 4x64,  B~2 carries a3 and a4
-// Gather tables are u32 words holding two u16 entries (bit 15: minus sign, bits 0-10: sm_index of the
-// source triple), laid out [k][c][term/2] with k padded to a multiple of 4 (Kp).
+//
+// Gather tables: one uint2 {off_plus, off_minus} per PAIR of gather terms of an effective-block
+// entry (eq. 4.2): entry = sum_j ( blk[off_plus_j] - blk[off_minus_j] ).  Every entry has as many
+// +1 as -1 terms (the eps (C g5) weights are balanced, and sigma_P only swaps the two halves), so no
+// sign bits are needed; a padded k (k >= K) has off_plus == off_minus and contributes exactly 0.
+// Offsets are BYTE offsets into the staged block of that side, with the sink-spin plane of the
+// reading lane folded in (the kernel adds compile-time plane offsets only):
+//   16x16 sides    [k][row r = 2*c + (a & 1)][nw]          planes a = (r & 1) + {0, 2}
+//   64x4  A side   [k][row r = 2*(cX & 3) + (a & 1)][g = cX >> 2][1]   planes a = (r & 1) + {0, 2}
+//   64x4  B side   [k][a][nw]                               plane a
+// k is padded to a multiple of 4 (one DMMA k-step).
 constexpr int MAX_PAIR_ELEMS = 16;
-struct Diag2Rec {
-    uint32_t offA, offB; // word offsets: operand A (the M side) and operand B (the N side)
+constexpr int MAX_PAIR_UNITS = 512; // unit records of one sink pair are staged in shared memory
+struct Diag3Rec {
+    uint32_t offA, offB; // uint2 offsets into Plan::tab3: operand A (the M side) and operand B (the N side)
+    uint16_t sbeg, send; // k-steps [sbeg, send) of this diagram covered by this record
+    uint8_t nwA, nwB;    // uint2 words (term pairs) per entry
     uint16_t K;          // size of the shared index (1, 9, 36, 144)
-    uint16_t kbeg, kend; // this record covers k in [kbeg, kend), both multiples of 4 (kend may pass K: padding)
-    uint8_t nA, nB;      // gather terms per entry
 };
-struct Unit2Rec {
-    int diag_begin, diag_end; // range in Plan::diags2
+struct Unit3Rec {        // in schedule order (cost descending) per sink pair
+    int diag_begin, diag_end; // range in Plan::diags3
     int cls;
-    int cost;
+    int slot;                 // row of the per-item unit scratch (units grouped by elementary correlator)
 };
-struct Pair2Rec {
+struct Pair3Rec {
     int slot1, slot2;
-    int unit_begin, nunits;  // units grouped by elementary correlator (elem_unit_begin)
-    int sched_begin;         // Plan::sched[sched_begin + i]: local unit index, cost descending
+    int unit_begin, nunits;  // Plan::units3 range (schedule order)
     int nelem;
-    int elem_unit_begin[MAX_PAIR_ELEMS + 1]; // local unit ranges per elementary correlator
+    int elem_unit_begin[MAX_PAIR_ELEMS + 1]; // scratch-row ranges per elementary correlator
     int chan_begin, nchan;   // range in Plan::pair_chans
 };
 struct PairChanRec {
     int ch, pad;
     double coef[MAX_PAIR_ELEMS]; // channel = sum_e coef[e] * elementary correlator e (eqs. 2.2-2.3)
 };
+struct ChainRec { // order in which one CTA walks the sink pairs of one momentum q
+    int pair;
+    int load1, load2; // 1: this item must (re)load B~1(q) / B~2(-q); 0: the staged block is reused
+};
+
+struct uint2x { uint32_t x, y; }; // host mirror of CUDA uint2
 
 struct DiagramInfo { // host-side description (tests, statistics)
     int P[6];
@@ -117,13 +133,13 @@ struct Plan {
     std::vector<int> chan_pair; // pair index of each channel
     double sumK_std = 0;        // sum over channels of sum_d K_d (the paper's count)
     double sumK_exec = 0;       // sum over distinct elementary correlators
-    // v2 (DMMA) product kernel tables
-    std::vector<Pair2Rec> pairs2;
-    std::vector<Unit2Rec> units2;
-    std::vector<Diag2Rec> diags2;
-    std::vector<uint32_t> tab2;
-    std::vector<int> sched;
+    // product kernel tables
+    std::vector<Pair3Rec> pairs3;
+    std::vector<Unit3Rec> units3;
+    std::vector<Diag3Rec> diags3;
+    std::vector<uint2x> tab3;
     std::vector<PairChanRec> pair_chans;
+    std::vector<ChainRec> chain;
     int max_pair_units = 0;
     double sumKp_exec = 0; // executed k-steps x 4 (padding included)
 };
