@@ -25,7 +25,7 @@ struct Slice {
     double2* own[3] = {nullptr, nullptr, nullptr};     // library-owned copies for host input
     double2* B = nullptr;  // [V][R] normal blocks, x-space then momentum space (in place)
     double2* Ft = nullptr; // [V][nch][256]
-    double2* scratch = nullptr;            // [grid][2][max_pair_units][256] unit results
+    double2* scratch = nullptr;            // [grid][PROD_NBUF][max_pair_units][256] unit results
     unsigned long long* counter = nullptr; // work-item counter of the persistent product kernel
 };
 
@@ -283,7 +283,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
 
     // workspace: per slice in flight, blocks + elementary correlators + channel correlators
     size_t nchan = c->plan.channels.size();
-    size_t scratch_elems = (size_t)c->prod_grid * 2 * c->plan.max_pair_units * 256;
+    size_t scratch_elems = (size_t)c->prod_grid * PROD_NBUF * c->plan.max_pair_units * 256;
     size_t per_slice = (c->V * (c->R + nchan * 256) + scratch_elems) * sizeof(double2);
     size_t free_b = 0, total_b = 0;
     CUX(cudaMemGetInfo(&free_b, &total_b));

@@ -37,7 +37,9 @@ constexpr uint32_t PLANE_BYTES = SM_PLANE * 16u;  // 27 840
 constexpr uint32_t BLOCK_BYTES = SM_BLOCK * 16u;  // 111 360
 // shared-memory map (bytes)
 constexpr uint32_t SMO_S1 = 0, SMO_S2 = BLOCK_BYTES, SMO_UNITS = 2 * BLOCK_BYTES;
-constexpr uint32_t SMO_CTRL = SMO_UNITS + MAX_PAIR_UNITS * 16u;
+constexpr uint32_t SMO_DIAGS = SMO_UNITS + MAX_PAIR_UNITS * 16u;
+constexpr uint32_t SMO_CTRL = SMO_DIAGS + MAX_PAIR_DIAGS * 16u;
+constexpr int PROD_NBUF = 4; // depth of the unit-result ring between compute and epilogue warps
 constexpr size_t PROD_SMEM = SMO_CTRL + 128;
 static_assert(sizeof(Unit3Rec) == 16 && sizeof(Diag3Rec) == 16, "record sizes");
 static_assert(PROD_SMEM <= 232448, "shared memory budget of one SM");
@@ -47,7 +49,7 @@ struct ProdCtrl { // at SMO_CTRL
     int next_unit;                   // work counter of the current item
     int pad;
     long long qtask[2];              // prefetched momentum-task indices (alternating slots)
-    int meta_q[2], meta_pair[2];     // item descriptors handed to the epilogue warps
+    int meta_q[PROD_NBUF], meta_pair[PROD_NBUF]; // item descriptors handed to the epilogue warps
 };
 
 // ---- PTX helpers ----------------------------------------------------------------------------
@@ -79,7 +81,8 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 __device__ __forceinline__ void named_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void named_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-enum { BAR_COMPUTE = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4 };
+enum { BAR_COMPUTE = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 2 + PROD_NBUF };
+static_assert(2 + 2 * PROD_NBUF <= 16, "named barriers");
 
 // ---- gathers (eq. 4.2) ----------------------------------------------------------------------
 // One table word = one (+, -) pair of byte offsets into a staged block.  ld_pair issues the
@@ -125,8 +128,8 @@ __device__ __forceinline__ void mma_square(AccSquare& c, const double2 (&A)[2], 
         }
 }
 
-__device__ __forceinline__ Diag3Rec load_diag(const Diag3Rec* __restrict__ p) {
-    const int4 v = __ldg(reinterpret_cast<const int4*>(p));
+__device__ __forceinline__ Diag3Rec load_diag(const Diag3Rec* p) { // p: shared memory
+    const int4 v = *reinterpret_cast<const int4*>(p);
     Diag3Rec d;
     d.offA = (uint32_t)v.x; d.offB = (uint32_t)v.y;
     d.sbeg = (uint16_t)((uint32_t)v.z & 0xffffu); d.send = (uint16_t)((uint32_t)v.z >> 16);
@@ -135,7 +138,7 @@ __device__ __forceinline__ Diag3Rec load_diag(const Diag3Rec* __restrict__ p) {
     return d;
 }
 
-__device__ __forceinline__ void run_unit_square(const Unit3Rec u, const Diag3Rec* __restrict__ diags,
+__device__ __forceinline__ void run_unit_square(const Unit3Rec u, const Diag3Rec* diags,
                                                 const uint2* __restrict__ tab, const char* s1, const char* s2,
                                                 double2* __restrict__ out, int lane) {
     const int r = lane >> 2, kk = lane & 3;
@@ -237,7 +240,7 @@ __device__ __forceinline__ void wide_fold_B(const double2 (&ub)[4][1], const dou
     sub_pair<1, false>(ub[3], vb[3], Bv);
 }
 
-__device__ __forceinline__ void run_unit_wide(const Unit3Rec u, const Diag3Rec* __restrict__ diags,
+__device__ __forceinline__ void run_unit_wide(const Unit3Rec u, const Diag3Rec* diags,
                                               const uint2* __restrict__ tab, const char* s1, const char* s2,
                                               double2* __restrict__ out, int lane) {
     const int r = lane >> 2, kk = lane & 3, aY = r & 3, hi = r >> 2;
@@ -298,7 +301,7 @@ struct ProdArgs {
     const uint2* tab;
     const PairChanRec* pair_chans;
     const ChainRec* chain; // [npairs]
-    double2* scratch;    // [gridDim.x][2][max_pair_units][256]
+    double2* scratch;    // [gridDim.x][PROD_NBUF][max_pair_units][256]
     int max_pair_units;
     double2* Ft;         // [V][nch_out][256]
     int ch_begin, nch_out;
@@ -328,7 +331,7 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* 
 #pragma unroll
             for (int m = 0; m < 4; ++m) s[m] = make_double2(0.0, 0.0);
             const int ub = pr->elem_unit_begin[e], ue = pr->elem_unit_begin[e + 1];
-#pragma unroll 4
+#pragma unroll 8
             for (int ul = ub; ul < ue; ++ul) {
 #pragma unroll
                 for (int m = 0; m < 4; ++m) {
@@ -368,13 +371,14 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
     char* s1 = smem + SMO_S1;
     char* s2 = smem + SMO_S2;
     Unit3Rec* s_units = reinterpret_cast<Unit3Rec*>(smem + SMO_UNITS);
+    Diag3Rec* s_diags = reinterpret_cast<Diag3Rec*>(smem + SMO_DIAGS);
     volatile ProdCtrl* ctl = reinterpret_cast<volatile ProdCtrl*>(smem + SMO_CTRL);
     void* mbar1 = smem + SMO_CTRL + offsetof(ProdCtrl, mbar1);
     void* mbar2 = smem + SMO_CTRL + offsetof(ProdCtrl, mbar2);
     int* next_unit = reinterpret_cast<int*>(smem + SMO_CTRL + offsetof(ProdCtrl, next_unit));
     const int tid = threadIdx.x;
     const size_t scr_stride = (size_t)a.max_pair_units * 256;
-    double2* scr0 = a.scratch + (size_t)blockIdx.x * 2 * scr_stride;
+    double2* scr0 = a.scratch + (size_t)blockIdx.x * PROD_NBUF * scr_stride;
 
     if (tid == 0) {
         mbar_init(mbar1, 1);
@@ -388,7 +392,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         // ---------------- epilogue warps: combine item i while the compute warps run item i+1
         const int et = tid - PROD_CTHREADS;
         for (unsigned it = 0;; ++it) {
-            const int b = it & 1;
+            const int b = it % PROD_NBUF;
             named_sync(BAR_FULL0 + b, PROD_THREADS);
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
@@ -407,7 +411,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
     long long qt = 0;
     size_t q = 0, mq = 0;
     for (unsigned it = 0;; ++it) {
-        const int b = it & 1;
+        const int b = it % PROD_NBUF;
         named_sync(BAR_COMPUTE, PROD_CTHREADS); // the staged blocks and unit records of the previous item are consumed
         if (pos == 0) {
             qt = ctl->qtask[ntask & 1];
@@ -416,7 +420,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
                 mq = minus_q(a.L, q);
             }
         }
-        if (it >= 2) named_sync(BAR_EMPTY0 + b, PROD_THREADS); // scratch buffer b and its descriptor are free again
+        if (it >= PROD_NBUF) named_sync(BAR_EMPTY0 + b, PROD_THREADS); // scratch buffer b and its descriptor are free again
         if (qt >= a.ntasks) { // no work left: tell the epilogue warps and leave
             if (tid == 0) ctl->meta_pair[b] = -1;
             __threadfence_block();
@@ -432,19 +436,23 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             *next_unit = 0;
             ctl->meta_q[b] = (int)q;
             ctl->meta_pair[b] = ip;
+            // unit and diagram records of the pair ride on the first staging barrier of the item
             const uint32_t ubytes = (uint32_t)nunits * (uint32_t)sizeof(Unit3Rec);
+            const uint32_t dbytes = (uint32_t)__ldg(&pr->ndiags) * (uint32_t)sizeof(Diag3Rec);
             const Unit3Rec* usrc = a.units + __ldg(&pr->unit_begin);
+            const Diag3Rec* dsrc = a.diags + __ldg(&pr->diag_begin);
+            void* rbar = load1 ? mbar1 : mbar2;
+            if (load1) mbar_expect_tx(mbar1, BLOCK_BYTES + ubytes + dbytes);
+            if (load2) mbar_expect_tx(mbar2, BLOCK_BYTES + (load1 ? 0u : ubytes + dbytes));
+            bulk_g2s(s_units, usrc, ubytes, rbar);
+            bulk_g2s(s_diags, dsrc, dbytes, rbar);
             if (load1) {
                 const char* g1 = reinterpret_cast<const char*>(a.Bq + q * a.R + (size_t)__ldg(&pr->slot1) * SM_BLOCK);
-                mbar_expect_tx(mbar1, BLOCK_BYTES + ubytes);
-                bulk_g2s(s_units, usrc, ubytes, mbar1);
 #pragma unroll
                 for (int p = 0; p < 4; ++p) bulk_g2s(s1 + p * PLANE_BYTES, g1 + p * PLANE_BYTES, PLANE_BYTES, mbar1);
             }
             if (load2) {
                 const char* g2 = reinterpret_cast<const char*>(a.Bq + mq * a.R + (size_t)__ldg(&pr->slot2) * SM_BLOCK);
-                mbar_expect_tx(mbar2, BLOCK_BYTES + (load1 ? 0u : ubytes));
-                if (!load1) bulk_g2s(s_units, usrc, ubytes, mbar2);
 #pragma unroll
                 for (int p = 0; p < 4; ++p) bulk_g2s(s2 + p * PLANE_BYTES, g2 + p * PLANE_BYTES, PLANE_BYTES, mbar2);
             }
@@ -452,17 +460,31 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         if (load1) { mbar_wait(mbar1, ph1); ph1 ^= 1u; }
         if (load2) { mbar_wait(mbar2, ph2); ph2 ^= 1u; }
         double2* scr = scr0 + b * scr_stride;
-        for (;;) {
+        // Units are taken one ahead: while unit i runs, the head of the gather tables of the warp's
+        // next unit is pulled into L1 (table words are the first link of every gather chain).
+        auto grab = [&]() {
             int i = 0;
             if (lane == 0) i = atomicAdd(next_unit, 1);
-            i = __shfl_sync(0xffffffffu, i, 0);
-            if (i >= nunits) break;
+            return __shfl_sync(0xffffffffu, i, 0);
+        };
+        int i = grab();
+        while (i < nunits) {
             const int4 uv = *reinterpret_cast<const int4*>(s_units + i);
             Unit3Rec u;
             u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
+            const int inext = grab();
+            if (inext < nunits && lane < 16) {
+                const Diag3Rec nd = load_diag(s_diags + s_units[inext].diag_begin);
+                const int wide = s_units[inext].cls >= 2;
+                const uint32_t off = (lane < 8) ? nd.offA + (uint32_t)nd.sbeg * (wide ? 128u : 32u * nd.nwA)
+                                                : nd.offB + (uint32_t)nd.sbeg * (wide ? 64u : 32u * nd.nwB);
+                const char* ptr = reinterpret_cast<const char*>(a.tab + off) + (lane & 7) * 128;
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr));
+            }
             double2* out = scr + (size_t)u.slot * 256;
-            if (u.cls < 2) run_unit_square(u, a.diags, a.tab, s1, s2, out, lane);
-            else run_unit_wide(u, a.diags, a.tab, s1, s2, out, lane);
+            if (u.cls < 2) run_unit_square(u, s_diags, a.tab, s1, s2, out, lane);
+            else run_unit_wide(u, s_diags, a.tab, s1, s2, out, lane);
+            i = inext;
         }
         __threadfence_block();
         named_arrive(BAR_FULL0 + b, PROD_THREADS); // unit results of this item are in scratch buffer b

@@ -454,6 +454,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         pr.slot1 = slot_of[pair_list[ip].first];
         pr.slot2 = slot_of[pair_list[ip].second];
         pr.unit_begin = (int)plan.units3.size();
+        pr.diag_begin = (int)plan.diags3.size();
         pr.nelem = (int)order.size();
         std::vector<Unit3Rec> units;
         std::vector<int> cost_of;
@@ -462,9 +463,9 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             for (int cls = 0; cls < 4; ++cls) {
                 Unit3Rec u;
                 int ucost = 0;
-                u.cls = cls; u.diag_begin = (int)plan.diags3.size();
+                u.cls = cls; u.diag_begin = (int)plan.diags3.size() - pr.diag_begin;
                 auto flush = [&] {
-                    u.diag_end = (int)plan.diags3.size();
+                    u.diag_end = (int)plan.diags3.size() - pr.diag_begin;
                     if (u.diag_end > u.diag_begin) { u.slot = (int)units.size(); units.push_back(u); cost_of.push_back(ucost); }
                     u.diag_begin = u.diag_end; ucost = 0;
                 };
@@ -504,7 +505,8 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             }
         }
         pr.nunits = (int)units.size();
-        if (pr.nunits > MAX_PAIR_UNITS) return "internal: too many units for one sink pair";
+        pr.ndiags = (int)plan.diags3.size() - pr.diag_begin;
+        if (pr.nunits > MAX_PAIR_UNITS || pr.ndiags > MAX_PAIR_DIAGS) return "internal: too many units for one sink pair";
         for (int e = pr.nelem; e <= MAX_PAIR_ELEMS; ++e) pr.elem_unit_begin[e] = pr.nunits;
         plan.max_pair_units = std::max(plan.max_pair_units, pr.nunits);
         // schedule: units by decreasing cost (warps take them in this order)

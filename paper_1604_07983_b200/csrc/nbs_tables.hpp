@@ -85,7 +85,8 @@ struct ChanTermRec {
 //   64x4  B side   [k][a][nw]                               plane a
 // k is padded to a multiple of 4 (one DMMA k-step).
 constexpr int MAX_PAIR_ELEMS = 16;
-constexpr int MAX_PAIR_UNITS = 512; // unit records of one sink pair are staged in shared memory
+constexpr int MAX_PAIR_UNITS = 256; // unit and diagram records of one sink pair are staged in shared memory
+constexpr int MAX_PAIR_DIAGS = 256;
 struct Diag3Rec {
     uint32_t offA, offB; // uint2 offsets into Plan::tab3: operand A (the M side) and operand B (the N side)
     uint16_t sbeg, send; // k-steps [sbeg, send) of this diagram covered by this record
@@ -93,13 +94,14 @@ struct Diag3Rec {
     uint16_t K;          // size of the shared index (1, 9, 36, 144)
 };
 struct Unit3Rec {        // in schedule order (cost descending) per sink pair
-    int diag_begin, diag_end; // range in Plan::diags3
+    int diag_begin, diag_end; // range in the sink pair's diagram records (relative to Pair3Rec::diag_begin)
     int cls;
     int slot;                 // row of the per-item unit scratch (units grouped by elementary correlator)
 };
 struct Pair3Rec {
     int slot1, slot2;
     int unit_begin, nunits;  // Plan::units3 range (schedule order)
+    int diag_begin, ndiags;  // Plan::diags3 range
     int nelem;
     int elem_unit_begin[MAX_PAIR_ELEMS + 1]; // scratch-row ranges per elementary correlator
     int chan_begin, nchan;   // range in Plan::pair_chans
@@ -146,7 +148,7 @@ struct Plan {
 
 // Returns "" on success, else an error message (invalid id, flavour violation).
 std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps = 18,
-                       int unit_cost_max = 40);
+                       int unit_cost_max = 64);
 
 // Diagrams of one channel in enumeration order (source terms major, permutations lexicographic).
 std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& out);
