@@ -151,10 +151,11 @@ int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st) {
 }
 
 int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, int nslots, unsigned dq_mask, double2* out,
-                  size_t row_stride, int staged, cudaStream_t st) {
-    size_t smem = (3 * 144 + 9 * 432) * sizeof(double2);
-    k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, smem, st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask, c->d_brec,
-                                                           c->d_bterm, out, row_stride, staged);
+                  size_t row_stride, cudaStream_t st) {
+    int ndq = 0;
+    for (int b = 0; b < 9; ++b) ndq += (dq_mask >> b) & 1u;
+    k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, blocks_smem_bytes(ndq), st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask,
+                                                                          c->d_brec, c->d_bterm, out, row_stride);
     CU(c, cudaGetLastError());
     ++c->launches;
     return NBS_OK;
@@ -305,8 +306,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         c->slice[i].counter = (unsigned long long*)cnt;
     }
     CUX(cudaFuncSetAttribute(k_product, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
-    CUX(cudaFuncSetAttribute(k_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)((3 * 144 + 9 * 432) * sizeof(double2))));
+    CUX(cudaFuncSetAttribute(k_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)blocks_smem_bytes(9)));
     *out = c;
     return NBS_OK;
 #undef CUC
@@ -352,8 +352,20 @@ int nbs_blocks_x(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes,
     if (sl.t != t) return fail(c, NBS_ESTATE, "time slice not loaded");
     if (out_bytes < c->V * BLOCK_ELEMS * sizeof(double2)) return fail(c, NBS_EINVAL, "output buffer too small");
     CU(c, cudaSetDevice(c->device));
-    return launch_blocks(c, sl, c->d_one_baryon + baryon, 1, c->dq_mask_of[baryon], (double2*)out_dev, BLOCK_ELEMS, 0,
-                         (cudaStream_t)stream);
+    // the kernel writes the staged layout; convert to [site][alpha][xi1][xi2][xi3] for the caller
+    cudaStream_t st = (cudaStream_t)stream;
+    double2* tmp = nullptr;
+    CU(c, cudaMalloc((void**)&tmp, c->V * (size_t)SM_BLOCK * sizeof(double2)));
+    int rc = launch_blocks(c, sl, c->d_one_baryon + baryon, 1, c->dq_mask_of[baryon], tmp, SM_BLOCK, st);
+    if (rc == NBS_OK) {
+        const size_t n = c->V * (size_t)BLOCK_ELEMS;
+        k_unstage<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(tmp, c->V, (double2*)out_dev);
+        ++c->launches;
+        cudaError_t e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(c, e, "nbs_blocks_x"); }
+    }
+    cudaFree(tmp);
+    return rc;
 }
 
 int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_t out_bytes, int memloc, void* stream) {
@@ -375,7 +387,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     int rc;
     {
         StageTimer tm(c, NBS_STAGE_BLOCKS, st);
-        rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, 1, st);
+        rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
         if (rc) return rc;
     }
     {

@@ -35,9 +35,13 @@ __device__ __forceinline__ void cfma(double2& acc, double2 a, double2 b) {
 // ---------------------------------------------------------------------------------------------
 // (i) NormalBaryonBlocks, eq. 4.1.  One CTA per lattice site.
 //   phase 1: diquarks D^{f0f1}_c(i,j) = sum_{ab, beta gamma} eps_abc (C g5)_{beta gamma}
-//            S_f0[(a,beta), i] S_f1[(b,gamma), j]                       -> shared memory
-//   phase 2: block[a][xi0 xi1 xi2] = sum_terms coef sum_c D_c(xi_p0, xi_p1) S_f2[(c,a), xi_p2]
-//            written straight to HBM, consecutive threads -> consecutive components.
+//            S_f0[(a,beta), i] S_f1[(b,gamma), j]            -> shared memory (needed types only)
+//   phase 2: block[a][xi0 xi1 xi2] = sum_terms coef sum_c D_c(xi_p0, xi_p1) S_f2[(c,a), xi_p2],
+//            one half row (2 sink spins of one baryon) at a time: every thread owns a register
+//            tile of 2 (spins) x 2 x 2 x 2 (xi0, xi1, xi2) outputs, so each shared-memory operand
+//            is used 4 times (0.5 loads per complex MAC for any permutation p); the half row is
+//            assembled in shared memory in the staged layout of nbs_tables.hpp (plane a at
+//            a*SM_PLANE, triple at sm_index, pads = 0) and copied to HBM fully coalesced.
 // ---------------------------------------------------------------------------------------------
 struct BTermRec {
     double coef;
@@ -49,15 +53,52 @@ struct BlockRec {
 };
 
 constexpr int BLOCKS_THREADS = 256;
+constexpr int BLOCKS_TILES = 216;               // 6 x 6 x 6 tiles of 2 x 2 x 2 source triples
+constexpr int BLOCKS_HALF = 2 * SM_PLANE;       // complex entries of a half row
+inline size_t blocks_smem_bytes(int ndq) { return (size_t)(3 * 144 + ndq * 432 + BLOCKS_HALF) * sizeof(double2); }
 
-__global__ void __launch_bounds__(BLOCKS_THREADS)
+// acc[a][e0][e1][e2] += coef * sum_c D_c(xi_P0, xi_P1) * S[(c, a0 + a), xi_P2] over the thread's tile
+template <int P0, int P1, int P2>
+__device__ __forceinline__ void blocks_term(double2 (&acc)[2][2][2][2], const double2* __restrict__ Dq,
+                                            const double2* __restrict__ S2, double coef, int a0, const int (&x)[3]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double2 Dv[2][2], Sv[2][2];
+#pragma unroll
+        for (int ja = 0; ja < 2; ++ja)
+#pragma unroll
+            for (int jb = 0; jb < 2; ++jb) Dv[ja][jb] = Dq[c * 144 + (x[P0] + ja) * 12 + x[P1] + jb];
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const double2 v = S2[(c + 3 * (a0 + a)) * 12 + x[P2] + j];
+                Sv[a][j] = make_double2(coef * v.x, coef * v.y);
+            }
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int e0 = 0; e0 < 2; ++e0)
+#pragma unroll
+                for (int e1 = 0; e1 < 2; ++e1)
+#pragma unroll
+                    for (int e2 = 0; e2 < 2; ++e2) {
+                        const int e[3] = {e0, e1, e2};
+                        cfma(acc[a][e0][e1][e2], Dv[e[P0]][e[P1]], Sv[a][e[P2]]);
+                    }
+    }
+}
+
+__global__ void __launch_bounds__(BLOCKS_THREADS, 2)
 k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const double2* __restrict__ Ss,
          const int* __restrict__ baryon_of_slot, int nslots, unsigned dq_mask,
          const BlockRec* __restrict__ brec, const BTermRec* __restrict__ bterm,
-         double2* __restrict__ out, size_t row_stride, int staged) {
+         double2* __restrict__ out, size_t row_stride) {
     extern __shared__ double2 smem[];
-    double2* sS = smem;            // [3][144]
-    double2* sD = smem + 3 * 144;  // [9][3][144]
+    const int ndq = __popc(dq_mask);
+    double2* sS = smem;                  // [3][144]
+    double2* sD = smem + 3 * 144;        // [ndq][3][144], needed diquark types in increasing dq order
+    double2* sO = sD + ndq * 432;        // [2][SM_PLANE] half row being assembled
     const size_t site = blockIdx.x;
     const int tid = threadIdx.x;
     for (int i = tid; i < 144; i += BLOCKS_THREADS) {
@@ -66,19 +107,21 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
         sS[288 + i] = Ss[site * 144 + i];
     }
     __syncthreads();
-    for (int idx = tid; idx < 9 * 432; idx += BLOCKS_THREADS) {
-        int dq = idx / 432;
-        if (!((dq_mask >> dq) & 1u)) continue;
-        int rem = idx - dq * 432;
-        int c = rem / 144, i = (rem / 12) % 12, j = rem % 12;
+    for (int idx = tid; idx < ndq * 432; idx += BLOCKS_THREADS) {
+        const int slot_dq = idx / 432;
+        int dq = 0; // the slot_dq-th set bit of dq_mask
+        for (int seen = 0; dq < 9; ++dq)
+            if ((dq_mask >> dq) & 1u) { if (seen == slot_dq) break; ++seen; }
+        const int rem = idx - slot_dq * 432;
+        const int c = rem / 144, i = (rem / 12) % 12, j = rem % 12;
         const double2* S0 = sS + (dq / 3) * 144;
         const double2* S1 = sS + (dq % 3) * 144;
-        int a = (c + 1) % 3, b = (c + 2) % 3;
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
         double2 acc = make_double2(0.0, 0.0), neg = make_double2(0.0, 0.0);
         // (C g5)_{01} = +1, (C g5)_{10} = -1, (C g5)_{23} = +1, (C g5)_{32} = -1
 #pragma unroll
         for (int pr = 0; pr < 2; ++pr) {
-            int be = 2 * pr, ga = 2 * pr + 1;
+            const int be = 2 * pr, ga = 2 * pr + 1;
             cfma(acc, S0[(a + 3 * be) * 12 + i], S1[(b + 3 * ga) * 12 + j]); // +eps +cg5
             cfma(neg, S0[(a + 3 * ga) * 12 + i], S1[(b + 3 * be) * 12 + j]); // +eps -cg5
             cfma(neg, S0[(b + 3 * be) * 12 + i], S1[(a + 3 * ga) * 12 + j]); // -eps +cg5
@@ -86,45 +129,60 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
         }
         sD[idx] = csub(acc, neg);
     }
+    // pads of the half-row buffer stay zero for the whole kernel
+    if (tid < 24) sO[(tid / 12) * SM_PLANE + (tid % 12) * SM_STRIDE1 + 144] = make_double2(0.0, 0.0);
     __syncthreads();
+
+    const int x[3] = {2 * (tid / 36), 2 * ((tid / 6) % 6), 2 * (tid % 6)}; // tile origin (tid < 216)
     double2* orow = out + site * row_stride;
-    // staged != 0: every (site, slot) row is written in the padded, skewed layout the product
-    // kernel gathers from (nbs_tables.hpp: plane a at a*SM_PLANE, triple at sm_index, pads = 0), so
-    // that staging a block is a plain bulk copy.  staged == 0: [alpha][xi1][xi2][xi3] (nbs_blocks_x).
-    const int row_elems = staged ? SM_BLOCK : BLOCK_ELEMS;
-    const int total = nslots * row_elems;
-    for (int idx = tid; idx < total; idx += BLOCKS_THREADS) {
-        int slot = idx / row_elems;
-        int rem = idx - slot * row_elems;
-        int al, xi[3];
-        if (staged) {
-            al = rem / SM_PLANE;
-            int w = rem - al * SM_PLANE;
-            xi[0] = w / SM_STRIDE1;
-            w -= xi[0] * SM_STRIDE1;
-            if (w == 144) { orow[idx] = make_double2(0.0, 0.0); continue; } // pad
-            xi[1] = w / 12;
-            int x3 = w - xi[1] * 12 - xi[1];
-            xi[2] = x3 < 0 ? x3 + 12 : x3;
-        } else {
-            al = rem / NTRIPLE;
-            int t = rem - al * NTRIPLE;
-            xi[0] = t / 144; xi[1] = (t / 12) % 12; xi[2] = t % 12;
-        }
-        BlockRec br = brec[baryon_of_slot[slot]];
-        double2 val = make_double2(0.0, 0.0);
-        for (int it = br.term_begin; it < br.term_end; ++it) {
-            BTermRec bt = bterm[it];
-            const double2* Dq = sD + bt.dq * 432 + xi[bt.p0] * 12 + xi[bt.p1];
-            const double2* S2 = sS + bt.f2 * 144 + (3 * al) * 12 + xi[bt.p2];
-            double2 acc = make_double2(0.0, 0.0);
+    for (int slot = 0; slot < nslots; ++slot) {
+        const BlockRec br = brec[baryon_of_slot[slot]];
+        for (int half = 0; half < 2; ++half) {
+            if (tid < BLOCKS_TILES) {
+                double2 acc[2][2][2][2];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) cfma(acc, Dq[c * 144], S2[c * 12]);
-            val.x = fma(bt.coef, acc.x, val.x);
-            val.y = fma(bt.coef, acc.y, val.y);
+                for (int i = 0; i < 16; ++i) (&acc[0][0][0][0])[i] = make_double2(0.0, 0.0);
+                for (int it = br.term_begin; it < br.term_end; ++it) {
+                    const BTermRec bt = bterm[it];
+                    const double2* Dq = sD + __popc(dq_mask & ((1u << bt.dq) - 1u)) * 432;
+                    const double2* S2 = sS + bt.f2 * 144;
+                    const int perm = bt.p0 * 3 + bt.p1; // (p0, p1) fixes the permutation
+                    switch (perm) {
+                    case 1: blocks_term<0, 1, 2>(acc, Dq, S2, bt.coef, 2 * half, x); break;
+                    case 2: blocks_term<0, 2, 1>(acc, Dq, S2, bt.coef, 2 * half, x); break;
+                    case 3: blocks_term<1, 0, 2>(acc, Dq, S2, bt.coef, 2 * half, x); break;
+                    case 5: blocks_term<1, 2, 0>(acc, Dq, S2, bt.coef, 2 * half, x); break;
+                    case 6: blocks_term<2, 0, 1>(acc, Dq, S2, bt.coef, 2 * half, x); break;
+                    default: blocks_term<2, 1, 0>(acc, Dq, S2, bt.coef, 2 * half, x); break;
+                    }
+                }
+#pragma unroll
+                for (int a = 0; a < 2; ++a)
+#pragma unroll
+                    for (int e0 = 0; e0 < 2; ++e0)
+#pragma unroll
+                        for (int e1 = 0; e1 < 2; ++e1)
+#pragma unroll
+                            for (int e2 = 0; e2 < 2; ++e2)
+                                sO[a * SM_PLANE + sm_index(x[0] + e0, x[1] + e1, x[2] + e2)] = acc[a][e0][e1][e2];
+            }
+            __syncthreads();
+            double2* dst = orow + (size_t)slot * SM_BLOCK + half * BLOCKS_HALF;
+            for (int i = tid; i < BLOCKS_HALF; i += BLOCKS_THREADS) dst[i] = sO[i];
+            __syncthreads();
         }
-        orow[idx] = val;
     }
+}
+
+// Staged block rows [site][SM_BLOCK] -> [site][alpha][xi1][xi2][xi3] (nbs_blocks_x, tests only).
+__global__ void __launch_bounds__(256)
+k_unstage(const double2* __restrict__ in, size_t V, double2* __restrict__ out) {
+    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= V * BLOCK_ELEMS) return;
+    const size_t site = idx / BLOCK_ELEMS;
+    const int rem = (int)(idx - site * BLOCK_ELEMS);
+    const int al = rem / NTRIPLE, t = rem - al * NTRIPLE;
+    out[idx] = in[site * SM_BLOCK + al * SM_PLANE + sm_index(t / 144, (t / 12) % 12, t % 12)];
 }
 
 // ---------------------------------------------------------------------------------------------

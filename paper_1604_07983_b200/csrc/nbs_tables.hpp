@@ -22,7 +22,12 @@ constexpr int BLOCK_ELEMS = 6912; // 4 sink spins x 12^3
 constexpr int SM_STRIDE1 = 145;
 constexpr int SM_PLANE = 12 * SM_STRIDE1;  // 1740
 constexpr int SM_BLOCK = 4 * SM_PLANE;     // 6960 complex per staged block
-constexpr int sm_index(int xi1, int xi2, int xi3) { return xi1 * SM_STRIDE1 + xi2 * 12 + (xi3 + xi2) % 12; }
+#ifdef __CUDACC__
+#define NBS_HD __host__ __device__
+#else
+#define NBS_HD
+#endif
+NBS_HD constexpr int sm_index(int xi1, int xi2, int xi3) { return xi1 * SM_STRIDE1 + xi2 * 12 + (xi3 + xi2) % 12; }
 
 // One elementary operator  eps_abc (q_f0,a  C g5  q_f1,b) q_f2,c  with a real coefficient
 // (eqs. 2.2-2.3).  Flavours: 0 = u, 1 = d, 2 = s.
