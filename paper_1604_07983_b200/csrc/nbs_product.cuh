@@ -318,8 +318,8 @@ __device__ __forceinline__ size_t minus_q(int L, size_t q) {
 // correlators = real combinations of them (eqs. 2.2-2.3) -> Ft[q][ch][256].
 __device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* __restrict__ pr, size_t q,
                                              const double2* __restrict__ scr, int et) {
-    constexpr int CG = 4; // channels per pass over the unit results
-    const int nelem = pr->nelem, nchan = pr->nchan;
+    constexpr int CG = 6; // channels per pass over the unit results
+    const int nelem = pr->nelem, nchan = pr->nchan, swap_mask = pr->swap_mask;
     for (int c0 = 0; c0 < nchan; c0 += CG) {
         double2 acc[CG][4];
 #pragma unroll
@@ -340,14 +340,35 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* 
                     s[m].y += v.y;
                 }
             }
+            // source swap (reading A11): the same sums at the component with a3 <-> a4
+            // exchanged live in another lane of the same 16-lane group
+            const bool sw = (swap_mask >> e) & 1;
+            double2 ss[4];
+            if (sw) {
+                const int src_lane = (et & 0x10) | ((et & 3) << 2) | ((et >> 2) & 3);
+#pragma unroll
+                for (int m = 0; m < 4; ++m) {
+                    ss[m].x = __shfl_sync(0xffffffffu, s[m].x, src_lane);
+                    ss[m].y = __shfl_sync(0xffffffffu, s[m].y, src_lane);
+                }
+            }
 #pragma unroll
             for (int c = 0; c < CG; ++c) {
                 if (c0 + c < nchan) {
-                    const double k = __ldg(&a.pair_chans[pr->chan_begin + c0 + c].coef[e]);
+                    const PairChanRec* pc = a.pair_chans + pr->chan_begin + c0 + c;
+                    const double k = __ldg(&pc->coef[e]);
 #pragma unroll
                     for (int m = 0; m < 4; ++m) {
                         acc[c][m].x = fma(k, s[m].x, acc[c][m].x);
                         acc[c][m].y = fma(k, s[m].y, acc[c][m].y);
+                    }
+                    if (sw) {
+                        const double ks = __ldg(&pc->coefS[e]);
+#pragma unroll
+                        for (int m = 0; m < 4; ++m) {
+                            acc[c][m].x = fma(ks, ss[m].x, acc[c][m].x);
+                            acc[c][m].y = fma(ks, ss[m].y, acc[c][m].y);
+                        }
                     }
                 }
             }

@@ -358,52 +358,19 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         }
     }
 
-    // flatten: pairs -> elems -> diagrams -> gather tables (deduplicated by content)
-    std::map<std::vector<uint16_t>, uint32_t> dedupe;
-    auto intern = [&](const std::vector<uint16_t>& g) {
-        auto it = dedupe.find(g);
-        if (it != dedupe.end()) return it->second;
-        uint32_t off = (uint32_t)plan.gather.size();
-        plan.gather.insert(plan.gather.end(), g.begin(), g.end());
-        while (plan.gather.size() % 8) plan.gather.push_back(0); // 16-byte aligned tables
-        dedupe[g] = off;
-        return off;
-    };
-    std::vector<std::map<Key, int>> elem_id(pair_list.size());
-    for (size_t ip = 0; ip < pair_list.size(); ++ip) {
-        PairRec pr;
-        pr.slot1 = slot_of[pair_list[ip].first];
-        pr.slot2 = slot_of[pair_list[ip].second];
-        pr.elem_begin = (int)plan.elems.size();
+    // Source-swap reduction (reading A11): exchanging the two source operators gives
+    //   E[B3 B4]_{a1 a2 a3 a4} = - E[B4 B3]_{a1 a2 a4 a3},
+    // so of two elementary correlators of one sink pair whose source operators are each other's
+    // swap only the lexicographically smaller key is computed; the epilogue reads the other one
+    // from it with a3 <-> a4 exchanged and the sign flipped.
+    auto swapped = [](const Key& k) { return Key{k[3], k[4], k[5], k[0], k[1], k[2]}; };
+    std::vector<std::vector<Key>> pair_comp_order(pair_list.size()); // computed keys
+    for (size_t ip = 0; ip < pair_list.size(); ++ip)
         for (auto& k : pair_elem_order[ip]) {
-            ElemRec er;
-            er.diag_begin = (int)plan.diagrams.size();
-            for (auto& d : pair_elems[ip][k]) {
-                SideTable s1 = make_side(d.P, d.sign); // sigma_P folded into side 1
-                SideTable s2 = make_side(d.P + 3, +1);
-                DiagramRec r;
-                r.off1 = intern(s1.g); r.off2 = intern(s2.g);
-                r.K = (uint16_t)s1.K;
-                r.n1 = (uint8_t)s1.n; r.n2 = (uint8_t)s2.n;
-                r.C1 = (uint8_t)s1.C; r.C2 = (uint8_t)s2.C;
-                r.mask1 = (uint8_t)s1.carries;
-                r.pad = 0;
-                if (s1.K != s2.K || (s1.carries ^ s2.carries) != 3) return "internal: inconsistent cut";
-                plan.diagrams.push_back(r);
-                plan.sumK_exec += s1.K;
-            }
-            er.diag_end = (int)plan.diagrams.size();
-            elem_id[ip][k] = (int)plan.elems.size();
-            plan.elems.push_back(er);
+            const Key ks = swapped(k);
+            const bool derived = ks != k && pair_elems[ip].count(ks) && ks < k;
+            if (!derived) pair_comp_order[ip].push_back(k);
         }
-        pr.elem_end = (int)plan.elems.size();
-        plan.pairs.push_back(pr);
-    }
-    plan.chan_term_begin.push_back(0);
-    for (size_t ic = 0; ic < channels.size(); ++ic) {
-        for (auto& ct : chan_ct[ic]) plan.chan_terms.push_back(ChanTermRec{elem_id[ct.pair][ct.key], ct.coef});
-        plan.chan_term_begin.push_back((int)plan.chan_terms.size());
-    }
 
     // ---- product kernel tables: pairs -> (<= MAX_PAIR_ELEMS elementary correlators) -> units -> diagrams
     // layout: 0 = 16x16 side, 1 = 64x4 A side, 2 = 64x4 B side (see nbs_tables.hpp)
@@ -447,7 +414,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
     };
     const int UNIT_SPLIT_STEPS = unit_split_steps, UNIT_COST_MAX = unit_cost_max; // cost: 2 per 16x16 step, 3 per 64x4 step
     for (size_t ip = 0; ip < pair_list.size(); ++ip) {
-        const std::vector<Key>& order = pair_elem_order[ip];
+        const std::vector<Key>& order = pair_comp_order[ip];
         // at most 15 distinct elementary source operator pairs share the flavour content of one sink pair
         if (order.size() > (size_t)MAX_PAIR_ELEMS) return "internal: more than 16 elementary correlators for one sink pair";
         Pair3Rec pr;
@@ -456,6 +423,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         pr.unit_begin = (int)plan.units3.size();
         pr.diag_begin = (int)plan.diags3.size();
         pr.nelem = (int)order.size();
+        pr.swap_mask = 0;
         std::vector<Unit3Rec> units;
         std::vector<int> cost_of;
         for (size_t e = 0; e < order.size(); ++e) {
@@ -486,6 +454,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
                     r.offA = intern3(A, c < 2 ? 0 : 1); r.offB = intern3(B, c < 2 ? 0 : 2);
                     if (!tab_err.empty()) return tab_err;
                     r.K = (uint16_t)s1.K;
+                    plan.sumK_exec += s1.K;
                     r.nwA = (uint8_t)(A.n / 2); r.nwB = (uint8_t)(B.n / 2);
                     // split long diagrams into k-ranges so that a sink pair with few diagrams
                     // still spreads over all warps of the CTA
@@ -521,10 +490,15 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             PairChanRec pc;
             pc.ch = (int)ic; pc.pad = 0;
             bool any = false;
-            for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = 0.0;
+            for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = pc.coefS[e] = 0.0;
             for (auto& ct : chan_ct[ic])
-                for (size_t e = 0; e < order.size(); ++e)
+                for (size_t e = 0; e < order.size(); ++e) {
                     if (order[e] == ct.key) { pc.coef[e] += ct.coef; any = true; }
+                    else if (order[e] == swapped(ct.key)) { // derived: - (computed one with a3 <-> a4)
+                        pc.coefS[e] -= ct.coef; any = true;
+                        pr.swap_mask |= 1 << e;
+                    }
+                }
             if (any) plan.pair_chans.push_back(pc);
         }
         pr.nchan = (int)plan.pair_chans.size() - pr.chan_begin;

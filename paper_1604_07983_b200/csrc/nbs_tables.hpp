@@ -51,27 +51,6 @@ struct BlockTerm {
 };
 std::vector<BlockTerm> block_terms(int baryon);
 
-// Device-side records (plain old data, copied verbatim).
-struct DiagramRec {
-    uint32_t off1, off2; // offsets (in uint16 units) of the two gather tables
-    uint16_t K;          // size of the shared index xi~_d (1, 9, 36, 144)
-    uint8_t n1, n2;      // gather terms per effective-block entry, side 1 / side 2
-    uint8_t C1, C2;      // number of carried source-spin combinations, side 1 / side 2 (C1*C2 = 16)
-    uint8_t mask1;       // bit0: side 1 carries a3; bit1: side 1 carries a4
-    uint8_t pad;
-};
-struct ElemRec {
-    int diag_begin, diag_end; // range in the diagram array
-};
-struct PairRec {
-    int slot1, slot2;         // block slots (index into the context's list of needed baryons)
-    int elem_begin, elem_end; // range in the elementary-correlator array
-};
-struct ChanTermRec {
-    int elem; // global elementary-correlator index
-    double coef;
-};
-
 // ---- product kernel (DMMA) records ----------------------------------------------------------
 // A "unit" is the work of one warp: a few diagrams (or k-ranges of one diagram) of ONE elementary
 // correlator that share one accumulator layout (class).  Classes (which effective
@@ -110,10 +89,12 @@ struct Pair3Rec {
     int nelem;
     int elem_unit_begin[MAX_PAIR_ELEMS + 1]; // scratch-row ranges per elementary correlator
     int chan_begin, nchan;   // range in Plan::pair_chans
+    int swap_mask;           // bit e: some channel needs elementary correlator e with a3 <-> a4 exchanged
 };
 struct PairChanRec {
     int ch, pad;
-    double coef[MAX_PAIR_ELEMS]; // channel = sum_e coef[e] * elementary correlator e (eqs. 2.2-2.3)
+    double coef[MAX_PAIR_ELEMS];  // channel = sum_e coef[e] * E_e + coefS[e] * (E_e with a3 <-> a4), eqs. 2.2-2.3;
+    double coefS[MAX_PAIR_ELEMS]; // coefS carries the minus sign of the source swap (reading A11)
 };
 struct ChainRec { // order in which one CTA walks the sink pairs of one momentum q
     int pair;
@@ -131,12 +112,6 @@ struct DiagramInfo { // host-side description (tests, statistics)
 struct Plan {
     std::vector<nbs_channel> channels;
     std::vector<int> baryons; // needed sink baryon ids, slot order
-    std::vector<PairRec> pairs;
-    std::vector<ElemRec> elems;
-    std::vector<DiagramRec> diagrams;
-    std::vector<uint16_t> gather; // bit 15: minus sign; bits 0-10: triple index t
-    std::vector<int> chan_term_begin; // size nch+1
-    std::vector<ChanTermRec> chan_terms;
     std::vector<int> chan_pair; // pair index of each channel
     double sumK_std = 0;        // sum over channels of sum_d K_d (the paper's count)
     double sumK_exec = 0;       // sum over distinct elementary correlators
