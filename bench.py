@@ -28,8 +28,11 @@ if ROOT not in sys.path:
 
 METRIC = "nbs_correlator_time_slices_per_s_52ch_32c64_fp64"
 UNIT = "time-slices/s"
-FP64_PEAK_TFLOPS = 37.2  # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz; the
-#                          in-tree probe measured 37.1 (DMMA) / 33.7 (DFMA) TFLOP/s on this pool
+FP64_PEAK_TFLOPS = 37.2  # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz; a register-resident
+#                          probe on this pool measured 37.1 (DMMA.8x8x4) and 34.2 (DFMA) TFLOP/s; the two share the units
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_product launch on this workload, from the ncu --set full
+# capture summarised in profiles/r1_v4_summary.md (update together with that file)
+PRODUCT_DRAM_TRAFFIC_BYTES = 110.2e9
 
 
 def parse():
@@ -276,7 +279,7 @@ def main():
         "stages_ms_per_step": {k: v[0] / max(v[1], 1) for k, v in stage.items()},
         "roofline": {"bound": "alu", "kernel": "product (effective blocks x product, eqs. 4.2-4.3)",
                      "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": PRODUCT_DRAM_TRAFFIC_BYTES,
                      "peak_source": "derived FP64 pipe peak 148 SM x 64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
                      "flops_per_launch_algorithmic": alg_flops,
                      "flops_per_launch_executed": flops["product_executed"] * V,

@@ -38,7 +38,10 @@ constexpr uint32_t BLOCK_BYTES = SM_BLOCK * 16u;  // 111 360
 // shared-memory map (bytes)
 constexpr uint32_t SMO_S1 = 0, SMO_S2 = BLOCK_BYTES, SMO_UNITS = 2 * BLOCK_BYTES;
 constexpr uint32_t SMO_DIAGS = SMO_UNITS + MAX_PAIR_UNITS * 16u;
-constexpr uint32_t SMO_CTRL = SMO_DIAGS + MAX_PAIR_DIAGS * 16u;
+constexpr int EPI_CG = 6; // channels per epilogue pass over the unit results
+constexpr uint32_t SMO_EPI = SMO_DIAGS + MAX_PAIR_DIAGS * 16u; // epilogue's copy of the pair and channel records
+constexpr uint32_t EPI_PAIR_BYTES = (sizeof(Pair3Rec) + 15u) / 16u * 16u;
+constexpr uint32_t SMO_CTRL = SMO_EPI + EPI_PAIR_BYTES + EPI_CG * (uint32_t)sizeof(PairChanRec) + 8u;
 constexpr int PROD_NBUF = 4; // depth of the unit-result ring between compute and epilogue warps
 constexpr size_t PROD_SMEM = SMO_CTRL + 128;
 static_assert(sizeof(Unit3Rec) == 16 && sizeof(Diag3Rec) == 16, "record sizes");
@@ -81,8 +84,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 __device__ __forceinline__ void named_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void named_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-enum { BAR_COMPUTE = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 2 + PROD_NBUF };
-static_assert(2 + 2 * PROD_NBUF <= 16, "named barriers");
+enum { BAR_COMPUTE = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 2 + PROD_NBUF, BAR_EPI = 2 + 2 * PROD_NBUF };
+static_assert(3 + 2 * PROD_NBUF <= 16, "named barriers");
+static_assert(sizeof(Pair3Rec) % 4 == 0 && sizeof(PairChanRec) % 8 == 0 && SMO_CTRL % 8 == 0, "record alignment");
+
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // ---- gathers (eq. 4.2) ----------------------------------------------------------------------
 // One table word = one (+, -) pair of byte offsets into a staged block.  ld_pair issues the
@@ -164,6 +170,7 @@ __device__ __forceinline__ void run_unit_square(const Unit3Rec u, const Diag3Rec
                 ld_pair<2, PS>(s1, wa, ua, va); // one step past the end reads a valid (unused) entry
                 ld_pair<2, PS>(s2, wb, ub, vb);
                 na = __ldg(tA + 32); nb = __ldg(tB + 32);
+                prefetch_l1(tA + 5 * 32); prefetch_l1(tB + 5 * 32); // L2 latency > 2 k-steps: pull the words into L1 early
                 mma_square(acc, A, B);
                 sub_pair<2, true>(ua, va, A);
                 sub_pair<2, true>(ub, vb, B);
@@ -267,6 +274,7 @@ __device__ __forceinline__ void run_unit_wide(const Unit3Rec u, const Diag3Rec* 
             wide_fold_B(ub, vb, Bv);
             wide_loads_A(sA, na01, na23, ua, va); // one step past the end reads valid (unused) entries
             na01 = __ldg(tA + 64); na23 = __ldg(tA + 65);
+            prefetch_l1(tA + 3 * 64); prefetch_l1(tB + 3 * 32); // L2 latency > 1 k-step: pull the words into L1 early
             mma_wide(acc, A, Bv[0], hi);
 #pragma unroll
             for (int g = 0; g < 4; ++g) sub_pair<2, true>(ua[g], va[g], A[g]);
@@ -315,15 +323,30 @@ __device__ __forceinline__ size_t minus_q(int L, size_t q) {
 }
 
 // Epilogue of one item: elementary correlators = sums of unit results (fixed order), channel
-// correlators = real combinations of them (eqs. 2.2-2.3) -> Ft[q][ch][256].
-__device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* __restrict__ pr, size_t q,
-                                             const double2* __restrict__ scr, int et) {
-    constexpr int CG = 6; // channels per pass over the unit results
+// correlators = real combinations of them (eqs. 2.2-2.3) -> Ft[q][ch][256].  The pair record and
+// the channel coefficients are first copied to shared memory (one L2 round trip for the item
+// instead of one per use); thread et owns the spin components et + 64 m.
+__device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q, const double2* __restrict__ scr,
+                                             int et, char* s_epi) {
+    Pair3Rec* pr = reinterpret_cast<Pair3Rec*>(s_epi);
+    PairChanRec* pcs = reinterpret_cast<PairChanRec*>(s_epi + EPI_PAIR_BYTES);
+    {
+        const int* src = reinterpret_cast<const int*>(a.pairs + ip);
+        if (et < (int)(sizeof(Pair3Rec) / 4)) reinterpret_cast<int*>(pr)[et] = __ldg(src + et);
+    }
+    named_sync(BAR_EPI, PROD_ETHREADS);
     const int nelem = pr->nelem, nchan = pr->nchan, swap_mask = pr->swap_mask;
-    for (int c0 = 0; c0 < nchan; c0 += CG) {
-        double2 acc[CG][4];
+    for (int c0 = 0; c0 < nchan; c0 += EPI_CG) {
+        const int nc = min(EPI_CG, nchan - c0);
+        {
+            const double* src = reinterpret_cast<const double*>(a.pair_chans + pr->chan_begin + c0);
+            const int nwords = nc * (int)(sizeof(PairChanRec) / 8);
+            for (int i = et; i < nwords; i += PROD_ETHREADS) reinterpret_cast<double*>(pcs)[i] = __ldg(src + i);
+        }
+        named_sync(BAR_EPI, PROD_ETHREADS);
+        double2 acc[EPI_CG][4];
 #pragma unroll
-        for (int c = 0; c < CG; ++c)
+        for (int c = 0; c < EPI_CG; ++c)
 #pragma unroll
             for (int m = 0; m < 4; ++m) acc[c][m] = make_double2(0.0, 0.0);
         for (int e = 0; e < nelem; ++e) {
@@ -331,14 +354,23 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* 
 #pragma unroll
             for (int m = 0; m < 4; ++m) s[m] = make_double2(0.0, 0.0);
             const int ub = pr->elem_unit_begin[e], ue = pr->elem_unit_begin[e + 1];
-#pragma unroll 8
-            for (int ul = ub; ul < ue; ++ul) {
+            // rows in groups of EG with all loads of a group in flight (an elementary correlator has
+            // ~5 unit rows: a plain unrolled loop would run them one by one through its remainder)
+            constexpr int EG = 4;
+            for (int ul = ub; ul < ue; ul += EG) {
+                double2 v[EG][4];
 #pragma unroll
-                for (int m = 0; m < 4; ++m) {
-                    const double2 v = __ldcg(scr + (size_t)ul * 256 + et + 64 * m);
-                    s[m].x += v.x;
-                    s[m].y += v.y;
-                }
+                for (int j = 0; j < EG; ++j)
+#pragma unroll
+                    for (int m = 0; m < 4; ++m)
+                        v[j][m] = (ul + j < ue) ? __ldcg(scr + (size_t)(ul + j) * 256 + et + 64 * m) : make_double2(0.0, 0.0);
+#pragma unroll
+                for (int j = 0; j < EG; ++j)
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        s[m].x += v[j][m].x;
+                        s[m].y += v[j][m].y;
+                    }
             }
             // source swap (reading A11): the same sums at the component with a3 <-> a4
             // exchanged live in another lane of the same 16-lane group
@@ -353,17 +385,16 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* 
                 }
             }
 #pragma unroll
-            for (int c = 0; c < CG; ++c) {
-                if (c0 + c < nchan) {
-                    const PairChanRec* pc = a.pair_chans + pr->chan_begin + c0 + c;
-                    const double k = __ldg(&pc->coef[e]);
+            for (int c = 0; c < EPI_CG; ++c) {
+                if (c < nc) {
+                    const double k = pcs[c].coef[e];
 #pragma unroll
                     for (int m = 0; m < 4; ++m) {
                         acc[c][m].x = fma(k, s[m].x, acc[c][m].x);
                         acc[c][m].y = fma(k, s[m].y, acc[c][m].y);
                     }
                     if (sw) {
-                        const double ks = __ldg(&pc->coefS[e]);
+                        const double ks = pcs[c].coefS[e];
 #pragma unroll
                         for (int m = 0; m < 4; ++m) {
                             acc[c][m].x = fma(ks, ss[m].x, acc[c][m].x);
@@ -374,15 +405,16 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, const Pair3Rec* 
             }
         }
 #pragma unroll
-        for (int c = 0; c < CG; ++c) {
-            if (c0 + c < nchan) {
-                const int ch = __ldg(&a.pair_chans[pr->chan_begin + c0 + c].ch) - a.ch_begin;
+        for (int c = 0; c < EPI_CG; ++c) {
+            if (c < nc) {
+                const int ch = pcs[c].ch - a.ch_begin;
                 if (ch >= 0 && ch < a.nch_out) {
 #pragma unroll
                     for (int m = 0; m < 4; ++m) __stcs(a.Ft + (q * a.nch_out + ch) * 256 + et + 64 * m, acc[c][m]);
                 }
             }
         }
+        named_sync(BAR_EPI, PROD_ETHREADS); // the channel records may be overwritten by the next pass / item
     }
 }
 
@@ -418,7 +450,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
-            combine_item(a, a.pairs + ip, q, scr0 + b * scr_stride, et);
+            combine_item(a, ip, q, scr0 + b * scr_stride, et, smem + SMO_EPI);
             named_arrive(BAR_EMPTY0 + b, PROD_THREADS);
         }
         return;
@@ -493,8 +525,9 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             const int4 uv = *reinterpret_cast<const int4*>(s_units + i);
             Unit3Rec u;
             u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
-            const int inext = grab();
-            if (inext < nunits && lane < 16) {
+            // (not near the end of the item: holding a unit back there would lengthen the tail)
+            const int inext = (i + 2 * PROD_CWARPS < nunits) ? grab() : -1;
+            if (inext >= 0 && inext < nunits && lane < 16) {
                 const Diag3Rec nd = load_diag(s_diags + s_units[inext].diag_begin);
                 const int wide = s_units[inext].cls >= 2;
                 const uint32_t off = (lane < 8) ? nd.offA + (uint32_t)nd.sbeg * (wide ? 128u : 32u * nd.nwA)
@@ -505,7 +538,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             double2* out = scr + (size_t)u.slot * 256;
             if (u.cls < 2) run_unit_square(u, s_diags, a.tab, s1, s2, out, lane);
             else run_unit_wide(u, s_diags, a.tab, s1, s2, out, lane);
-            i = inext;
+            i = inext >= 0 ? inext : grab();
         }
         __threadfence_block();
         named_arrive(BAR_FULL0 + b, PROD_THREADS); // unit results of this item are in scratch buffer b

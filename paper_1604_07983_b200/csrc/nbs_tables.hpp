@@ -69,8 +69,8 @@ std::vector<BlockTerm> block_terms(int baryon);
 //   64x4  B side   [k][a][nw]                               plane a
 // k is padded to a multiple of 4 (one DMMA k-step).
 constexpr int MAX_PAIR_ELEMS = 16;
-constexpr int MAX_PAIR_UNITS = 256; // unit and diagram records of one sink pair are staged in shared memory
-constexpr int MAX_PAIR_DIAGS = 256;
+constexpr int MAX_PAIR_UNITS = 128; // unit and diagram records of one sink pair are staged in shared memory
+constexpr int MAX_PAIR_DIAGS = 192;
 struct Diag3Rec {
     uint32_t offA, offB; // uint2 offsets into Plan::tab3: operand A (the M side) and operand B (the N side)
     uint16_t sbeg, send; // k-steps [sbeg, send) of this diagram covered by this record
@@ -128,7 +128,7 @@ struct Plan {
 
 // Returns "" on success, else an error message (invalid id, flavour violation).
 std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps = 18,
-                       int unit_cost_max = 64);
+                       int unit_cost_max = 80);
 
 // Diagrams of one channel in enumeration order (source terms major, permutations lexicographic).
 std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& out);

@@ -221,3 +221,55 @@ def test_errors(torch_cuda, nbs):
         with pytest.raises(nbs.NbsError) as e:
             ctx.correlator(0, 0, 52, out=small)
         assert e.value.code == nbs.NBS_EINVAL
+
+
+def test_full_size_32cubed_52_channels_sparse_support(torch_cuda, nbs, oracle):
+    """BASELINE.json configs[2] in the launch configuration bench.py times (32^3, T = 64, all 52
+    channels, u != d != s), on outputs the oracle can compute one by one: the propagators of
+    configs[2] are kept on 5 sites and zeroed elsewhere, so the blocks (products of propagators at
+    one site) live on those sites and eq. 2.4 gives
+        F(r) = sum_{(i, j): x_i - x_j = r (mod L)} pair_tensor(B1(x_i), B2(x_j)),
+    non-zero at <= 21 displacements r and exactly zero at the other 32747.  The CUDA path runs its
+    full-volume kernels (blocks, 32-point FFTs, product over all 32768 momenta, inverse FFT)."""
+    torch = torch_cuda
+    L, T, t = 32, 64, 17
+    V = L ** 3
+    cfg = synth.CONFIGS[2]
+    sites = [(0, 0, 0), (1, 31, 5), (31, 31, 31), (16, 0, 7), (3, 30, 12)]
+    idx = np.array([x + L * (y + L * z) for x, y, z in sites])
+    full = synth.config_slice(cfg, t)
+    S_sup = {f: np.ascontiguousarray(full[f][idx]) for f in "uds"}  # [5][12][12]
+    S = {}
+    for f in "uds":
+        S[f] = np.zeros_like(full[f])
+        S[f][idx] = S_sup[f]
+    del full
+    chans = oracle.channels52()
+    blocks = {n: oracle.block(S_sup, n) for n in oracle.sink_names(chans)}
+    ii, jj = np.meshgrid(np.arange(len(sites)), np.arange(len(sites)), indexing="ij")
+    ii, jj = ii.ravel(), jj.ravel()
+    rs = []
+    for i, j in zip(ii, jj):
+        d = [(sites[i][a] - sites[j][a]) % L for a in range(3)]
+        rs.append(d[0] + L * (d[1] + L * d[2]))
+    rs = np.array(rs)
+    uniq = sorted(set(rs.tolist()))
+    ref = np.zeros((len(chans), 256, len(uniq)), dtype=np.complex128)
+    for c, ch in enumerate(chans):
+        G = oracle.pair_tensor(blocks[ch[0]][ii], blocks[ch[1]][jj], ch).reshape(len(ii), 256)
+        for p, r in enumerate(rs):
+            ref[c, :, uniq.index(int(r))] += G[p]
+    with nbs.Nbs(L, T) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(t, d["u"], d["d"], d["s"])
+        F = ctx.correlator(t).reshape(len(chans), 256, V)
+        torch.cuda.synchronize()
+    ref_dev = torch.from_numpy(ref).cuda()
+    col = torch.tensor(uniq, device="cuda")
+    scale = ref_dev.abs().amax(dim=(1, 2))
+    assert float(scale.min()) > 0
+    err_on = (F[:, :, col] - ref_dev).abs().amax(dim=(1, 2)) / scale
+    F[:, :, col] = 0
+    err_off = F.abs().amax(dim=(1, 2)) / scale
+    worst = torch.maximum(err_on, err_off)
+    assert float(worst.max()) <= RTOL, (int(worst.argmax()), float(err_on.max()), float(err_off.max()))
