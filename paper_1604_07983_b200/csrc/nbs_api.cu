@@ -50,6 +50,8 @@ struct nbs_ctx {
     PairChanRec* d_pair_chans = nullptr;
     int* d_qorder = nullptr;
     int prod_grid = 0;
+    long long ntasks = 0;   // entries of d_qorder
+    long long nselfconj = 0; // momenta with q == -q
     int* d_baryon_of_slot = nullptr;
     int* d_one_baryon = nullptr; // scratch for nbs_blocks_x
     BlockRec* d_brec = nullptr;
@@ -253,12 +255,17 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
             x = x ? L - x : 0; y = y ? L - y : 0; z = z ? L - z : 0;
             return x + (size_t)L * (y + (size_t)L * z);
         };
+        // if every sink pair has identical baryons the momenta q > -q have nothing to compute
+        const bool skip_upper = c->plan.chain_half_n == 0;
         for (size_t q = 0; q < c->V; ++q) {
             if (seen[q]) continue;
             qorder.push_back((int)q); seen[q] = 1;
             size_t m = neg(q);
-            if (!seen[m]) { qorder.push_back((int)m); seen[m] = 1; }
+            if (!seen[m]) { if (!skip_upper) qorder.push_back((int)m); seen[m] = 1; }
         }
+        c->ntasks = (long long)qorder.size();
+        c->nselfconj = 0;
+        for (size_t q = 0; q < c->V; ++q) c->nselfconj += neg(q) == q;
         CUC(upload(c, c->d_qorder, qorder));
     }
     {
@@ -401,8 +408,8 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         CU(c, cudaMemsetAsync(sl.counter, 0, sizeof(unsigned long long), st));
         ProdArgs pa;
         pa.Bq = sl.B; pa.R = c->R; pa.L = c->L;
-        pa.npairs = (int)c->plan.pairs3.size();
-        pa.ntasks = (long long)c->V;
+        pa.chain_full_n = c->plan.chain_full_n; pa.chain_half_n = c->plan.chain_half_n;
+        pa.ntasks = c->ntasks;
         pa.qorder = c->d_qorder;
         pa.pairs = c->d_pairs3; pa.units = c->d_units3; pa.diags = c->d_diags3;
         pa.tab = reinterpret_cast<const uint2*>(c->d_tab3);
@@ -501,7 +508,9 @@ int nbs_model_flops(const nbs_ctx* c, double* blocks, double* fft, double* produ
 
 int nbs_exec_flops(const nbs_ctx* c, double* product_executed) {
     if (!c) return NBS_EINVAL;
-    if (product_executed) *product_executed = 8.0 * 256.0 * c->plan.sumK_exec;
+    // pairs of identical sink baryons are computed for the momenta q <= -q only
+    const double self_frac = 0.5 * (double)(c->V + c->nselfconj) / (double)c->V;
+    if (product_executed) *product_executed = 8.0 * 256.0 * (c->plan.sumK_exec + self_frac * c->plan.sumK_exec_self);
     return NBS_OK;
 }
 

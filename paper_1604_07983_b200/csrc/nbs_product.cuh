@@ -300,15 +300,15 @@ struct ProdArgs {
     const double2* Bq;   // [V][R] momentum-space normal blocks, every (site, slot) row in the staged layout
     size_t R;            // row length (complex) = nslots * SM_BLOCK
     int L;
-    int npairs;
-    long long ntasks;    // V momentum tasks
+    int chain_full_n, chain_half_n; // chain[0 .. full_n): all pairs (momenta q <= -q); then the half chain
+    long long ntasks;    // momentum tasks = entries of qorder
     const int* qorder;   // [V] momenta with q and -q adjacent
     const Pair3Rec* pairs;
     const Unit3Rec* units;
     const Diag3Rec* diags;
     const uint2* tab;
     const PairChanRec* pair_chans;
-    const ChainRec* chain; // [npairs]
+    const ChainRec* chain; // [chain_full_n + chain_half_n]
     double2* scratch;    // [gridDim.x][PROD_NBUF][max_pair_units][256]
     int max_pair_units;
     double2* Ft;         // [V][nch_out][256]
@@ -336,6 +336,8 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
     }
     named_sync(BAR_EPI, PROD_ETHREADS);
     const int nelem = pr->nelem, nchan = pr->nchan, swap_mask = pr->swap_mask;
+    const size_t mq = minus_q(a.L, q);
+    const bool mirror = pr->self_swap && mq != q;
     for (int c0 = 0; c0 < nchan; c0 += EPI_CG) {
         const int nc = min(EPI_CG, nchan - c0);
         {
@@ -411,6 +413,12 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
                 if (ch >= 0 && ch < a.nch_out) {
 #pragma unroll
                     for (int m = 0; m < 4; ++m) __stcs(a.Ft + (q * a.nch_out + ch) * 256 + et + 64 * m, acc[c][m]);
+                    if (mirror) { // sink swap: F~(-q)_{a2 a1 a3 a4} = - F~(q)_{a1 a2 a3 a4}; here a1 = m, a2 = et >> 4
+#pragma unroll
+                        for (int m = 0; m < 4; ++m)
+                            __stcs(a.Ft + (mq * a.nch_out + ch) * 256 + ((et >> 4) * 4 + m) * 16 + (et & 15),
+                                   make_double2(-acc[c][m].x, -acc[c][m].y));
+                    }
                 }
             }
         }
@@ -463,6 +471,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
     unsigned ntask = 0;
     long long qt = 0;
     size_t q = 0, mq = 0;
+    int cbase = 0, clen = 1;
     for (unsigned it = 0;; ++it) {
         const int b = it % PROD_NBUF;
         named_sync(BAR_COMPUTE, PROD_CTHREADS); // the staged blocks and unit records of the previous item are consumed
@@ -471,6 +480,9 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             if (qt < a.ntasks) {
                 q = (size_t)__ldg(a.qorder + qt);
                 mq = minus_q(a.L, q);
+                // momenta q > -q leave the pairs of identical sink baryons to the task of -q
+                cbase = (mq < q) ? a.chain_full_n : 0;
+                clen = (mq < q) ? a.chain_half_n : a.chain_full_n;
             }
         }
         if (it >= PROD_NBUF) named_sync(BAR_EMPTY0 + b, PROD_THREADS); // scratch buffer b and its descriptor are free again
@@ -480,8 +492,8 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             named_arrive(BAR_FULL0 + b, PROD_THREADS);
             break;
         }
-        const int ip = __ldg(&a.chain[pos].pair);
-        const int load1 = __ldg(&a.chain[pos].load1), load2 = __ldg(&a.chain[pos].load2);
+        const int ip = __ldg(&a.chain[cbase + pos].pair);
+        const int load1 = __ldg(&a.chain[cbase + pos].load1), load2 = __ldg(&a.chain[cbase + pos].load2);
         const Pair3Rec* pr = a.pairs + ip;
         const int nunits = __ldg(&pr->nunits);
         if (tid == 0) {
@@ -542,7 +554,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         }
         __threadfence_block();
         named_arrive(BAR_FULL0 + b, PROD_THREADS); // unit results of this item are in scratch buffer b
-        if (++pos == a.npairs) { pos = 0; ++ntask; }
+        if (++pos == clen) { pos = 0; ++ntask; }
     }
 }
 

@@ -424,6 +424,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         pr.diag_begin = (int)plan.diags3.size();
         pr.nelem = (int)order.size();
         pr.swap_mask = 0;
+        pr.self_swap = (pair_list[ip].first == pair_list[ip].second) ? 1 : 0;
         std::vector<Unit3Rec> units;
         std::vector<int> cost_of;
         for (size_t e = 0; e < order.size(); ++e) {
@@ -454,7 +455,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
                     r.offA = intern3(A, c < 2 ? 0 : 1); r.offB = intern3(B, c < 2 ? 0 : 2);
                     if (!tab_err.empty()) return tab_err;
                     r.K = (uint16_t)s1.K;
-                    plan.sumK_exec += s1.K;
+                    (pr.self_swap ? plan.sumK_exec_self : plan.sumK_exec) += s1.K;
                     r.nwA = (uint8_t)(A.n / 2); r.nwB = (uint8_t)(B.n / 2);
                     // split long diagrams into k-ranges so that a sink pair with few diagrams
                     // still spreads over all warps of the CTA
@@ -506,13 +507,17 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
     }
     plan.tab3.insert(plan.tab3.end(), 1024, uint2x{0, 0}); // the kernel prefetches a few k-steps past a table's end
 
-    // ---- chain: order of the sink pairs inside one momentum task that reloads the fewest blocks
-    {
-        const int n = (int)plan.pairs3.size();
+    // ---- chains: order of the sink pairs inside one momentum task that reloads the fewest blocks.
+    // Full chain (all pairs) for the momenta q <= -q (index order), half chain (without the pairs of
+    // identical sink baryons) for the others: for B1 == B2 the sink-swap relation (DESIGN.md reading
+    // A11)  F~_{a1 a2 ..}(-q) = - F~_{a2 a1 ..}(q)  gives the -q result from the q result.
+    auto make_chain = [&](const std::vector<int>& ids) {
+        const int n = (int)ids.size();
         auto tcost = [&](int a, int b) {
-            return (plan.pairs3[a].slot1 != plan.pairs3[b].slot1) + (plan.pairs3[a].slot2 != plan.pairs3[b].slot2);
+            return (plan.pairs3[ids[a]].slot1 != plan.pairs3[ids[b]].slot1) + (plan.pairs3[ids[a]].slot2 != plan.pairs3[ids[b]].slot2);
         };
         std::vector<int> best;
+        if (n == 0) return;
         if (n <= 16) { // exact: shortest Hamiltonian path by subset DP
             const int N = 1 << n, INF = 1 << 28;
             std::vector<int> dp((size_t)N * n, INF), from((size_t)N * n, -1);
@@ -546,11 +551,22 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         }
         for (int s = 0; s < n; ++s) {
             ChainRec cr;
-            cr.pair = best[s];
-            cr.load1 = (s == 0) || plan.pairs3[best[s]].slot1 != plan.pairs3[best[s - 1]].slot1;
-            cr.load2 = (s == 0) || plan.pairs3[best[s]].slot2 != plan.pairs3[best[s - 1]].slot2;
+            cr.pair = ids[best[s]];
+            cr.load1 = (s == 0) || plan.pairs3[cr.pair].slot1 != plan.pairs3[ids[best[s - 1]]].slot1;
+            cr.load2 = (s == 0) || plan.pairs3[cr.pair].slot2 != plan.pairs3[ids[best[s - 1]]].slot2;
             plan.chain.push_back(cr);
         }
+    };
+    {
+        std::vector<int> all, half;
+        for (int i = 0; i < (int)plan.pairs3.size(); ++i) {
+            all.push_back(i);
+            if (!plan.pairs3[i].self_swap) half.push_back(i);
+        }
+        make_chain(all);
+        plan.chain_full_n = (int)plan.chain.size();
+        make_chain(half);
+        plan.chain_half_n = (int)plan.chain.size() - plan.chain_full_n;
     }
     return "";
 }

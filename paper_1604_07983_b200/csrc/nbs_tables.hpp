@@ -90,6 +90,7 @@ struct Pair3Rec {
     int elem_unit_begin[MAX_PAIR_ELEMS + 1]; // scratch-row ranges per elementary correlator
     int chan_begin, nchan;   // range in Plan::pair_chans
     int swap_mask;           // bit e: some channel needs elementary correlator e with a3 <-> a4 exchanged
+    int self_swap;           // 1: identical sink baryons; computed for q <= -q only, mirrored to -q by the epilogue
 };
 struct PairChanRec {
     int ch, pad;
@@ -114,14 +115,16 @@ struct Plan {
     std::vector<int> baryons; // needed sink baryon ids, slot order
     std::vector<int> chan_pair; // pair index of each channel
     double sumK_std = 0;        // sum over channels of sum_d K_d (the paper's count)
-    double sumK_exec = 0;       // sum over distinct elementary correlators
+    double sumK_exec = 0;       // sum over the computed elementary correlators of pairs of different sink baryons
+    double sumK_exec_self = 0;  // same for pairs of identical sink baryons (executed for about half of the momenta)
     // product kernel tables
     std::vector<Pair3Rec> pairs3;
     std::vector<Unit3Rec> units3;
     std::vector<Diag3Rec> diags3;
     std::vector<uint2x> tab3;
     std::vector<PairChanRec> pair_chans;
-    std::vector<ChainRec> chain;
+    std::vector<ChainRec> chain; // full chain, then the half chain
+    int chain_full_n = 0, chain_half_n = 0;
     int max_pair_units = 0;
     double sumKp_exec = 0; // executed k-steps x 4 (padding included)
 };

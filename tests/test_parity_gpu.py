@@ -273,3 +273,15 @@ def test_full_size_32cubed_52_channels_sparse_support(torch_cuda, nbs, oracle):
     err_off = F.abs().amax(dim=(1, 2)) / scale
     worst = torch.maximum(err_on, err_off)
     assert float(worst.max()) <= RTOL, (int(worst.argmax()), float(err_on.max()), float(err_off.max()))
+
+
+@pytest.mark.parametrize("L", [3, 4])
+def test_identical_sink_baryons_only(torch_cuda, nbs, oracle, L):
+    """Channel lists made of identical-baryon sinks only: the product kernel computes the momenta
+    q <= -q and mirrors them to -q with the sink-swap relation (reading A11); odd L has one
+    self-conjugate momentum, even L eight."""
+    S = props(L, seed=17)
+    chans = [("L", "L", "L", "L"), ("L", "L", "S0", "S0"), ("S0", "S0", "Sp", "Sm"), ("p", "p", "p", "p")]
+    F = run_gpu(torch_cuda, nbs, L, S, chans)
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
