@@ -271,6 +271,72 @@ k_fft_axis_pow2(double2* __restrict__ data, size_t R, int axis, const double2* _
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// x and y transforms of one z-plane in ONE pass over HBM (rows a2 / a5): a CTA stages the L x L
+// sites of a plane for C = 256 / L consecutive components in shared memory (128-byte segments per
+// site at L = 32), runs the L*C x-lines and then the L*C y-lines with the in-register FFT, and
+// writes the plane back -- or, for the last inverse pass (TOUT), straight into the caller's layout
+// out[component][r] with r = x + L (y + L z), 16 KB contiguous per component: the separate
+// transpose pass disappears.  Site stride C + 1 keeps every phase free of bank conflicts.
+// ---------------------------------------------------------------------------------------------
+template <int L>
+constexpr size_t fft_xy_smem_bytes() { return (size_t)L * L * (256 / L + 1) * sizeof(double2); }
+
+template <int L, bool INV, bool TOUT>
+__global__ void __launch_bounds__(256)
+k_fft_xy(double2* __restrict__ data, size_t R, double scale, double2* __restrict__ tout, size_t V) {
+    constexpr int C = 256 / L, CS = C + 1, NS = L * L;
+    extern __shared__ double2 smem[];
+    const size_t r0 = (size_t)blockIdx.x * C;
+    const int z = blockIdx.y, tid = threadIdx.x;
+    const int nc = (int)((R - r0 < (size_t)C) ? (R - r0) : (size_t)C);
+    double2* plane = data + (size_t)z * NS * R + r0;
+    for (int i = tid; i < NS * C; i += 256) {
+        const int site = i / C, c = i % C;
+        if (c < nc) smem[site * CS + c] = plane[(size_t)site * R + c];
+    }
+    __syncthreads();
+    {
+        const int y = tid / C, c = tid % C; // x-lines
+        if (c < nc) {
+            double2 a[L];
+#pragma unroll
+            for (int j = 0; j < L; ++j) a[j] = smem[(y * L + j) * CS + c];
+            fft_inreg<L, INV>(a, nullptr);
+#pragma unroll
+            for (int j = 0; j < L; ++j) smem[(y * L + j) * CS + c] = a[j];
+        }
+    }
+    __syncthreads();
+    {
+        const int x = tid / C, c = tid % C; // y-lines
+        if (c < nc) {
+            double2 a[L];
+#pragma unroll
+            for (int j = 0; j < L; ++j) a[j] = smem[(j * L + x) * CS + c];
+            fft_inreg<L, INV>(a, nullptr);
+#pragma unroll
+            for (int j = 0; j < L; ++j) {
+                double2 v = a[j];
+                if (INV) { v.x *= scale; v.y *= scale; }
+                smem[(j * L + x) * CS + c] = v;
+            }
+        }
+    }
+    __syncthreads();
+    if (TOUT) {
+        for (int i = tid; i < NS * C; i += 256) {
+            const int c = i / NS, site = i % NS;
+            if (c < nc) tout[(r0 + c) * V + (size_t)z * NS + site] = smem[site * CS + c];
+        }
+    } else {
+        for (int i = tid; i < NS * C; i += 256) {
+            const int site = i / C, c = i % C;
+            if (c < nc) plane[(size_t)site * R + c] = smem[site * CS + c];
+        }
+    }
+}
+
 constexpr int FFT_MAXL = 64;
 
 // Any L (direct O(L^2) DFT); used for lattice sizes that are not powers of two.
