@@ -23,7 +23,8 @@ struct Slice {
     int t = -1;
     const double2* S[3] = {nullptr, nullptr, nullptr}; // u, d, s (device)
     double2* own[3] = {nullptr, nullptr, nullptr};     // library-owned copies for host input
-    double2* B = nullptr;  // [V][R] normal blocks, x-space then momentum space (in place)
+    double2* B = nullptr;  // [V][R] normal blocks, compact rows, x-space then momentum space (in place)
+    double2* Be = nullptr; // [V][Re] antisymmetric blocks expanded to full staged blocks (momentum space)
     double2* Ft = nullptr; // [V][nch][256]
     double2* scratch = nullptr;            // [grid][PROD_NBUF][max_pair_units][256] unit results
     unsigned long long* counter = nullptr; // work-item counter of the persistent product kernel
@@ -40,7 +41,8 @@ struct nbs_ctx {
     size_t workspace = 0;
     int nslices = 0;
     Slice slice[NSLOTS_MAX];
-    size_t R = 0; // block row length (complex) = nbaryons * SM_BLOCK (staged layout, nbs_tables.hpp)
+    size_t R = 0;  // compact block row length (complex): Plan::row_elems (nbs_tables.hpp)
+    size_t Re = 0; // expanded row length: n_asym * SM_BLOCK
     // device tables
     Pair3Rec* d_pairs3 = nullptr;
     Unit3Rec* d_units3 = nullptr;
@@ -54,6 +56,10 @@ struct nbs_ctx {
     long long nselfconj = 0; // momenta with q == -q
     int* d_baryon_of_slot = nullptr;
     int* d_one_baryon = nullptr; // scratch for nbs_blocks_x
+    int2* d_slot_info = nullptr;     // (row offset, block kind) of every slot
+    int* d_gather = nullptr;         // expansion map of the antisymmetric slots
+    int2x* d_slot_src = nullptr;     // where the product kernel stages every slot from
+    int2* d_one_slot_info = nullptr; // the same for a single baryon (nbs_blocks_x)
     BlockRec* d_brec = nullptr;
     BTermRec* d_bterm = nullptr;
     double2* d_tw = nullptr;
@@ -182,12 +188,12 @@ int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st, do
     return NBS_OK;
 }
 
-int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, int nslots, unsigned dq_mask, double2* out,
-                  size_t row_stride, cudaStream_t st) {
+int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, const int2* d_info, int nslots, unsigned dq_mask,
+                  double2* out, size_t row_stride, cudaStream_t st) {
     int ndq = 0;
     for (int b = 0; b < 9; ++b) ndq += (dq_mask >> b) & 1u;
     k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, blocks_smem_bytes(ndq), st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask,
-                                                                          c->d_brec, c->d_bterm, out, row_stride);
+                                                                          c->d_brec, c->d_bterm, d_info, out, row_stride);
     CU(c, cudaGetLastError());
     ++c->launches;
     return NBS_OK;
@@ -228,7 +234,8 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     if (!err.empty()) { delete c; return fail(nullptr, NBS_EINVAL, err); }
     c->L = L; c->T = T; c->device = device;
     c->V = (size_t)L * L * L;
-    c->R = c->plan.baryons.size() * (size_t)SM_BLOCK;
+    c->R = (size_t)c->plan.row_elems;
+    c->Re = (size_t)c->plan.n_asym * SM_BLOCK;
 
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -315,6 +322,15 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         for (int b = 0; b < NBS_NUM_BARYONS; ++b) ids[b] = b;
         CUX(cudaMemcpy(c->d_one_baryon, ids.data(), ids.size() * sizeof(int), cudaMemcpyHostToDevice));
     }
+    {
+        std::vector<int2> info, one;
+        for (size_t i = 0; i < c->plan.baryons.size(); ++i) info.push_back(make_int2(c->plan.slot_off[i], c->plan.slot_kind[i]));
+        for (int b = 0; b < NBS_NUM_BARYONS; ++b) one.push_back(make_int2(0, block_kind(b)));
+        CUC(upload(c, c->d_slot_info, info));
+        CUC(upload(c, c->d_gather, c->plan.gather));
+        CUC(upload(c, c->d_slot_src, c->plan.slot_src));
+        CUC(upload(c, c->d_one_slot_info, one));
+    }
     CUC(upload(c, c->d_brec, brec));
     CUC(upload(c, c->d_bterm, bterm));
     CUC(upload(c, c->d_tw, tw));
@@ -322,7 +338,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     // workspace: per slice in flight, blocks + elementary correlators + channel correlators
     size_t nchan = c->plan.channels.size();
     size_t scratch_elems = (size_t)c->prod_grid * PROD_NBUF * c->plan.max_pair_units * 256;
-    size_t per_slice = (c->V * (c->R + nchan * 256) + scratch_elems) * sizeof(double2);
+    size_t per_slice = (c->V * (c->R + c->Re + nchan * 256) + scratch_elems) * sizeof(double2);
     size_t free_b = 0, total_b = 0;
     CUX(cudaMemGetInfo(&free_b, &total_b));
     size_t avail = (size_t)(0.92 * (double)free_b);
@@ -336,6 +352,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     }
     for (int i = 0; i < c->nslices; ++i) {
         CUC(dev_alloc(c, c->slice[i].B, c->V * c->R));
+        CUC(dev_alloc(c, c->slice[i].Be, std::max<size_t>(c->V * c->Re, 1)));
         CUC(dev_alloc(c, c->slice[i].Ft, c->V * nchan * 256));
         CUC(dev_alloc(c, c->slice[i].scratch, scratch_elems));
         double2* cnt = nullptr;
@@ -394,11 +411,13 @@ int nbs_blocks_x(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes,
     // the kernel writes the staged layout; convert to [site][alpha][xi1][xi2][xi3] for the caller
     cudaStream_t st = (cudaStream_t)stream;
     double2* tmp = nullptr;
-    CU(c, cudaMalloc((void**)&tmp, c->V * (size_t)SM_BLOCK * sizeof(double2)));
-    int rc = launch_blocks(c, sl, c->d_one_baryon + baryon, 1, c->dq_mask_of[baryon], tmp, SM_BLOCK, st);
+    const int kind = block_kind(baryon);
+    CU(c, cudaMalloc((void**)&tmp, c->V * (size_t)block_elems(kind) * sizeof(double2)));
+    int rc = launch_blocks(c, sl, c->d_one_baryon + baryon, c->d_one_slot_info + baryon, 1, c->dq_mask_of[baryon], tmp,
+                           (size_t)block_elems(kind), st);
     if (rc == NBS_OK) {
         const size_t n = c->V * (size_t)BLOCK_ELEMS;
-        k_unstage<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(tmp, c->V, (double2*)out_dev);
+        k_unstage<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(tmp, c->V, kind, (double2*)out_dev);
         ++c->launches;
         cudaError_t e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(c, e, "nbs_blocks_x"); }
@@ -426,20 +445,26 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     int rc;
     {
         StageTimer tm(c, NBS_STAGE_BLOCKS, st);
-        rc = launch_blocks(c, sl, c->d_baryon_of_slot, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
+        rc = launch_blocks(c, sl, c->d_baryon_of_slot, c->d_slot_info, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
         if (rc) return rc;
     }
     {
         StageTimer tm(c, NBS_STAGE_FFT_FWD, st);
         rc = fft3d(c, sl.B, c->R, false, st);
         if (rc) return rc;
+        if (c->Re) { // antisymmetric blocks: mirror halves restored for the gathers of the product kernel
+            k_expand<<<(unsigned)c->V, 256, 0, st>>>(sl.B, c->R, c->d_gather, (int)c->Re, sl.Be);
+            CU(c, cudaGetLastError());
+            ++c->launches;
+        }
     }
     // (ii)+(iii) effective blocks and their products -> elementary correlators -> channels
     {
         StageTimer tm(c, NBS_STAGE_PRODUCT, st);
         CU(c, cudaMemsetAsync(sl.counter, 0, sizeof(unsigned long long), st));
         ProdArgs pa;
-        pa.Bq = sl.B; pa.R = c->R; pa.L = c->L;
+        pa.Bc = sl.B; pa.Rc = c->R; pa.Be = sl.Be; pa.Re = c->Re; pa.L = c->L;
+        pa.slot_src = reinterpret_cast<const int2*>(c->d_slot_src);
         pa.chain_full_n = c->plan.chain_full_n; pa.chain_half_n = c->plan.chain_half_n;
         pa.ntasks = c->ntasks;
         pa.qorder = c->d_qorder;
@@ -456,7 +481,11 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     }
     // inverse FFT and final layout F[ch][a1 a2 a3 a4][r]
     double2* dst = (double2*)out;
-    if (memloc == NBS_MEM_HOST) dst = sl.B; // the block buffer is free again: device staging for the host copy
+    if (memloc == NBS_MEM_HOST) { // a block buffer is free again: device staging for the host copy
+        if (need <= c->V * c->R * sizeof(double2)) dst = sl.B;
+        else if (need <= c->V * c->Re * sizeof(double2)) dst = sl.Be;
+        else return fail(c, NBS_ENOMEM, "channel range too large for the device staging of a host output; use a smaller range");
+    }
     const bool fused = fft_fused(c);
     {
         StageTimer tm(c, NBS_STAGE_FFT_INV, st);

@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(BLOCKS_THREADS, 2)
 k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const double2* __restrict__ Ss,
          const int* __restrict__ baryon_of_slot, int nslots, unsigned dq_mask,
          const BlockRec* __restrict__ brec, const BTermRec* __restrict__ bterm,
-         double2* __restrict__ out, size_t row_stride) {
+         const int2* __restrict__ slot_info, double2* __restrict__ out, size_t row_stride) {
     extern __shared__ double2 smem[];
     const int ndq = __popc(dq_mask);
     double2* sS = smem;                  // [3][144]
@@ -129,16 +129,36 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
         }
         sD[idx] = csub(acc, neg);
     }
-    // pads of the half-row buffer stay zero for the whole kernel
-    if (tid < 24) sO[(tid / 12) * SM_PLANE + (tid % 12) * SM_STRIDE1 + 144] = make_double2(0.0, 0.0);
     __syncthreads();
 
-    const int x[3] = {2 * (tid / 36), 2 * ((tid / 6) % 6), 2 * (tid % 6)}; // tile origin (tid < 216)
     double2* orow = out + site * row_stride;
     for (int slot = 0; slot < nslots; ++slot) {
         const BlockRec br = brec[baryon_of_slot[slot]];
-        for (int half = 0; half < 2; ++half) {
-            if (tid < BLOCKS_TILES) {
+        const int2 info = slot_info[slot]; // (offset inside the site row, block kind)
+        const int kind = info.y;
+        // full blocks: two passes of 2 sink spins, 216 tiles each; antisymmetric blocks (nbs_tables.hpp):
+        // one pass, 2 x 126 tiles on or above the diagonal of the antisymmetric slot pair
+        const int npass = (kind == BK_FULL) ? 2 : 1;
+        for (int pass = 0; pass < npass; ++pass) {
+            int x[3], a0 = 2 * pass;
+            bool active;
+            if (kind == BK_FULL) {
+                active = tid < BLOCKS_TILES;
+                x[0] = 2 * (tid / 36); x[1] = 2 * ((tid / 6) % 6); x[2] = 2 * (tid % 6);
+                if (tid < 24) sO[(tid / 12) * SM_PLANE + (tid % 12) * SM_STRIDE1 + 144] = make_double2(0.0, 0.0);
+            } else {
+                active = tid < 252;
+                const int h = tid / 126, tt = tid - h * 126;
+                int ia = 0, rem = tt / 6;
+                while (rem >= 6 - ia) { rem -= 6 - ia; ++ia; }
+                const int ib = ia + rem, ic = tt % 6;
+                a0 = 2 * h;
+                x[2] = 2 * ib;
+                if (kind == BK_ASYM13) { x[0] = 2 * ia; x[1] = 2 * ic; }
+                else { x[1] = 2 * ia; x[0] = 2 * ic; }
+                if (tid < 48) sO[(tid / 12) * AS_PLANE + (tid % 12) * AS_ROW + 66] = make_double2(0.0, 0.0);
+            }
+            if (active) {
                 double2 acc[2][2][2][2];
 #pragma unroll
                 for (int i = 0; i < 16; ++i) (&acc[0][0][0][0])[i] = make_double2(0.0, 0.0);
@@ -148,12 +168,12 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                     const double2* S2 = sS + bt.f2 * 144;
                     const int perm = bt.p0 * 3 + bt.p1; // (p0, p1) fixes the permutation
                     switch (perm) {
-                    case 1: blocks_term<0, 1, 2>(acc, Dq, S2, bt.coef, 2 * half, x); break;
-                    case 2: blocks_term<0, 2, 1>(acc, Dq, S2, bt.coef, 2 * half, x); break;
-                    case 3: blocks_term<1, 0, 2>(acc, Dq, S2, bt.coef, 2 * half, x); break;
-                    case 5: blocks_term<1, 2, 0>(acc, Dq, S2, bt.coef, 2 * half, x); break;
-                    case 6: blocks_term<2, 0, 1>(acc, Dq, S2, bt.coef, 2 * half, x); break;
-                    default: blocks_term<2, 1, 0>(acc, Dq, S2, bt.coef, 2 * half, x); break;
+                    case 1: blocks_term<0, 1, 2>(acc, Dq, S2, bt.coef, a0, x); break;
+                    case 2: blocks_term<0, 2, 1>(acc, Dq, S2, bt.coef, a0, x); break;
+                    case 3: blocks_term<1, 0, 2>(acc, Dq, S2, bt.coef, a0, x); break;
+                    case 5: blocks_term<1, 2, 0>(acc, Dq, S2, bt.coef, a0, x); break;
+                    case 6: blocks_term<2, 0, 1>(acc, Dq, S2, bt.coef, a0, x); break;
+                    default: blocks_term<2, 1, 0>(acc, Dq, S2, bt.coef, a0, x); break;
                     }
                 }
 #pragma unroll
@@ -163,26 +183,55 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
 #pragma unroll
                         for (int e1 = 0; e1 < 2; ++e1)
 #pragma unroll
-                            for (int e2 = 0; e2 < 2; ++e2)
-                                sO[a * SM_PLANE + sm_index(x[0] + e0, x[1] + e1, x[2] + e2)] = acc[a][e0][e1][e2];
+                            for (int e2 = 0; e2 < 2; ++e2) {
+                                const int xi0 = x[0] + e0, xi1 = x[1] + e1, xi2 = x[2] + e2;
+                                if (kind == BK_FULL) {
+                                    sO[a * SM_PLANE + sm_index(xi0, xi1, xi2)] = acc[a][e0][e1][e2];
+                                } else {
+                                    const int xa = (kind == BK_ASYM13) ? xi0 : xi1, xc = (kind == BK_ASYM13) ? xi1 : xi0;
+                                    if (xa < xi2) sO[(a0 + a) * AS_PLANE + xc * AS_ROW + as_pair_index(xa, xi2)] = acc[a][e0][e1][e2];
+                                }
+                            }
             }
             __syncthreads();
-            double2* dst = orow + (size_t)slot * SM_BLOCK + half * BLOCKS_HALF;
-            for (int i = tid; i < BLOCKS_HALF; i += BLOCKS_THREADS) dst[i] = sO[i];
+            const int n = (kind == BK_FULL) ? BLOCKS_HALF : AS_BLOCK;
+            double2* dst = orow + info.x + ((kind == BK_FULL) ? pass * BLOCKS_HALF : 0);
+            for (int i = tid; i < n; i += BLOCKS_THREADS) dst[i] = sO[i];
             __syncthreads();
         }
     }
 }
 
-// Staged block rows [site][SM_BLOCK] -> [site][alpha][xi1][xi2][xi3] (nbs_blocks_x, tests only).
+// Expansion of the antisymmetric blocks after the forward FFT: compact rows [site][Rc] -> full staged
+// blocks [site][Re] (Plan::gather): mirror entries with the sign flipped, pads and diagonal zero.
+// Writes are fully coalesced; every compact element is read twice (through L2).
 __global__ void __launch_bounds__(256)
-k_unstage(const double2* __restrict__ in, size_t V, double2* __restrict__ out) {
+k_expand(const double2* __restrict__ compact, size_t Rc, const int* __restrict__ gather, int Re, double2* __restrict__ full) {
+    const double2* src = compact + (size_t)blockIdx.x * Rc;
+    double2* dst = full + (size_t)blockIdx.x * Re;
+    for (int j = threadIdx.x; j < Re; j += 256) {
+        const int g = __ldg(gather + j);
+        double2 v = make_double2(0.0, 0.0);
+        if (g >= 0) {
+            v = src[g & 0x3fffffff];
+            if (g & (1 << 30)) { v.x = -v.x; v.y = -v.y; }
+        }
+        dst[j] = v;
+    }
+}
+
+// Staged block rows [site][block of `kind`] -> [site][alpha][xi1][xi2][xi3] (nbs_blocks_x, tests only):
+// mirrored entries of an antisymmetric block are reconstructed with their sign.
+__global__ void __launch_bounds__(256)
+k_unstage(const double2* __restrict__ in, size_t V, int kind, double2* __restrict__ out) {
     const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
     if (idx >= V * BLOCK_ELEMS) return;
     const size_t site = idx / BLOCK_ELEMS;
     const int rem = (int)(idx - site * BLOCK_ELEMS);
     const int al = rem / NTRIPLE, t = rem - al * NTRIPLE;
-    out[idx] = in[site * SM_BLOCK + al * SM_PLANE + sm_index(t / 144, (t / 12) % 12, t % 12)];
+    const Located loc = locate(kind, t / 144, (t / 12) % 12, t % 12);
+    const double2 v = in[site * block_elems(kind) + al * plane_elems(kind) + loc.idx];
+    out[idx] = loc.sign > 0 ? v : make_double2(-v.x, -v.y);
 }
 
 // ---------------------------------------------------------------------------------------------

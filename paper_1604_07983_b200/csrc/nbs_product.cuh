@@ -297,8 +297,14 @@ __device__ __forceinline__ void run_unit_wide(const Unit3Rec u, const Diag3Rec* 
 }
 
 struct ProdArgs {
-    const double2* Bq;   // [V][R] momentum-space normal blocks, every (site, slot) row in the staged layout
-    size_t R;            // row length (complex) = nslots * SM_BLOCK
+    // momentum-space normal blocks as full staged blocks: slot s is staged from buffer slot_src[s].x
+    // (0: compact rows Bc[V][Rc], where the blocks without an antisymmetry are stored staged; 1: expanded
+    // rows Be[V][Re] of the antisymmetric blocks) at complex offset slot_src[s].y inside the site row
+    const double2* Bc;
+    size_t Rc;
+    const double2* Be;
+    size_t Re;
+    const int2* slot_src;
     int L;
     int chain_full_n, chain_half_n; // chain[0 .. full_n): all pairs (momenta q <= -q); then the half chain
     long long ntasks;    // momentum tasks = entries of qorder
@@ -512,12 +518,14 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             bulk_g2s(s_units, usrc, ubytes, rbar);
             bulk_g2s(s_diags, dsrc, dbytes, rbar);
             if (load1) {
-                const char* g1 = reinterpret_cast<const char*>(a.Bq + q * a.R + (size_t)__ldg(&pr->slot1) * SM_BLOCK);
+                const int2 src = __ldg(a.slot_src + __ldg(&pr->slot1));
+                const char* g1 = reinterpret_cast<const char*>((src.x ? a.Be + q * a.Re : a.Bc + q * a.Rc) + src.y);
 #pragma unroll
                 for (int p = 0; p < 4; ++p) bulk_g2s(s1 + p * PLANE_BYTES, g1 + p * PLANE_BYTES, PLANE_BYTES, mbar1);
             }
             if (load2) {
-                const char* g2 = reinterpret_cast<const char*>(a.Bq + mq * a.R + (size_t)__ldg(&pr->slot2) * SM_BLOCK);
+                const int2 src = __ldg(a.slot_src + __ldg(&pr->slot2));
+                const char* g2 = reinterpret_cast<const char*>((src.x ? a.Be + mq * a.Re : a.Bc + mq * a.Rc) + src.y);
 #pragma unroll
                 for (int p = 0; p < 4; ++p) bulk_g2s(s2 + p * PLANE_BYTES, g2 + p * PLANE_BYTES, PLANE_BYTES, mbar2);
             }

@@ -244,6 +244,13 @@ int diagram_K(const int* P) {
 
 const BaryonDef& baryon_def(int id) { return kBaryons[id]; }
 
+int block_kind(int baryon) {
+    const BaryonDef& B = kBaryons[baryon];
+    if (B.slot[0] == B.slot[2]) return BK_ASYM13;
+    if (B.slot[1] == B.slot[2]) return BK_ASYM23;
+    return BK_FULL;
+}
+
 std::vector<BlockTerm> block_terms(int baryon) {
     const BaryonDef& B = kBaryons[baryon];
     std::vector<BlockTerm> out;
@@ -371,6 +378,29 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             const bool derived = ks != k && pair_elems[ip].count(ks) && ks < k;
             if (!derived) pair_comp_order[ip].push_back(k);
         }
+
+    // compact site row; expansion map of the antisymmetric slots into full staged blocks
+    for (size_t sl = 0; sl < plan.baryons.size(); ++sl) {
+        const int kind = block_kind(plan.baryons[sl]);
+        const int base = plan.row_elems;
+        plan.slot_off.push_back(base);
+        plan.slot_kind.push_back(kind);
+        plan.row_elems += block_elems(kind);
+        if (kind == BK_FULL) { plan.slot_src.push_back(int2x{0, base}); continue; }
+        const int ebase = plan.n_asym * SM_BLOCK;
+        plan.slot_src.push_back(int2x{1, ebase});
+        ++plan.n_asym;
+        plan.gather.resize(ebase + SM_BLOCK, -1);
+        for (int al = 0; al < 4; ++al)
+            for (int x1 = 0; x1 < NXI; ++x1)
+                for (int x2 = 0; x2 < NXI; ++x2)
+                    for (int x3 = 0; x3 < NXI; ++x3) {
+                        if ((kind == BK_ASYM13 ? x1 : x2) == x3) continue; // diagonal: zero
+                        const Located loc = locate(kind, x1, x2, x3);
+                        const int src = base + al * AS_PLANE + loc.idx;
+                        plan.gather[ebase + al * SM_PLANE + sm_index(x1, x2, x3)] = src | (loc.sign < 0 ? (1 << 30) : 0);
+                    }
+    }
 
     // ---- product kernel tables: pairs -> (<= MAX_PAIR_ELEMS elementary correlators) -> units -> diagrams
     // layout: 0 = 16x16 side, 1 = 64x4 A side, 2 = 64x4 B side (see nbs_tables.hpp)

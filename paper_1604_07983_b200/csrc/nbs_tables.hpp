@@ -29,6 +29,33 @@ constexpr int SM_BLOCK = 4 * SM_PLANE;     // 6960 complex per staged block
 #endif
 NBS_HD constexpr int sm_index(int xi1, int xi2, int xi3) { return xi1 * SM_STRIDE1 + xi2 * 12 + (xi3 + xi2) % 12; }
 
+// Blocks of baryons with two quarks of one flavour are antisymmetric under the exchange of those
+// two source slots (the Wick sign of exchanging the two identical quark fields): p, Sigma+, Sigma-
+// in slots (1,3), n, Xi0, Xi- in slots (2,3).  Only the entries with xi_a < xi_b are built and
+// Fourier transformed (66 of 144 index pairs; 46 % of the data), in the "compact" layout
+//   antisymmetric plane: [xi_c (free slot): 12][pair (xi_a < xi_b): 66, then one pad]  (row 67);
+// after the transform they are expanded (mirror entries with the sign flipped, diagonal zero) into
+// the full staged layout the product kernel gathers from.
+enum { BK_FULL = 0, BK_ASYM13 = 1, BK_ASYM23 = 2 };
+constexpr int AS_ROW = 67;
+constexpr int AS_PLANE = 12 * AS_ROW;  // 804
+constexpr int AS_BLOCK = 4 * AS_PLANE; // 3216 complex per compact antisymmetric block
+NBS_HD constexpr int as_pair_index(int a, int b) { return a * (23 - a) / 2 + (b - a - 1); } // a < b
+NBS_HD constexpr int plane_elems(int kind) { return kind == BK_FULL ? SM_PLANE : AS_PLANE; }
+NBS_HD constexpr int block_elems(int kind) { return 4 * plane_elems(kind); }
+struct Located {
+    int idx;  // position inside the sink-spin plane of the compact layout
+    int sign; // +1, or -1 if the stored partner carries the opposite sign
+};
+NBS_HD constexpr Located locate(int kind, int xi1, int xi2, int xi3) {
+    if (kind == BK_FULL) return Located{sm_index(xi1, xi2, xi3), 1};
+    const int a = (kind == BK_ASYM13) ? xi1 : xi2, b = xi3, c = (kind == BK_ASYM13) ? xi2 : xi1;
+    if (a == b) return Located{c * AS_ROW + 66, 1}; // identically zero (the pad)
+    if (a < b) return Located{c * AS_ROW + as_pair_index(a, b), 1};
+    return Located{c * AS_ROW + as_pair_index(b, a), -1};
+}
+int block_kind(int baryon); // from the slot flavours of eqs. 2.2-2.3
+
 // One elementary operator  eps_abc (q_f0,a  C g5  q_f1,b) q_f2,c  with a real coefficient
 // (eqs. 2.2-2.3).  Flavours: 0 = u, 1 = d, 2 = s.
 struct ElemTerm {
@@ -103,6 +130,7 @@ struct ChainRec { // order in which one CTA walks the sink pairs of one momentum
 };
 
 struct uint2x { uint32_t x, y; }; // host mirror of CUDA uint2
+struct int2x { int x, y; };
 
 struct DiagramInfo { // host-side description (tests, statistics)
     int P[6];
@@ -113,6 +141,17 @@ struct DiagramInfo { // host-side description (tests, statistics)
 struct Plan {
     std::vector<nbs_channel> channels;
     std::vector<int> baryons; // needed sink baryon ids, slot order
+    // compact site row (what k_blocks writes and the FFT transforms): every slot's block in the layout of its kind
+    std::vector<int> slot_off, slot_kind;
+    int row_elems = 0;
+    // Antisymmetric slots are expanded after the FFT into a second buffer of full staged blocks
+    // (row = n_asym * SM_BLOCK): expanded element j takes compact element gather[j] & 0x3fffffff of the
+    // same site, negated if bit 30 is set; -1 = zero (pads and the diagonal xi_a == xi_b).
+    std::vector<int> gather;
+    int n_asym = 0;
+    // where the product kernel stages slot s from: slot_src[s].x = 0: compact row at offset .y (full
+    // kinds are already staged blocks there); 1: expanded row at offset .y
+    std::vector<int2x> slot_src;
     std::vector<int> chan_pair; // pair index of each channel
     double sumK_std = 0;        // sum over channels of sum_d K_d (the paper's count)
     double sumK_exec = 0;       // sum over the computed elementary correlators of pairs of different sink baryons
