@@ -44,7 +44,7 @@ constexpr uint32_t EPI_PAIR_BYTES = (sizeof(Pair3Rec) + 15u) / 16u * 16u;
 constexpr uint32_t SMO_CTRL = SMO_EPI + EPI_PAIR_BYTES + EPI_CG * (uint32_t)sizeof(PairChanRec) + 8u;
 constexpr int PROD_NBUF = 4; // depth of the unit-result ring between compute and epilogue warps
 constexpr size_t PROD_SMEM = SMO_CTRL + 128;
-static_assert(sizeof(Unit3Rec) == 16 && sizeof(Diag3Rec) == 16, "record sizes");
+static_assert(sizeof(Unit3Rec) == 16 && sizeof(Diag3Rec) == 16 && sizeof(ChainRec) == 48, "record sizes");
 static_assert(PROD_SMEM <= 232448, "shared memory budget of one SM");
 
 struct ProdCtrl { // at SMO_CTRL
@@ -478,6 +478,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
     long long qt = 0;
     size_t q = 0, mq = 0;
     int cbase = 0, clen = 1;
+    int4 nh0 = make_int4(0, 0, 0, 0), nh1 = nh0, nh2 = nh0; // next chain record
     for (unsigned it = 0;; ++it) {
         const int b = it % PROD_NBUF;
         named_sync(BAR_COMPUTE, PROD_CTHREADS); // the staged blocks and unit records of the previous item are consumed
@@ -498,38 +499,39 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             named_arrive(BAR_FULL0 + b, PROD_THREADS);
             break;
         }
-        const int ip = __ldg(&a.chain[cbase + pos].pair);
-        const int load1 = __ldg(&a.chain[cbase + pos].load1), load2 = __ldg(&a.chain[cbase + pos].load2);
+        // chain record of this item (prefetched during the previous item of the same momentum task)
+        const int4* crec = reinterpret_cast<const int4*>(a.chain + cbase + pos);
+        const int4 h0 = (pos > 0) ? nh0 : __ldg(crec);
+        const int ip = h0.x, load1 = h0.y, load2 = h0.z, nunits = h0.w;
         const Pair3Rec* pr = a.pairs + ip;
-        const int nunits = __ldg(&pr->nunits);
         if (tid == 0) {
-            if (pos == 0) ctl->qtask[(ntask + 1) & 1] = (long long)atomicAdd(a.counter, 1ull); // next momentum task
+            const int4 h1 = (pos > 0) ? nh1 : __ldg(crec + 1); // unit_begin, ndiags, diag_begin
+            const int4 h2 = (pos > 0) ? nh2 : __ldg(crec + 2); // buf1, off1, buf2, off2
             *next_unit = 0;
             ctl->meta_q[b] = (int)q;
             ctl->meta_pair[b] = ip;
             // unit and diagram records of the pair ride on the first staging barrier of the item
             const uint32_t ubytes = (uint32_t)nunits * (uint32_t)sizeof(Unit3Rec);
-            const uint32_t dbytes = (uint32_t)__ldg(&pr->ndiags) * (uint32_t)sizeof(Diag3Rec);
-            const Unit3Rec* usrc = a.units + __ldg(&pr->unit_begin);
-            const Diag3Rec* dsrc = a.diags + __ldg(&pr->diag_begin);
+            const uint32_t dbytes = (uint32_t)h1.y * (uint32_t)sizeof(Diag3Rec);
             void* rbar = load1 ? mbar1 : mbar2;
             if (load1) mbar_expect_tx(mbar1, BLOCK_BYTES + ubytes + dbytes);
             if (load2) mbar_expect_tx(mbar2, BLOCK_BYTES + (load1 ? 0u : ubytes + dbytes));
-            bulk_g2s(s_units, usrc, ubytes, rbar);
-            bulk_g2s(s_diags, dsrc, dbytes, rbar);
             if (load1) {
-                const int2 src = __ldg(a.slot_src + __ldg(&pr->slot1));
-                const char* g1 = reinterpret_cast<const char*>((src.x ? a.Be + q * a.Re : a.Bc + q * a.Rc) + src.y);
+                const char* g1 = reinterpret_cast<const char*>((h2.x ? a.Be + q * a.Re : a.Bc + q * a.Rc) + h2.y);
 #pragma unroll
                 for (int p = 0; p < 4; ++p) bulk_g2s(s1 + p * PLANE_BYTES, g1 + p * PLANE_BYTES, PLANE_BYTES, mbar1);
             }
             if (load2) {
-                const int2 src = __ldg(a.slot_src + __ldg(&pr->slot2));
-                const char* g2 = reinterpret_cast<const char*>((src.x ? a.Be + mq * a.Re : a.Bc + mq * a.Rc) + src.y);
+                const char* g2 = reinterpret_cast<const char*>((h2.z ? a.Be + mq * a.Re : a.Bc + mq * a.Rc) + h2.w);
 #pragma unroll
                 for (int p = 0; p < 4; ++p) bulk_g2s(s2 + p * PLANE_BYTES, g2 + p * PLANE_BYTES, PLANE_BYTES, mbar2);
             }
+            bulk_g2s(s_units, a.units + h1.x, ubytes, rbar);
+            bulk_g2s(s_diags, a.diags + h1.z, dbytes, rbar);
+            if (pos == 0) ctl->qtask[(ntask + 1) & 1] = (long long)atomicAdd(a.counter, 1ull); // next momentum task
+            if (pos + 1 < clen) { nh1 = __ldg(crec + 4); nh2 = __ldg(crec + 5); }
         }
+        if (pos + 1 < clen) nh0 = __ldg(crec + 3);
         if (load1) { mbar_wait(mbar1, ph1); ph1 ^= 1u; }
         if (load2) { mbar_wait(mbar2, ph2); ph2 ^= 1u; }
         double2* scr = scr0 + b * scr_stride;

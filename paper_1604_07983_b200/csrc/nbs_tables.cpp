@@ -584,6 +584,10 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             cr.pair = ids[best[s]];
             cr.load1 = (s == 0) || plan.pairs3[cr.pair].slot1 != plan.pairs3[ids[best[s - 1]]].slot1;
             cr.load2 = (s == 0) || plan.pairs3[cr.pair].slot2 != plan.pairs3[ids[best[s - 1]]].slot2;
+            const Pair3Rec& pr = plan.pairs3[cr.pair];
+            cr.nunits = pr.nunits; cr.unit_begin = pr.unit_begin; cr.ndiags = pr.ndiags; cr.diag_begin = pr.diag_begin; cr.pad = 0;
+            cr.buf1 = plan.slot_src[pr.slot1].x; cr.off1 = plan.slot_src[pr.slot1].y;
+            cr.buf2 = plan.slot_src[pr.slot2].x; cr.off2 = plan.slot_src[pr.slot2].y;
             plan.chain.push_back(cr);
         }
     };

@@ -124,9 +124,12 @@ struct PairChanRec {
     double coef[MAX_PAIR_ELEMS];  // channel = sum_e coef[e] * E_e + coefS[e] * (E_e with a3 <-> a4), eqs. 2.2-2.3;
     double coefS[MAX_PAIR_ELEMS]; // coefS carries the minus sign of the source swap (reading A11)
 };
-struct ChainRec { // order in which one CTA walks the sink pairs of one momentum q
+struct ChainRec { // order in which one CTA walks the sink pairs of one momentum; self-contained staging descriptor
     int pair;
     int load1, load2; // 1: this item must (re)load B~1(q) / B~2(-q); 0: the staged block is reused
+    int nunits;
+    int unit_begin, ndiags, diag_begin, pad;
+    int buf1, off1, buf2, off2; // Plan::slot_src of the two blocks
 };
 
 struct uint2x { uint32_t x, y; }; // host mirror of CUDA uint2
