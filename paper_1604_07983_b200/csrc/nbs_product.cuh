@@ -503,7 +503,6 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         const int4* crec = reinterpret_cast<const int4*>(a.chain + cbase + pos);
         const int4 h0 = (pos > 0) ? nh0 : __ldg(crec);
         const int ip = h0.x, load1 = h0.y, load2 = h0.z, nunits = h0.w;
-        const Pair3Rec* pr = a.pairs + ip;
         if (tid == 0) {
             const int4 h1 = (pos > 0) ? nh1 : __ldg(crec + 1); // unit_begin, ndiags, diag_begin
             const int4 h2 = (pos > 0) ? nh2 : __ldg(crec + 2); // buf1, off1, buf2, off2
