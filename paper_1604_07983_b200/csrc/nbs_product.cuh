@@ -432,6 +432,20 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
     }
 }
 
+// L1 prefetch of the head (8 lines each) of the two gather tables of a unit's first diagram record.
+__device__ __forceinline__ void prefetch_unit(const Unit3Rec* urec, const Diag3Rec* drecs, const uint2* __restrict__ tab,
+                                              int lane) {
+    if (lane < 16) {
+        const int4 uv = *reinterpret_cast<const int4*>(urec);
+        const int4 dv = *reinterpret_cast<const int4*>(drecs + uv.x);
+        const uint32_t sbeg = (uint32_t)dv.z & 0xffffu, nwA = (uint32_t)dv.w & 0xffu, nwB = ((uint32_t)dv.w >> 8) & 0xffu;
+        const bool wide = uv.z >= 2;
+        const uint32_t off = (lane < 8) ? (uint32_t)dv.x + sbeg * (wide ? 128u : 32u * nwA)
+                                        : (uint32_t)dv.y + sbeg * (wide ? 64u : 32u * nwB);
+        prefetch_l1(reinterpret_cast<const char*>(tab + off) + (lane & 7) * 128);
+    }
+}
+
 __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
     extern __shared__ __align__(128) char prod_smem[];
     char* smem = prod_smem;
@@ -503,8 +517,8 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         const int4* crec = reinterpret_cast<const int4*>(a.chain + cbase + pos);
         const int4 h0 = (pos > 0) ? nh0 : __ldg(crec);
         const int ip = h0.x, load1 = h0.y, load2 = h0.z, nunits = h0.w;
+        const int4 h1 = (pos > 0) ? nh1 : __ldg(crec + 1); // unit_begin, ndiags, diag_begin
         if (tid == 0) {
-            const int4 h1 = (pos > 0) ? nh1 : __ldg(crec + 1); // unit_begin, ndiags, diag_begin
             const int4 h2 = (pos > 0) ? nh2 : __ldg(crec + 2); // buf1, off1, buf2, off2
             *next_unit = 0;
             ctl->meta_q[b] = (int)q;
@@ -528,14 +542,17 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             bulk_g2s(s_units, a.units + h1.x, ubytes, rbar);
             bulk_g2s(s_diags, a.diags + h1.z, dbytes, rbar);
             if (pos == 0) ctl->qtask[(ntask + 1) & 1] = (long long)atomicAdd(a.counter, 1ull); // next momentum task
-            if (pos + 1 < clen) { nh1 = __ldg(crec + 4); nh2 = __ldg(crec + 5); }
+            if (pos + 1 < clen) nh2 = __ldg(crec + 5);
         }
-        if (pos + 1 < clen) nh0 = __ldg(crec + 3);
+        if (pos + 1 < clen) { nh0 = __ldg(crec + 3); nh1 = __ldg(crec + 4); }
+        // while the copies fly: table heads of the unit this warp will probably start with
+        if ((tid >> 5) < nunits) prefetch_unit(a.units + h1.x + (tid >> 5), a.diags + h1.z, a.tab, lane);
         if (load1) { mbar_wait(mbar1, ph1); ph1 ^= 1u; }
         if (load2) { mbar_wait(mbar2, ph2); ph2 ^= 1u; }
         double2* scr = scr0 + b * scr_stride;
-        // Units are taken one ahead: while unit i runs, the head of the gather tables of the warp's
-        // next unit is pulled into L1 (table words are the first link of every gather chain).
+        // Table words are the first link of every gather chain and come from L2: the head of the
+        // tables of the unit this warp will probably take next (i + number of compute warps) is pulled
+        // into L1 while unit i runs -- a hint only, units are still taken from the counter when needed.
         auto grab = [&]() {
             int i = 0;
             if (lane == 0) i = atomicAdd(next_unit, 1);
@@ -546,20 +563,11 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             const int4 uv = *reinterpret_cast<const int4*>(s_units + i);
             Unit3Rec u;
             u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
-            // (not near the end of the item: holding a unit back there would lengthen the tail)
-            const int inext = (i + 2 * PROD_CWARPS < nunits) ? grab() : -1;
-            if (inext >= 0 && inext < nunits && lane < 16) {
-                const Diag3Rec nd = load_diag(s_diags + s_units[inext].diag_begin);
-                const int wide = s_units[inext].cls >= 2;
-                const uint32_t off = (lane < 8) ? nd.offA + (uint32_t)nd.sbeg * (wide ? 128u : 32u * nd.nwA)
-                                                : nd.offB + (uint32_t)nd.sbeg * (wide ? 64u : 32u * nd.nwB);
-                const char* ptr = reinterpret_cast<const char*>(a.tab + off) + (lane & 7) * 128;
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr));
-            }
+            if (i + PROD_CWARPS < nunits) prefetch_unit(s_units + i + PROD_CWARPS, s_diags, a.tab, lane);
             double2* out = scr + (size_t)u.slot * 256;
             if (u.cls < 2) run_unit_square(u, s_diags, a.tab, s1, s2, out, lane);
             else run_unit_wide(u, s_diags, a.tab, s1, s2, out, lane);
-            i = inext >= 0 ? inext : grab();
+            i = grab();
         }
         __threadfence_block();
         named_arrive(BAR_FULL0 + b, PROD_THREADS); // unit results of this item are in scratch buffer b
