@@ -146,7 +146,7 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_1604_07983_b200 import nbs
+    from paper_1604_07983_b200 import nbs, replicas
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
@@ -163,7 +163,7 @@ def main():
     T = cfg["T"]
     npool = min(4, K + W)
     # this rank's time slices: T-parallel replicas (t = rank, rank + world, ...)
-    pool_t = [(rank + i * world) % T for i in range(npool)]
+    pool_t = replicas.rank_slices(rank, world, T, count=npool)
     host = []
     for t in pool_t:
         S = synth.config_slice(cfg, t, L=L)
@@ -261,18 +261,15 @@ def main():
         assert np.isfinite(out_host.view(torch.float64)[:1024]).all()
 
     # ---------------- max over ranks ----------------
-    if world > 1:
-        tmax = torch.tensor([ms, e2e["ms"] if e2e else 0.0], dtype=torch.float64, device=dev)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax[0]);
-        if e2e:
-            e2e["ms"] = float(tmax[1])
+    ms, ms_e2e_max = replicas.max_over_ranks([ms, e2e["ms"] if e2e else 0.0], device=dev)
+    if e2e:
+        e2e["ms"] = ms_e2e_max
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    value = world * K / (ms * 1e-3)
+    value = replicas.aggregate_throughput(K, world, ms)
     prod_ms, prod_calls = stage["product"]
     prod_avg_s = prod_ms * 1e-3 / max(prod_calls, 1)
     alg_flops = flops["product"] * V  # 256 * sum_d K_d cMAC x 8 flop per q, standard count
