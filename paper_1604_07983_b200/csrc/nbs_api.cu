@@ -151,9 +151,9 @@ int launch_fft_axis(nbs_ctx* c, double2* data, size_t R, int axis, double scale,
 
 template <int L>
 int launch_fft_xy_out(nbs_ctx* c, double2* data, size_t R, double scale, double2* tout, cudaStream_t st) {
-    constexpr int C = 256 / L;
+    constexpr int C = fft_xy_comps<L>();
     dim3 grid((unsigned)((R + C - 1) / C), (unsigned)L);
-    k_fft_xy<L, true, true><<<grid, 256, fft_xy_smem_bytes<L>(), st>>>(data, R, scale, tout, c->V);
+    k_fft_xy<L, true, true><<<grid, L * C, fft_xy_smem_bytes<L>(), st>>>(data, R, scale, tout, c->V);
     CU(c, cudaGetLastError());
     ++c->launches;
     return NBS_OK;

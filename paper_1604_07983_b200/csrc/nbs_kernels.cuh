@@ -328,19 +328,22 @@ k_fft_axis_pow2(double2* __restrict__ data, size_t R, int axis, const double2* _
 // out[component][r] with r = x + L (y + L z), 16 KB contiguous per component: the separate
 // transpose pass disappears.  Site stride C + 1 keeps every phase free of bank conflicts.
 // ---------------------------------------------------------------------------------------------
+// components per CTA: 256 / L (4 per CTA at L = 32, two CTAs per SM, was measured slower: 64-byte read segments)
 template <int L>
-constexpr size_t fft_xy_smem_bytes() { return (size_t)L * L * (256 / L + 1) * sizeof(double2); }
+__host__ __device__ constexpr int fft_xy_comps() { return 256 / L; }
+template <int L>
+constexpr size_t fft_xy_smem_bytes() { return (size_t)L * L * (fft_xy_comps<L>() + 1) * sizeof(double2); }
 
 template <int L, bool INV, bool TOUT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(L * fft_xy_comps<L>())
 k_fft_xy(double2* __restrict__ data, size_t R, double scale, double2* __restrict__ tout, size_t V) {
-    constexpr int C = 256 / L, CS = C + 1, NS = L * L;
+    constexpr int C = fft_xy_comps<L>(), CS = C + 1, NS = L * L, NT = L * C;
     extern __shared__ double2 smem[];
     const size_t r0 = (size_t)blockIdx.x * C;
     const int z = blockIdx.y, tid = threadIdx.x;
     const int nc = (int)((R - r0 < (size_t)C) ? (R - r0) : (size_t)C);
     double2* plane = data + (size_t)z * NS * R + r0;
-    for (int i = tid; i < NS * C; i += 256) {
+    for (int i = tid; i < NS * C; i += NT) {
         const int site = i / C, c = i % C;
         if (c < nc) smem[site * CS + c] = plane[(size_t)site * R + c];
     }
@@ -374,12 +377,12 @@ k_fft_xy(double2* __restrict__ data, size_t R, double scale, double2* __restrict
     }
     __syncthreads();
     if (TOUT) {
-        for (int i = tid; i < NS * C; i += 256) {
+        for (int i = tid; i < NS * C; i += NT) {
             const int c = i / NS, site = i % NS;
             if (c < nc) tout[(r0 + c) * V + (size_t)z * NS + site] = smem[site * CS + c];
         }
     } else {
-        for (int i = tid; i < NS * C; i += 256) {
+        for (int i = tid; i < NS * C; i += NT) {
             const int site = i / C, c = i % C;
             if (c < nc) plane[(size_t)site * R + c] = smem[site * CS + c];
         }
