@@ -55,7 +55,13 @@ struct BlockRec {
 constexpr int BLOCKS_THREADS = 256;
 constexpr int BLOCKS_TILES = 216;               // 6 x 6 x 6 tiles of 2 x 2 x 2 source triples
 constexpr int BLOCKS_HALF = 2 * SM_PLANE;       // complex entries of a half row
-inline size_t blocks_smem_bytes(int ndq) { return (size_t)(3 * 144 + ndq * 432 + BLOCKS_HALF) * sizeof(double2); }
+// Shared-memory operand layouts of k_blocks, chosen so that the register tiles of a warp (tile origins
+// 2 i per index, lanes on consecutive i) read without bank conflicts: a source index xi sits at
+// dq_rank(xi) = (xi & 1) * 6 + (xi >> 1) (even and odd values de-interleaved: the lanes' even origins
+// become consecutive), and a diquark row is 13 entries long (odd stride for lanes that walk the rows).
+constexpr int DQ_ROW = 13, DQ_C = 12 * DQ_ROW, DQ_SIZE = 3 * DQ_C; // per diquark type: [c][rank(xi)][rank(xi')]
+__host__ __device__ constexpr int dq_rank(int xi) { return (xi & 1) * 6 + (xi >> 1); }
+inline size_t blocks_smem_bytes(int ndq) { return (size_t)(3 * 144 + ndq * DQ_SIZE + BLOCKS_HALF) * sizeof(double2); }
 
 // acc[a][e0][e1][e2] += coef * sum_c D_c(xi_P0, xi_P1) * S[(c, a0 + a), xi_P2] over the thread's tile
 template <int P0, int P1, int P2>
@@ -67,12 +73,13 @@ __device__ __forceinline__ void blocks_term(double2 (&acc)[2][2][2][2], const do
 #pragma unroll
         for (int ja = 0; ja < 2; ++ja)
 #pragma unroll
-            for (int jb = 0; jb < 2; ++jb) Dv[ja][jb] = Dq[c * 144 + (x[P0] + ja) * 12 + x[P1] + jb];
+            for (int jb = 0; jb < 2; ++jb) // x even: dq_rank(x + j) = 6 j + x / 2
+                Dv[ja][jb] = Dq[c * DQ_C + (6 * ja + (x[P0] >> 1)) * DQ_ROW + 6 * jb + (x[P1] >> 1)];
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                const double2 v = S2[(c + 3 * (a0 + a)) * 12 + x[P2] + j];
+                const double2 v = S2[(c + 3 * (a0 + a)) * 12 + 6 * j + (x[P2] >> 1)];
                 Sv[a][j] = make_double2(coef * v.x, coef * v.y);
             }
 #pragma unroll
@@ -98,13 +105,14 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
     const int ndq = __popc(dq_mask);
     double2* sS = smem;                  // [3][144]
     double2* sD = smem + 3 * 144;        // [ndq][3][144], needed diquark types in increasing dq order
-    double2* sO = sD + ndq * 432;        // [2][SM_PLANE] half row being assembled
+    double2* sO = sD + ndq * DQ_SIZE;    // [2][SM_PLANE] half row being assembled
     const size_t site = blockIdx.x;
     const int tid = threadIdx.x;
     for (int i = tid; i < 144; i += BLOCKS_THREADS) {
-        sS[i] = Su[site * 144 + i];
-        sS[144 + i] = Sd[site * 144 + i];
-        sS[288 + i] = Ss[site * 144 + i];
+        const int j = (i / 12) * 12 + dq_rank(i % 12); // source index de-interleaved
+        sS[j] = Su[site * 144 + i];
+        sS[144 + j] = Sd[site * 144 + i];
+        sS[288 + j] = Ss[site * 144 + i];
     }
     __syncthreads();
     for (int idx = tid; idx < ndq * 432; idx += BLOCKS_THREADS) {
@@ -113,7 +121,7 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
         for (int seen = 0; dq < 9; ++dq)
             if ((dq_mask >> dq) & 1u) { if (seen == slot_dq) break; ++seen; }
         const int rem = idx - slot_dq * 432;
-        const int c = rem / 144, i = (rem / 12) % 12, j = rem % 12;
+        const int c = rem / 144, ri = dq_rank((rem / 12) % 12), rj = dq_rank(rem % 12);
         const double2* S0 = sS + (dq / 3) * 144;
         const double2* S1 = sS + (dq % 3) * 144;
         const int a = (c + 1) % 3, b = (c + 2) % 3;
@@ -122,12 +130,12 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
 #pragma unroll
         for (int pr = 0; pr < 2; ++pr) {
             const int be = 2 * pr, ga = 2 * pr + 1;
-            cfma(acc, S0[(a + 3 * be) * 12 + i], S1[(b + 3 * ga) * 12 + j]); // +eps +cg5
-            cfma(neg, S0[(a + 3 * ga) * 12 + i], S1[(b + 3 * be) * 12 + j]); // +eps -cg5
-            cfma(neg, S0[(b + 3 * be) * 12 + i], S1[(a + 3 * ga) * 12 + j]); // -eps +cg5
-            cfma(acc, S0[(b + 3 * ga) * 12 + i], S1[(a + 3 * be) * 12 + j]); // -eps -cg5
+            cfma(acc, S0[(a + 3 * be) * 12 + ri], S1[(b + 3 * ga) * 12 + rj]); // +eps +cg5
+            cfma(neg, S0[(a + 3 * ga) * 12 + ri], S1[(b + 3 * be) * 12 + rj]); // +eps -cg5
+            cfma(neg, S0[(b + 3 * be) * 12 + ri], S1[(a + 3 * ga) * 12 + rj]); // -eps +cg5
+            cfma(acc, S0[(b + 3 * ga) * 12 + ri], S1[(a + 3 * be) * 12 + rj]); // -eps -cg5
         }
-        sD[idx] = csub(acc, neg);
+        sD[slot_dq * DQ_SIZE + c * DQ_C + ri * DQ_ROW + rj] = csub(acc, neg);
     }
     __syncthreads();
 
@@ -164,7 +172,7 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                 for (int i = 0; i < 16; ++i) (&acc[0][0][0][0])[i] = make_double2(0.0, 0.0);
                 for (int it = br.term_begin; it < br.term_end; ++it) {
                     const BTermRec bt = bterm[it];
-                    const double2* Dq = sD + __popc(dq_mask & ((1u << bt.dq) - 1u)) * 432;
+                    const double2* Dq = sD + __popc(dq_mask & ((1u << bt.dq) - 1u)) * DQ_SIZE;
                     const double2* S2 = sS + bt.f2 * 144;
                     const int perm = bt.p0 * 3 + bt.p1; // (p0, p1) fixes the permutation
                     switch (perm) {
