@@ -285,3 +285,34 @@ def test_identical_sink_baryons_only(torch_cuda, nbs, oracle, L):
     F = run_gpu(torch_cuda, nbs, L, S, chans)
     B = oracle.all_blocks(S, oracle.sink_names(chans))
     assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
+
+
+def test_full_size_32cubed_isospin_relations_config3(torch_cuda, nbs):
+    """BASELINE.json configs[3] (32^3, u = d = s, dense Gaussian propagators) in bench.py's launch
+    configuration: the exact relations between channels of the 52-list that hold when u = d
+    (pinned on the oracle in tests/test_oracle_pins.py::test_isospin_relations_u_equals_d) must hold
+    on the full-volume GPU result, and the sink-swap relation for the identical-baryon sink
+    Lambda Lambda (computed on half of the momenta and mirrored) must hold in r-space."""
+    torch = torch_cuda
+    L, T, t = 32, 64, 5
+    V = L ** 3
+    S = synth.config_slice(synth.CONFIGS[3], t)
+    with nbs.Nbs(L, T) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(t, d["u"], d["d"], d["s"])
+        F = ctx.correlator(t).reshape(52, 4, 4, 4, 4, V)
+        torch.cuda.synchronize()
+
+    def rel(a, b):
+        return float((a - b).abs().max() / torch.maximum(a.abs().max(), b.abs().max()))
+
+    pairs = [(16, 23, +1), (17, 22, +1), (11, 12, -1), (15, 21, -1), (19, 25, -1), (20, 26, +1), (34, 35, -1),
+             (38, 39, +1)]
+    for i, j, sgn in pairs:
+        assert rel(F[i], sgn * F[j]) <= RTOL, (i, j)
+    assert rel(F[18], F[24].transpose(2, 3)) <= RTOL
+    # Lambda Lambda <- Lambda Lambda (channel 10): F_{a1 a2 ..}(r) = - F_{a2 a1 ..}(-r)
+    x = torch.arange(L, device="cuda")
+    neg = (-x) % L
+    minus_r = (neg[:, None, None] + L * (neg[None, :, None] + L * neg[None, None, :])).permute(2, 1, 0).reshape(-1)
+    assert rel(F[10], -F[10].transpose(0, 1)[..., minus_r]) <= RTOL
