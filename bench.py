@@ -31,8 +31,8 @@ UNIT = "time-slices/s"
 FP64_PEAK_TFLOPS = 37.2  # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz; a register-resident
 #                          probe on this pool measured 37.1 (DMMA.8x8x4) and 34.2 (DFMA) TFLOP/s; the two share the units
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_product launch on this workload, from the ncu --set full
-# capture summarised in profiles/r1_v5_summary.md (update together with that file)
-PRODUCT_DRAM_TRAFFIC_BYTES = 83.7e9
+# capture summarised in profiles/r1_v6_summary.md (update together with that file)
+PRODUCT_DRAM_TRAFFIC_BYTES = 83.8e9
 
 
 def parse():
