@@ -169,10 +169,10 @@ int nbs_model_flops(const nbs_ctx* ctx, double* blocks, double* fft, double* pro
  */
 enum {
     NBS_STAGE_BLOCKS = 0,   /* (i) normal baryon blocks, eq. 4.1 */
-    NBS_STAGE_FFT_FWD = 1,  /* forward FFT of the block components */
+    NBS_STAGE_FFT_FWD = 1,  /* forward FFT of the block components (+ expansion of the antisymmetric blocks) */
     NBS_STAGE_PRODUCT = 2,  /* (ii)+(iii) effective blocks and their product, eqs. 4.2-4.3 */
-    NBS_STAGE_FFT_INV = 3,  /* inverse FFT, eq. 2.6 */
-    NBS_STAGE_OUTPUT = 4,   /* final layout F[ch][a1..a4][r] */
+    NBS_STAGE_FFT_INV = 3,  /* inverse FFT, eq. 2.6 (writes the final layout itself when L is a power of two <= 32) */
+    NBS_STAGE_OUTPUT = 4,   /* final layout F[ch][a1..a4][r] as a separate pass (other L; else never timed) */
     NBS_NUM_STAGES = 5
 };
 int nbs_set_timing(nbs_ctx* ctx, int enable);
