@@ -316,3 +316,16 @@ def test_full_size_32cubed_isospin_relations_config3(torch_cuda, nbs):
     neg = (-x) % L
     minus_r = (neg[:, None, None] + L * (neg[None, :, None] + L * neg[None, None, :])).permute(2, 1, 0).reshape(-1)
     assert rel(F[10], -F[10].transpose(0, 1)[..., minus_r]) <= RTOL
+
+
+def test_16cubed_config1_lattice_selected_channels(torch_cuda, nbs, oracle):
+    """BASELINE.json configs[1] lattice (16^3, u = d, s; time slice 7 of 32): element-by-element parity
+    on the whole volume for five channels that cover every accumulator layout, a Lambda/Sigma0 source
+    (shared elementary correlators, source swap) and an identical-baryon sink (sink swap)."""
+    L, t = 16, 7
+    S = synth.config_slice(synth.CONFIGS[1], t)
+    chans = [("p", "n", "p", "n"), ("p", "L", "S0", "p"), ("L", "L", "S0", "S0"), ("Sm", "X0", "Xm", "L"),
+             ("Xm", "X0", "Xm", "X0")]
+    F = run_gpu(torch_cuda, nbs, L, S, chans, t=t, T=32)
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
