@@ -176,6 +176,14 @@ enum {
     NBS_NUM_STAGES = 5
 };
 int nbs_set_timing(nbs_ctx* ctx, int enable);
+
+/*
+ * nbs_set_direct -- tiny-lattice path (row a7 of DESIGN.md, the "primitive" O(L^6) evaluation of
+ * eq. 2.4): with enable != 0 nbs_correlator takes the zero-momentum sum over X of B1(X+r) B2(X) as a shifted
+ * sum in x-space -- the same block, expansion and product kernels, one product task per displacement r that
+ * walks all sites X, no FFT.  Results equal the FFT path up to rounding.  Cost O(V^2): NBS_EINVAL for L > 8.
+ */
+int nbs_set_direct(nbs_ctx* ctx, int enable);
 int nbs_stage_times(nbs_ctx* ctx, double* ms, long long* calls, int reset);
 
 int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);

@@ -52,6 +52,7 @@ struct nbs_ctx {
     PairChanRec* d_pair_chans = nullptr;
     int* d_qorder = nullptr;
     int prod_grid = 0;
+    bool direct = false; // nbs_set_direct: eq. 2.4 as a shifted sum in x-space (tiny lattices)
     long long ntasks = 0;   // entries of d_qorder
     long long nselfconj = 0; // momenta with q == -q
     int* d_baryon_of_slot = nullptr;
@@ -450,8 +451,10 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     }
     {
         StageTimer tm(c, NBS_STAGE_FFT_FWD, st);
-        rc = fft3d(c, sl.B, c->R, false, st);
-        if (rc) return rc;
+        if (!c->direct) {
+            rc = fft3d(c, sl.B, c->R, false, st);
+            if (rc) return rc;
+        }
         if (c->Re) { // antisymmetric blocks: mirror halves restored for the gathers of the product kernel
             k_expand<<<(unsigned)c->V, 256, 0, st>>>(sl.B, c->R, c->d_gather, (int)c->Re, sl.Be);
             CU(c, cudaGetLastError());
@@ -466,7 +469,8 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         pa.Bc = sl.B; pa.Rc = c->R; pa.Be = sl.Be; pa.Re = c->Re; pa.L = c->L;
         pa.slot_src = reinterpret_cast<const int2*>(c->d_slot_src);
         pa.chain_full_n = c->plan.chain_full_n; pa.chain_half_n = c->plan.chain_half_n;
-        pa.ntasks = c->ntasks;
+        pa.ntasks = c->direct ? (long long)c->V : c->ntasks; // direct: one task per displacement r
+        pa.direct = c->direct ? 1 : 0;
         pa.qorder = c->d_qorder;
         pa.pairs = c->d_pairs3; pa.units = c->d_units3; pa.diags = c->d_diags3;
         pa.tab = reinterpret_cast<const uint2*>(c->d_tab3);
@@ -486,8 +490,8 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         else if (need <= c->V * c->Re * sizeof(double2)) dst = sl.Be;
         else return fail(c, NBS_ENOMEM, "channel range too large for the device staging of a host output; use a smaller range");
     }
-    const bool fused = fft_fused(c);
-    {
+    const bool fused = fft_fused(c) && !c->direct;
+    if (!c->direct) {
         StageTimer tm(c, NBS_STAGE_FFT_INV, st);
         rc = fft3d(c, sl.Ft, nout * 256, true, st, fused ? dst : nullptr);
         if (rc) return rc;
@@ -500,6 +504,13 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         ++c->launches;
     }
     if (memloc == NBS_MEM_HOST) CU(c, cudaMemcpyAsync(out, dst, need, cudaMemcpyDeviceToHost, st));
+    return NBS_OK;
+}
+
+int nbs_set_direct(nbs_ctx* c, int enable) {
+    if (!c) return NBS_EINVAL;
+    if (enable && c->L > 8) return fail(c, NBS_EINVAL, "the direct shifted sum is O(V^2): allowed for L <= 8 only");
+    c->direct = enable != 0;
     return NBS_OK;
 }
 

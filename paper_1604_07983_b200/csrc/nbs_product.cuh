@@ -53,6 +53,7 @@ struct ProdCtrl { // at SMO_CTRL
     int pad;
     long long qtask[2];              // prefetched momentum-task indices (alternating slots)
     int meta_q[PROD_NBUF], meta_pair[PROD_NBUF]; // item descriptors handed to the epilogue warps
+    int meta_acc[PROD_NBUF];                     // direct mode: add to the result already stored for this r
 };
 
 // ---- PTX helpers ----------------------------------------------------------------------------
@@ -321,6 +322,9 @@ struct ProdArgs {
     double2* Ft;         // [V][nch_out][256]
     int ch_begin, nch_out;
     unsigned long long* counter; // zeroed before the launch
+    // direct mode (tiny-L path, eq. 2.4 as a shifted sum): Bc / Be hold the x-space blocks, a task is
+    // a displacement r, its items are (X, sink pair) with B1 at X + r and B2 at X, and Ft[r] accumulates over X
+    int direct;
 };
 
 __device__ __forceinline__ size_t minus_q(int L, size_t q) {
@@ -329,12 +333,18 @@ __device__ __forceinline__ size_t minus_q(int L, size_t q) {
     return x + (size_t)L * (y + (size_t)L * z);
 }
 
+__device__ __forceinline__ size_t shifted_site(int L, size_t X, size_t r) { // X + r, periodic
+    const int x = (int)((X % L + r % L) % L), y = (int)(((X / L) % L + (r / L) % L) % L);
+    const int z = (int)((X / ((size_t)L * L) + r / ((size_t)L * L)) % L);
+    return x + (size_t)L * (y + (size_t)L * z);
+}
+
 // Epilogue of one item: elementary correlators = sums of unit results (fixed order), channel
 // correlators = real combinations of them (eqs. 2.2-2.3) -> Ft[q][ch][256].  The pair record and
 // the channel coefficients are first copied to shared memory (one L2 round trip for the item
 // instead of one per use); thread et owns the spin components et + 64 m.
-__device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q, const double2* __restrict__ scr,
-                                             int et, char* s_epi) {
+__device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q, bool accumulate,
+                                             const double2* __restrict__ scr, int et, char* s_epi) {
     Pair3Rec* pr = reinterpret_cast<Pair3Rec*>(s_epi);
     PairChanRec* pcs = reinterpret_cast<PairChanRec*>(s_epi + EPI_PAIR_BYTES);
     {
@@ -344,7 +354,7 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
     named_sync(BAR_EPI, PROD_ETHREADS);
     const int nelem = pr->nelem, nchan = pr->nchan, swap_mask = pr->swap_mask;
     const size_t mq = minus_q(a.L, q);
-    const bool mirror = pr->self_swap && mq != q;
+    const bool mirror = !a.direct && pr->self_swap && mq != q;
     for (int c0 = 0; c0 < nchan; c0 += EPI_CG) {
         const int nc = min(EPI_CG, nchan - c0);
         {
@@ -418,6 +428,14 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
             if (c < nc) {
                 const int ch = pcs[c].ch - a.ch_begin;
                 if (ch >= 0 && ch < a.nch_out) {
+                    if (accumulate) { // direct mode, X > 0: the same thread wrote this entry for the previous X
+#pragma unroll
+                        for (int m = 0; m < 4; ++m) {
+                            const double2 old = __ldcg(a.Ft + (q * a.nch_out + ch) * 256 + et + 64 * m);
+                            acc[c][m].x += old.x;
+                            acc[c][m].y += old.y;
+                        }
+                    }
 #pragma unroll
                     for (int m = 0; m < 4; ++m) __stcs(a.Ft + (q * a.nch_out + ch) * 256 + et + 64 * m, acc[c][m]);
                     if (mirror) { // sink swap: F~(-q)_{a2 a1 a3 a4} = - F~(q)_{a1 a2 a3 a4}; here a1 = m, a2 = et >> 4
@@ -479,7 +497,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
-            combine_item(a, ip, q, scr0 + b * scr_stride, et, smem + SMO_EPI);
+            combine_item(a, ip, q, ctl->meta_acc[b] != 0, scr0 + b * scr_stride, et, smem + SMO_EPI);
             named_arrive(BAR_EMPTY0 + b, PROD_THREADS);
         }
         return;
@@ -493,18 +511,26 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
     long long qt = 0;
     size_t q = 0, mq = 0;
     int cbase = 0, clen = 1;
+    size_t xs = 0, nsites = (size_t)a.L * a.L * a.L; // direct mode: site X of the shifted sum
     int4 nh0 = make_int4(0, 0, 0, 0), nh1 = nh0, nh2 = nh0; // next chain record
     for (unsigned it = 0;; ++it) {
         const int b = it % PROD_NBUF;
         named_sync(BAR_COMPUTE, PROD_CTHREADS); // the staged blocks and unit records of the previous item are consumed
         if (pos == 0) {
-            qt = ctl->qtask[ntask & 1];
+            if (!a.direct || xs == 0) qt = ctl->qtask[ntask & 1]; // new task
             if (qt < a.ntasks) {
-                q = (size_t)__ldg(a.qorder + qt);
-                mq = minus_q(a.L, q);
-                // momenta q > -q leave the pairs of identical sink baryons to the task of -q
-                cbase = (mq < q) ? a.chain_full_n : 0;
-                clen = (mq < q) ? a.chain_half_n : a.chain_full_n;
+                if (a.direct) { // task = displacement r = qt; this pass of the chain: site X = xs
+                    mq = xs;
+                    q = shifted_site(a.L, xs, (size_t)qt);
+                    cbase = 0;
+                    clen = a.chain_full_n;
+                } else {
+                    q = (size_t)__ldg(a.qorder + qt);
+                    mq = minus_q(a.L, q);
+                    // momenta q > -q leave the pairs of identical sink baryons to the task of -q
+                    cbase = (mq < q) ? a.chain_full_n : 0;
+                    clen = (mq < q) ? a.chain_half_n : a.chain_full_n;
+                }
             }
         }
         if (it >= PROD_NBUF) named_sync(BAR_EMPTY0 + b, PROD_THREADS); // scratch buffer b and its descriptor are free again
@@ -522,8 +548,9 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         if (tid == 0) {
             const int4 h2 = (pos > 0) ? nh2 : __ldg(crec + 2); // buf1, off1, buf2, off2
             *next_unit = 0;
-            ctl->meta_q[b] = (int)q;
+            ctl->meta_q[b] = a.direct ? (int)qt : (int)q; // row of Ft this item goes to
             ctl->meta_pair[b] = ip;
+            ctl->meta_acc[b] = (a.direct && xs > 0) ? 1 : 0;
             // unit and diagram records of the pair ride on the first staging barrier of the item
             const uint32_t ubytes = (uint32_t)nunits * (uint32_t)sizeof(Unit3Rec);
             const uint32_t dbytes = (uint32_t)h1.y * (uint32_t)sizeof(Diag3Rec);
@@ -542,7 +569,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             }
             bulk_g2s(s_units, a.units + h1.x, ubytes, rbar);
             bulk_g2s(s_diags, a.diags + h1.z, dbytes, rbar);
-            if (pos == 0) ctl->qtask[(ntask + 1) & 1] = (long long)atomicAdd(a.counter, 1ull); // next momentum task
+            if (pos == 0 && (!a.direct || xs == 0)) ctl->qtask[(ntask + 1) & 1] = (long long)atomicAdd(a.counter, 1ull); // next task
             if (pos + 1 < clen) nh2 = __ldg(crec + 5);
         }
         if (pos + 1 < clen) { nh0 = __ldg(crec + 3); nh1 = __ldg(crec + 4); }
@@ -572,7 +599,12 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         }
         __threadfence_block();
         named_arrive(BAR_FULL0 + b, PROD_THREADS); // unit results of this item are in scratch buffer b
-        if (++pos == clen) { pos = 0; ++ntask; }
+        if (++pos == clen) {
+            pos = 0;
+            if (a.direct && ++xs < nsites) continue; // same displacement, next site X
+            xs = 0;
+            ++ntask;
+        }
     }
 }
 

@@ -329,3 +329,37 @@ def test_16cubed_config1_lattice_selected_channels(torch_cuda, nbs, oracle):
     F = run_gpu(torch_cuda, nbs, L, S, chans, t=t, T=32)
     B = oracle.all_blocks(S, oracle.sink_names(chans))
     assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
+
+
+def test_direct_shifted_sum_path(torch_cuda, nbs, oracle):
+    """Row a7: eq. 2.4 as a shifted sum in x-space (nbs_set_direct), no FFT.  configs[0] (4^3, NN, u = d)
+    against the oracle's direct tier A, and all 52 channels on 3^3 against tier B and the FFT path."""
+    torch = torch_cuda
+    S = synth.config_slice(synth.CONFIGS[0], 0)
+    chans = [("p", "n", "p", "n")]
+    with nbs.Nbs(4, 1, chans) as ctx:
+        ctx.set_direct(True)
+        d = to_dev(torch, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        F = ctx.correlator(0)
+        torch.cuda.synchronize()
+        F = F.cpu().numpy()
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_direct(4, B, chans[0])[None], chans)
+
+    L = 3
+    S = props(L, seed=5)
+    chans = oracle.channels52()
+    with nbs.Nbs(L, 1) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        F_fft = ctx.correlator(0).cpu().numpy()
+        ctx.set_direct(True)
+        F_dir = ctx.correlator(0).cpu().numpy()
+        torch.cuda.synchronize()
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    Fo = oracle.correlator_fft(L, B, chans)
+    assert_parity(F_dir, Fo, chans)
+    assert_parity(F_dir, F_fft, chans)
+    with nbs.Nbs(16, 1, [("p", "n", "p", "n")]) as ctx, pytest.raises(nbs.NbsError):
+        ctx.set_direct(True)
