@@ -336,14 +336,15 @@ k_fft_axis_pow2(double2* __restrict__ data, size_t R, int axis, const double2* _
 // out[component][r] with r = x + L (y + L z), 16 KB contiguous per component: the separate
 // transpose pass disappears.  Site stride C + 1 keeps every phase free of bank conflicts.
 // ---------------------------------------------------------------------------------------------
-// components per CTA: 256 / L (4 per CTA at L = 32, two CTAs per SM, was measured slower: 64-byte read segments)
+// components per CTA: 256 / L; at L = 32 six (96-byte read segments, 112 KB of shared memory: two CTAs per SM
+// overlap their load, transform and store phases; 4 per CTA was measured slower, 8 fits only one CTA per SM)
 template <int L>
-__host__ __device__ constexpr int fft_xy_comps() { return 256 / L; }
+__host__ __device__ constexpr int fft_xy_comps() { return L >= 32 ? 6 : 256 / L; }
 template <int L>
 constexpr size_t fft_xy_smem_bytes() { return (size_t)L * L * (fft_xy_comps<L>() + 1) * sizeof(double2); }
 
 template <int L, bool INV, bool TOUT>
-__global__ void __launch_bounds__(L * fft_xy_comps<L>())
+__global__ void __launch_bounds__(L * fft_xy_comps<L>(), L >= 32 ? 2 : 1)
 k_fft_xy(double2* __restrict__ data, size_t R, double scale, double2* __restrict__ tout, size_t V) {
     constexpr int C = fft_xy_comps<L>(), CS = C + 1, NS = L * L, NT = L * C;
     extern __shared__ double2 smem[];
