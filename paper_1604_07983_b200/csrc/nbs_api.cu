@@ -59,6 +59,8 @@ struct nbs_ctx {
     int* d_one_baryon = nullptr; // scratch for nbs_blocks_x
     int2* d_slot_info = nullptr;     // (row offset, block kind) of every slot
     int* d_gather = nullptr;         // expansion map of the antisymmetric slots
+    int* d_gather_iso = nullptr;     // the same for the isospin-limit fast path (d == u)
+    unsigned dq_mask_iso = 0;
     int2x* d_slot_src = nullptr;     // where the product kernel stages every slot from
     int2* d_one_slot_info = nullptr; // the same for a single baryon (nbs_blocks_x)
     BlockRec* d_brec = nullptr;
@@ -134,16 +136,17 @@ int dev_alloc(nbs_ctx* c, double2*& dst, size_t ncomplex) {
 }
 
 template <bool INV>
-int launch_fft_axis(nbs_ctx* c, double2* data, size_t R, int axis, double scale, cudaStream_t st) {
+int launch_fft_axis(nbs_ctx* c, double2* data, size_t R, int axis, double scale, cudaStream_t st, size_t Rn = 0) {
     const int L = c->L;
-    dim3 grid((unsigned)((R + FFT_THREADS - 1) / FFT_THREADS), (unsigned)(L * L));
+    if (Rn == 0) Rn = R; // Rn: number of (leading) components to transform; R: row length
+    dim3 grid((unsigned)((Rn + FFT_THREADS - 1) / FFT_THREADS), (unsigned)(L * L));
     switch (L) {
-    case 2: k_fft_axis_pow2<2, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
-    case 4: k_fft_axis_pow2<4, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
-    case 8: k_fft_axis_pow2<8, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
-    case 16: k_fft_axis_pow2<16, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
-    case 32: k_fft_axis_pow2<32, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, axis, c->d_tw, scale); break;
-    default: k_fft_axis_generic<INV><<<grid, FFT_THREADS, 0, st>>>(data, R, L, axis, c->d_tw, scale); break;
+    case 2: k_fft_axis_pow2<2, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, Rn, axis, c->d_tw, scale); break;
+    case 4: k_fft_axis_pow2<4, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, Rn, axis, c->d_tw, scale); break;
+    case 8: k_fft_axis_pow2<8, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, Rn, axis, c->d_tw, scale); break;
+    case 16: k_fft_axis_pow2<16, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, Rn, axis, c->d_tw, scale); break;
+    case 32: k_fft_axis_pow2<32, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, Rn, axis, c->d_tw, scale); break;
+    default: k_fft_axis_generic<INV><<<grid, FFT_THREADS, 0, st>>>(data, R, Rn, L, axis, c->d_tw, scale); break;
     }
     CU(c, cudaGetLastError());
     ++c->launches;
@@ -175,15 +178,15 @@ bool fft_fused(const nbs_ctx* c) { return c->L == 2 || c->L == 4 || c->L == 8 ||
 // for the two passes it replaces at 32^3 and is not used forward).  Inverse with `tout` != NULL and
 // L a power of two <= 32: z pass, then the fused x-y kernel writes out[comp][r] directly, which
 // saves the transpose pass (8.4 -> 7.0 ms).  Other L: tout is ignored, the caller transposes.
-int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st, double2* tout = nullptr) {
+int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st, double2* tout = nullptr, size_t Rn = 0) {
     if (fft_fused(c) && inverse && tout) {
         int rc = launch_fft_axis<true>(c, data, R, 2, 1.0 / (double)c->L, st);
         if (rc) return rc;
         return launch_fft_xy_any(c, data, R, 1.0 / ((double)c->L * c->L), tout, st);
     }
     for (int axis = 0; axis < 3; ++axis) {
-        int rc = inverse ? launch_fft_axis<true>(c, data, R, axis, 1.0 / (double)c->L, st)
-                         : launch_fft_axis<false>(c, data, R, axis, 1.0, st);
+        int rc = inverse ? launch_fft_axis<true>(c, data, R, axis, 1.0 / (double)c->L, st, Rn)
+                         : launch_fft_axis<false>(c, data, R, axis, 1.0, st, Rn);
         if (rc) return rc;
     }
     return NBS_OK;
@@ -273,6 +276,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         brec[b].term_end = (int)bterm.size();
     }
     for (int b : c->plan.baryons) c->dq_mask |= c->dq_mask_of[b];
+    for (int i = 0; i < c->plan.n_slots_iso; ++i) c->dq_mask_iso |= c->dq_mask_of[c->plan.baryons[i]];
     std::vector<double2> tw(L);
     for (int m = 0; m < L; ++m) {
         long double ang = -2.0L * 3.141592653589793238462643383279502884L * m / L;
@@ -329,6 +333,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         for (int b = 0; b < NBS_NUM_BARYONS; ++b) one.push_back(make_int2(0, block_kind(b)));
         CUC(upload(c, c->d_slot_info, info));
         CUC(upload(c, c->d_gather, c->plan.gather));
+        CUC(upload(c, c->d_gather_iso, c->plan.gather_iso));
         CUC(upload(c, c->d_slot_src, c->plan.slot_src));
         CUC(upload(c, c->d_one_slot_info, one));
     }
@@ -442,21 +447,24 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     CU(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)stream;
 
+    // isospin-limit fast path: the caller passed the same array for u and d
+    const bool iso = sl.S[0] == sl.S[1] && c->plan.n_slots_iso < (int)c->plan.baryons.size();
     // (i) normal baryon blocks, then forward FFT in place
     int rc;
     {
         StageTimer tm(c, NBS_STAGE_BLOCKS, st);
-        rc = launch_blocks(c, sl, c->d_baryon_of_slot, c->d_slot_info, (int)c->plan.baryons.size(), c->dq_mask, sl.B, c->R, st);
+        rc = launch_blocks(c, sl, c->d_baryon_of_slot, c->d_slot_info, iso ? c->plan.n_slots_iso : (int)c->plan.baryons.size(),
+                           iso ? c->dq_mask_iso : c->dq_mask, sl.B, c->R, st);
         if (rc) return rc;
     }
     {
         StageTimer tm(c, NBS_STAGE_FFT_FWD, st);
         if (!c->direct) {
-            rc = fft3d(c, sl.B, c->R, false, st);
+            rc = fft3d(c, sl.B, c->R, false, st, nullptr, iso ? (size_t)c->plan.row_elems_iso : 0);
             if (rc) return rc;
         }
         if (c->Re) { // antisymmetric blocks: mirror halves restored for the gathers of the product kernel
-            k_expand<<<(unsigned)c->V, 256, 0, st>>>(sl.B, c->R, c->d_gather, (int)c->Re, sl.Be);
+            k_expand<<<(unsigned)c->V, 256, 0, st>>>(sl.B, c->R, iso ? c->d_gather_iso : c->d_gather, (int)c->Re, sl.Be);
             CU(c, cudaGetLastError());
             ++c->launches;
         }

@@ -311,9 +311,9 @@ constexpr int FFT_THREADS = 128;
 
 template <int L, bool INV>
 __global__ void __launch_bounds__(FFT_THREADS)
-k_fft_axis_pow2(double2* __restrict__ data, size_t R, int axis, const double2* __restrict__ tw, double scale) {
-    size_t r = (size_t)blockIdx.x * FFT_THREADS + threadIdx.x;
-    if (r >= R) return;
+k_fft_axis_pow2(double2* __restrict__ data, size_t R, size_t Rn, int axis, const double2* __restrict__ tw, double scale) {
+    size_t r = (size_t)blockIdx.x * FFT_THREADS + threadIdx.x; // the first Rn components of rows of length R
+    if (r >= Rn) return;
     size_t s0, st;
     line_geometry(L, axis, blockIdx.y, s0, st);
     double2 a[L];
@@ -403,9 +403,10 @@ constexpr int FFT_MAXL = 64;
 // Any L (direct O(L^2) DFT); used for lattice sizes that are not powers of two.
 template <bool INV>
 __global__ void __launch_bounds__(FFT_THREADS)
-k_fft_axis_generic(double2* __restrict__ data, size_t R, int L, int axis, const double2* __restrict__ tw, double scale) {
+k_fft_axis_generic(double2* __restrict__ data, size_t R, size_t Rn, int L, int axis, const double2* __restrict__ tw,
+                   double scale) {
     size_t r = (size_t)blockIdx.x * FFT_THREADS + threadIdx.x;
-    if (r >= R) return;
+    if (r >= Rn) return;
     size_t s0, st;
     line_geometry(L, axis, blockIdx.y, s0, st);
     double2 a[FFT_MAXL], b[FFT_MAXL];

@@ -379,6 +379,21 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             if (!derived) pair_comp_order[ip].push_back(k);
         }
 
+    // slot order: baryons whose block follows from a partner's in the isospin limit (n from p, Sigma- from
+    // Sigma+, Xi- from Xi0) go last, so that the fast path works on a prefix of the row
+    auto iso_partner = [&](int b) {
+        const int partner = (b == NBS_N) ? NBS_P : (b == NBS_SIGMA_M) ? NBS_SIGMA_P : (b == NBS_XI_M) ? NBS_XI_0 : -1;
+        return (partner >= 0 && slot_of.count(partner)) ? partner : -1;
+    };
+    {
+        std::vector<int> ordered;
+        for (int b : plan.baryons) if (iso_partner(b) < 0) ordered.push_back(b);
+        plan.n_slots_iso = (int)ordered.size();
+        for (int b : plan.baryons) if (iso_partner(b) >= 0) ordered.push_back(b);
+        plan.baryons = ordered;
+        for (size_t i = 0; i < ordered.size(); ++i) slot_of[ordered[i]] = (int)i;
+    }
+
     // compact site row; expansion map of the antisymmetric slots into full staged blocks
     for (size_t sl = 0; sl < plan.baryons.size(); ++sl) {
         const int kind = block_kind(plan.baryons[sl]);
@@ -399,6 +414,28 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
                         const Located loc = locate(kind, x1, x2, x3);
                         const int src = base + al * AS_PLANE + loc.idx;
                         plan.gather[ebase + al * SM_PLANE + sm_index(x1, x2, x3)] = src | (loc.sign < 0 ? (1 << 30) : 0);
+                    }
+    }
+
+    // expansion map of the isospin-limit fast path: derived slots gather from their partner's compact block
+    plan.gather_iso = plan.gather;
+    plan.row_elems_iso = plan.n_slots_iso < (int)plan.baryons.size() ? plan.slot_off[plan.n_slots_iso] : plan.row_elems;
+    for (size_t sl = plan.n_slots_iso; sl < plan.baryons.size(); ++sl) {
+        const int b = plan.baryons[sl], partner = iso_partner(b);
+        const int pbase = plan.slot_off[slot_of[partner]], pkind = block_kind(partner);
+        const int ebase = plan.slot_src[sl].y;
+        for (int al = 0; al < 4; ++al)
+            for (int x1 = 0; x1 < NXI; ++x1)
+                for (int x2 = 0; x2 < NXI; ++x2)
+                    for (int x3 = 0; x3 < NXI; ++x3) {
+                        // n(x1 x2 x3) = -p(x2 x1 x3);  Sigma-(x) = Sigma+(x);  Xi-(x) = -Xi0(x)
+                        const bool tr = (b == NBS_N);
+                        const int y1 = tr ? x2 : x1, y2 = tr ? x1 : x2;
+                        const int sign = (b == NBS_SIGMA_M) ? +1 : -1;
+                        int& g = plan.gather_iso[ebase + al * SM_PLANE + sm_index(x1, x2, x3)];
+                        if ((pkind == BK_ASYM13 ? y1 : y2) == x3) { g = -1; continue; } // partner's diagonal: zero
+                        const Located loc = locate(pkind, y1, y2, x3);
+                        g = (pbase + al * AS_PLANE + loc.idx) | ((sign * loc.sign < 0) ? (1 << 30) : 0);
                     }
     }
 

@@ -155,6 +155,12 @@ struct Plan {
     // where the product kernel stages slot s from: slot_src[s].x = 0: compact row at offset .y (full
     // kinds are already staged blocks there); 1: expanded row at offset .y
     std::vector<int2x> slot_src;
+    // Isospin-limit fast path (used when the caller passes d == u): with identical u and d
+    // propagators  n(xi1 xi2 xi3) = -p(xi2 xi1 xi3),  Sigma- = Sigma+,  Xi- = -Xi0  hold for the blocks, so the
+    // derived slots (placed last in the compact row) are neither built nor transformed: n_slots_iso slots and
+    // row_elems_iso components go through k_blocks / FFT, and gather_iso expands the derived ones from their partners.
+    int n_slots_iso = 0, row_elems_iso = 0;
+    std::vector<int> gather_iso;
     std::vector<int> chan_pair; // pair index of each channel
     double sumK_std = 0;        // sum over channels of sum_d K_d (the paper's count)
     double sumK_exec = 0;       // sum over the computed elementary correlators of pairs of different sink baryons
