@@ -88,7 +88,9 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
  * nbs_load_propagators -- hand the u, d, s propagators of time slice t to the library
  * ("Assuming that the quark propagators are already solved").
  *   u, d, s : each [L^3][12][12] complex128 (layout above).  Pointer equality (d == u, s == u)
- *             is allowed and means the same array.
+ *             is allowed and means the same array; d == u additionally selects the isospin-limit fast path
+ *             (PAPER.md:102): the n, Sigma-, Xi- blocks are derived from p, Sigma+, Xi0 instead of being built
+ *             and Fourier transformed (same results up to rounding).
  *   memloc  : NBS_MEM_DEVICE -> borrowed, must stay valid until the matching nbs_correlator(t)
  *             has completed on its stream;  NBS_MEM_HOST -> copied asynchronously on `stream`
  *             into library-owned device memory (the caller may reuse the host buffer after the
