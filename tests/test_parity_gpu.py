@@ -383,3 +383,13 @@ def test_isospin_fast_path_matches_general_path(torch_cuda, nbs, oracle):
     B = oracle.all_blocks(S, oracle.sink_names(chans))
     assert_parity(F_iso, oracle.correlator_fft(L, B, chans), chans)
     assert_parity(F_iso, F_gen, chans)
+
+
+def test_8cubed_selected_channels(torch_cuda, nbs, oracle):
+    """L = 8: the remaining power-of-two instance of the in-register FFT and of the fused inverse x-y kernel."""
+    L = 8
+    S = props(L, seed=19)
+    chans = [("p", "n", "p", "n"), ("S0", "L", "Sp", "Sm"), ("S0", "S0", "L", "L")]
+    F = run_gpu(torch_cuda, nbs, L, S, chans)
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
