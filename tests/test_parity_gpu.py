@@ -393,3 +393,26 @@ def test_8cubed_selected_channels(torch_cuda, nbs, oracle):
     F = run_gpu(torch_cuda, nbs, L, S, chans)
     B = oracle.all_blocks(S, oracle.sink_names(chans))
     assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
+
+
+def test_smallest_lattice(torch_cuda, nbs, oracle):
+    """L = 2, the smallest lattice nbs_create accepts (include/nbs.h): every momentum is its own negative, so
+    the sink-swap mirror of identical baryons never applies.  All 52 channels, through the FFT path and
+    through the direct shifted-sum path (row a7); L = 1 is rejected."""
+    torch = torch_cuda
+    L = 2
+    S = props(L, seed=33)
+    chans = oracle.channels52()
+    with nbs.Nbs(L, 1) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        F_fft = ctx.correlator(0).cpu().numpy()
+        ctx.set_direct(True)
+        F_dir = ctx.correlator(0).cpu().numpy()
+        torch.cuda.synchronize()
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    Fo = oracle.correlator_fft(L, B, chans)
+    assert_parity(F_fft, Fo, chans)
+    assert_parity(F_dir, Fo, chans)
+    with pytest.raises(nbs.NbsError):
+        nbs.Nbs(1, 1)
