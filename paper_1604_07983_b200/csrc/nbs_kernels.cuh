@@ -153,7 +153,6 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
             if (kind == BK_FULL) {
                 active = tid < BLOCKS_TILES;
                 x[0] = 2 * (tid / 36); x[1] = 2 * ((tid / 6) % 6); x[2] = 2 * (tid % 6);
-                if (tid < 24) sO[(tid / 12) * SM_PLANE + (tid % 12) * SM_STRIDE1 + 144] = make_double2(0.0, 0.0);
             } else {
                 active = tid < 252;
                 const int h = tid / 126, tt = tid - h * 126;
@@ -164,14 +163,15 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                 x[2] = 2 * ib;
                 if (kind == BK_ASYM13) { x[0] = 2 * ia; x[1] = 2 * ic; }
                 else { x[1] = 2 * ia; x[0] = 2 * ic; }
-                if (tid < 48) sO[(tid / 12) * AS_PLANE + (tid % 12) * AS_ROW + 66] = make_double2(0.0, 0.0);
             }
+            double2 acc[2][2][2][2];
             if (active) {
-                double2 acc[2][2][2][2];
 #pragma unroll
                 for (int i = 0; i < 16; ++i) (&acc[0][0][0][0])[i] = make_double2(0.0, 0.0);
+                BTermRec nxt = bterm[br.term_begin];
                 for (int it = br.term_begin; it < br.term_end; ++it) {
-                    const BTermRec bt = bterm[it];
+                    const BTermRec bt = nxt; // the next term record is fetched under this term's arithmetic
+                    if (it + 1 < br.term_end) nxt = bterm[it + 1];
                     const double2* Dq = sD + __popc(dq_mask & ((1u << bt.dq) - 1u)) * DQ_SIZE;
                     const double2* S2 = sS + bt.f2 * 144;
                     const int perm = bt.p0 * 3 + bt.p1; // (p0, p1) fixes the permutation
@@ -184,6 +184,16 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                     default: blocks_term<2, 1, 0>(acc, Dq, S2, bt.coef, a0, x); break;
                     }
                 }
+            }
+            // the bulk store of the previous half row (issued by thread 0) must have read sO before it is rewritten
+            if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            __syncthreads();
+            if (kind == BK_FULL) {
+                if (tid < 24) sO[(tid / 12) * SM_PLANE + (tid % 12) * SM_STRIDE1 + 144] = make_double2(0.0, 0.0);
+            } else {
+                if (tid < 48) sO[(tid / 12) * AS_PLANE + (tid % 12) * AS_ROW + 66] = make_double2(0.0, 0.0);
+            }
+            if (active) {
 #pragma unroll
                 for (int a = 0; a < 2; ++a)
 #pragma unroll
@@ -201,13 +211,18 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                                 }
                             }
             }
+            // the half row leaves through the async proxy (one bulk copy shared -> global), under the next pass
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncthreads();
-            const int n = (kind == BK_FULL) ? BLOCKS_HALF : AS_BLOCK;
-            double2* dst = orow + info.x + ((kind == BK_FULL) ? pass * BLOCKS_HALF : 0);
-            for (int i = tid; i < n; i += BLOCKS_THREADS) dst[i] = sO[i];
-            __syncthreads();
+            if (tid == 0) {
+                const int n = (kind == BK_FULL) ? BLOCKS_HALF : AS_BLOCK;
+                double2* dst = orow + info.x + ((kind == BK_FULL) ? pass * BLOCKS_HALF : 0);
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n\tcp.async.bulk.commit_group;"
+                             :: "l"(dst), "r"((uint32_t)__cvta_generic_to_shared(sO)), "r"((uint32_t)(n * sizeof(double2))) : "memory");
+            }
         }
     }
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); // sO must outlive the last copy
 }
 
 // Expansion of the antisymmetric blocks after the forward FFT: compact rows [site][Rc] -> full staged
