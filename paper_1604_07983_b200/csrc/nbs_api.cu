@@ -196,6 +196,7 @@ int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, const int2* d_i
                   double2* out, size_t row_stride, cudaStream_t st) {
     int ndq = 0;
     for (int b = 0; b < 9; ++b) ndq += (dq_mask >> b) & 1u;
+    if (nslots > BLOCKS_MAX_SLOTS) return fail(c, NBS_EINVAL, "too many block slots");
     k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, blocks_smem_bytes(ndq), st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask,
                                                                           c->d_brec, c->d_bterm, d_info, out, row_stride);
     CU(c, cudaGetLastError());

@@ -61,7 +61,8 @@ constexpr int BLOCKS_HALF = 2 * SM_PLANE;       // complex entries of a half row
 // become consecutive), and a diquark row is 13 entries long (odd stride for lanes that walk the rows).
 constexpr int DQ_ROW = 13, DQ_C = 12 * DQ_ROW, DQ_SIZE = 3 * DQ_C; // per diquark type: [c][rank(xi)][rank(xi')]
 __host__ __device__ constexpr int dq_rank(int xi) { return (xi & 1) * 6 + (xi >> 1); }
-inline size_t blocks_smem_bytes(int ndq) { return (size_t)(3 * 144 + ndq * DQ_SIZE + BLOCKS_HALF) * sizeof(double2); }
+constexpr int BLOCKS_MAX_SLOTS = 16; // per-slot records kept in shared memory (there are 11 interpolating fields)
+inline size_t blocks_smem_bytes(int ndq) { return (size_t)(3 * 144 + ndq * DQ_SIZE + BLOCKS_HALF + BLOCKS_MAX_SLOTS) * sizeof(double2); }
 
 // acc[a][e0][e1][e2] += coef * sum_c D_c(xi_P0, xi_P1) * S[(c, a0 + a), xi_P2] over the thread's tile
 template <int P0, int P1, int P2>
@@ -106,8 +107,14 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
     double2* sS = smem;                  // [3][144]
     double2* sD = smem + 3 * 144;        // [ndq][3][144], needed diquark types in increasing dq order
     double2* sO = sD + ndq * DQ_SIZE;    // [2][SM_PLANE] half row being assembled
+    int4* sSlot = reinterpret_cast<int4*>(sO + BLOCKS_HALF); // [nslots] {term_begin, term_end, row offset, block kind}
     const size_t site = blockIdx.x;
     const int tid = threadIdx.x;
+    if (tid < nslots) {
+        const BlockRec br = brec[baryon_of_slot[tid]];
+        const int2 info = slot_info[tid];
+        sSlot[tid] = make_int4(br.term_begin, br.term_end, info.x, info.y);
+    }
     for (int i = tid; i < 144; i += BLOCKS_THREADS) {
         const int j = (i / 12) * 12 + dq_rank(i % 12); // source index de-interleaved
         sS[j] = Su[site * 144 + i];
@@ -141,8 +148,9 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
 
     double2* orow = out + site * row_stride;
     for (int slot = 0; slot < nslots; ++slot) {
-        const BlockRec br = brec[baryon_of_slot[slot]];
-        const int2 info = slot_info[slot]; // (offset inside the site row, block kind)
+        const int4 rec = sSlot[slot];
+        const BlockRec br = {rec.x, rec.y};
+        const int2 info = make_int2(rec.z, rec.w); // (offset inside the site row, block kind)
         const int kind = info.y;
         // full blocks: two passes of 2 sink spins, 216 tiles each; antisymmetric blocks (nbs_tables.hpp):
         // one pass, 2 x 126 tiles on or above the diagonal of the antisymmetric slot pair
