@@ -215,7 +215,7 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                                     sO[a * SM_PLANE + sm_index(xi0, xi1, xi2)] = acc[a][e0][e1][e2];
                                 } else {
                                     const int xa = (kind == BK_ASYM13) ? xi0 : xi1, xc = (kind == BK_ASYM13) ? xi1 : xi0;
-                                    if (xa < xi2) sO[(a0 + a) * AS_PLANE + xc * AS_ROW + as_pair_index(xa, xi2)] = acc[a][e0][e1][e2];
+                                    if (xa < xi2) sO[(a0 + a) * AS_PLANE + as_row_rank(xc) * AS_ROW + as_pair_index(xa, xi2)] = acc[a][e0][e1][e2];
                                 }
                             }
             }

@@ -33,7 +33,9 @@ NBS_HD constexpr int sm_index(int xi1, int xi2, int xi3) { return xi1 * SM_STRID
 // two source slots (the Wick sign of exchanging the two identical quark fields): p, Sigma+, Sigma-
 // in slots (1,3), n, Xi0, Xi- in slots (2,3).  Only the entries with xi_a < xi_b are built and
 // Fourier transformed (66 of 144 index pairs; 46 % of the data), in the "compact" layout
-//   antisymmetric plane: [xi_c (free slot): 12][pair (xi_a < xi_b): 66, then one pad]  (row 67);
+//   antisymmetric plane: [rank(xi_c) (free slot): 12][pair (xi_a < xi_b): 66, then one pad]  (row 67),
+//   rank(xi) = 6 (xi & 1) + (xi >> 1): the lanes of the block kernel (tile origins xi_c = 2 i_c fastest, then
+//   xi_b = 2 i_b) store to rows 67 apart and pairs 2 apart, 3 n + const modulo the 8 bank groups;
 // after the transform they are expanded (mirror entries with the sign flipped, diagonal zero) into
 // the full staged layout the product kernel gathers from.
 enum { BK_FULL = 0, BK_ASYM13 = 1, BK_ASYM23 = 2 };
@@ -41,6 +43,7 @@ constexpr int AS_ROW = 67;
 constexpr int AS_PLANE = 12 * AS_ROW;  // 804
 constexpr int AS_BLOCK = 4 * AS_PLANE; // 3216 complex per compact antisymmetric block
 NBS_HD constexpr int as_pair_index(int a, int b) { return a * (23 - a) / 2 + (b - a - 1); } // a < b
+NBS_HD constexpr int as_row_rank(int c) { return (c & 1) * 6 + (c >> 1); }
 NBS_HD constexpr int plane_elems(int kind) { return kind == BK_FULL ? SM_PLANE : AS_PLANE; }
 NBS_HD constexpr int block_elems(int kind) { return 4 * plane_elems(kind); }
 struct Located {
@@ -50,9 +53,9 @@ struct Located {
 NBS_HD constexpr Located locate(int kind, int xi1, int xi2, int xi3) {
     if (kind == BK_FULL) return Located{sm_index(xi1, xi2, xi3), 1};
     const int a = (kind == BK_ASYM13) ? xi1 : xi2, b = xi3, c = (kind == BK_ASYM13) ? xi2 : xi1;
-    if (a == b) return Located{c * AS_ROW + 66, 1}; // identically zero (the pad)
-    if (a < b) return Located{c * AS_ROW + as_pair_index(a, b), 1};
-    return Located{c * AS_ROW + as_pair_index(b, a), -1};
+    if (a == b) return Located{as_row_rank(c) * AS_ROW + 66, 1}; // identically zero (the pad)
+    if (a < b) return Located{as_row_rank(c) * AS_ROW + as_pair_index(a, b), 1};
+    return Located{as_row_rank(c) * AS_ROW + as_pair_index(b, a), -1};
 }
 int block_kind(int baryon); // from the slot flavours of eqs. 2.2-2.3
 
