@@ -128,7 +128,7 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
         for (int seen = 0; dq < 9; ++dq)
             if ((dq_mask >> dq) & 1u) { if (seen == slot_dq) break; ++seen; }
         const int rem = idx - slot_dq * 432;
-        const int c = rem / 144, ri = dq_rank((rem / 12) % 12), rj = dq_rank(rem % 12);
+        const int c = rem / 144, ri = (rem / 12) % 12, rj = rem % 12; // positions (ranks) of xi, xi': lanes read consecutive entries
         const double2* S0 = sS + (dq / 3) * 144;
         const double2* S1 = sS + (dq % 3) * 144;
         const int a = (c + 1) % 3, b = (c + 2) % 3;
