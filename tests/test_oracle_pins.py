@@ -304,3 +304,82 @@ def test_pn_closed_form_with_diagonal_propagators():
     corr = np.array([np.sum(a[O._shift_index(L, r)] * b) for r in range(V)])
     ref = 1080 * np.einsum("ac,bd,r->abcdr", np.eye(4), np.eye(4), corr)
     assert _close(F, ref)
+
+
+# ------------------------------------------------------------------ displacement orientation (L > 2)
+# Reading A9 (eq. 2.1: B1 sits at X + r, B2 at X) and the q / -q pairing of eq. 2.6
+# (PAPER.md:59).  At L = 2 every r equals -r and every twiddle is +-1, so the pins above cannot tell
+# F(r) from F(-r); these run at L = 3 and 4, where r != -r, on channels with B1 != B2.
+ASYM_CHANNELS = [("p", "L", "Sp", "n"), ("S0", "L", "Sp", "Sm"), ("Xm", "L", "S0", "Xm")]
+
+
+def _site(L, x, y, z):
+    return x + L * (y + L * z)
+
+
+def test_orientation_tierA_equals_tierB_on_3cubed():
+    """eq. 2.4 (direct X-sum, B1 at X + r) == eq. 2.6 (B~1(q) B~2(-q), inverse FFT) at every r of a 3^3
+    lattice; F(r) != F(-r) there, so a swapped q <-> -q pairing or fft <-> ifft would fail."""
+    L = 3
+    S = rand_props(L, seed=31)
+    bl = O.all_blocks(S, O.sink_names(ASYM_CHANNELS))
+    FB = O.correlator_fft(L, bl, ASYM_CHANNELS)
+    mr = O.minus_q_index(L)
+    some = [_site(L, 1, 0, 0), _site(L, 2, 0, 0), _site(L, 1, 2, 0), _site(L, 2, 1, 0), _site(L, 0, 1, 2), _site(L, 0, 2, 1)]
+    for ic, ch in enumerate(ASYM_CHANNELS):
+        rs = list(range(L ** 3)) if ic == 0 else some  # every r for the first channel, three (r, -r) pairs for the others
+        FA = O.correlator_direct(L, bl, ch, rs=rs)
+        scale = abs(FA).max()
+        assert abs(FA[..., rs] - FB[ic][..., rs]).max() <= 1e-13 * scale, ch
+        # the test has teeth: the mirrored function is a different one
+        assert abs(FB[ic][..., rs] - FB[ic][..., mr[rs]]).max() > 1e-2 * scale, ch
+
+
+def test_orientation_two_site_support_4cubed():
+    """Propagators supported on two sites x0, x1 of a 4^3 lattice: blocks live on those sites, so eq. 2.4 gives
+    F(x0 - x1) = G(B1(x0), B2(x1)), F(x1 - x0) = G(B1(x1), B2(x0)), F(0) = G(x0, x0) + G(x1, x1) and zero at
+    the other 61 displacements (G = pair_tensor, the site-local sum over P and xi').  r = x0 - x1 = (1, 3, 2)
+    differs from -r = (3, 1, 2) (mod 4) on two axes.  Checked for tier A and tier B."""
+    L, V = 4, 64
+    x0, x1 = (2, 1, 3), (1, 2, 1)
+    i0, i1 = _site(L, *x0), _site(L, *x1)
+    r01 = _site(L, *[(a - b) % L for a, b in zip(x0, x1)])
+    r10 = _site(L, *[(b - a) % L for a, b in zip(x0, x1)])
+    assert r01 != r10 and r01 == _site(L, 1, 3, 2) and r10 == _site(L, 3, 1, 2)
+    full = rand_props(L, seed=32)
+    S = {f: np.zeros_like(full[f]) for f in "uds"}
+    for f in "uds":
+        S[f][[i0, i1]] = full[f][[i0, i1]]
+    bl = O.all_blocks(S, O.sink_names(ASYM_CHANNELS))
+    FB = O.correlator_fft(L, bl, ASYM_CHANNELS)
+    for ic, ch in enumerate(ASYM_CHANNELS):
+        B1, B2 = bl[ch[0]], bl[ch[1]]
+        G = O.pair_tensor(B1[[i0, i1, i0, i1]], B2[[i1, i0, i0, i1]], ch)  # (x0,x1), (x1,x0), (x0,x0), (x1,x1)
+        ref = np.zeros((4, 4, 4, 4, V), dtype=np.complex128)
+        ref[..., r01] = G[0]
+        ref[..., r10] = G[1]
+        ref[..., 0] = G[2] + G[3]
+        scale = abs(ref).max()
+        assert abs(G[0] - G[1]).max() > 1e-2 * scale  # F(r01) and F(r10) are different numbers
+        FA = O.correlator_direct(L, bl, ch, rs=[0, r01, r10, 1, 17, 63])
+        for r in (0, r01, r10, 1, 17, 63):
+            assert abs(FA[..., r] - ref[..., r]).max() <= 1e-13 * scale, (ch, r)
+        assert abs(FB[ic] - ref).max() <= 1e-13 * scale, ch
+
+
+def test_orientation_tierW_equals_tierA_on_3cubed():
+    """Brute-force Wick contraction (oracle/wick.c: operators B1 at X + r, B2 at X, eq. 2.1) against tier A at
+    asymmetric displacements of a 3^3 lattice, B1 != B2."""
+    from oracle import wick
+    L = 3
+    S = rand_props(L, seed=33)
+    ch = ("p", "L", "Sp", "n")
+    spins = [(0, 1, 0, 1), (1, 0, 3, 2)]
+    rs = [_site(L, 1, 0, 2), _site(L, 2, 0, 1), _site(L, 0, 1, 0)]  # r, -r, and another one
+    bl = O.all_blocks(S, ch[:2])
+    FA = O.correlator_direct(L, bl, ch, rs=rs)
+    FW = wick.wick_fourpt(L, S, ch, spins, rs)
+    FAs = np.array([[FA[s][r] for s in spins] for r in rs])
+    scale = abs(FW).max()
+    assert abs(FAs - FW).max() <= 1e-12 * scale
+    assert abs(FW[0] - FW[1]).max() > 1e-2 * scale  # F(r) != F(-r)
