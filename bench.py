@@ -28,11 +28,36 @@ if ROOT not in sys.path:
 
 METRIC = "nbs_correlator_time_slices_per_s_52ch_32c64_fp64"
 UNIT = "time-slices/s"
-FP64_PEAK_TFLOPS = 37.2  # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz; a register-resident
-#                          probe on this pool measured 37.1 (DMMA.8x8x4) and 34.2 (DFMA) TFLOP/s; the two share the units
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_product launch on this workload, from the ncu --set full
-# capture summarised in profiles/r1_v6_summary.md (update together with that file)
-PRODUCT_DRAM_TRAFFIC_BYTES = 83.8e9
+# Cross-check only: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz.  The roofline denominator is
+# MEASURED in this process by nbs_probe_fp64 (register-resident DMMA.8x8x4 on all SMs, include/nbs.h).
+FP64_PEAK_DERIVED_TFLOPS = 37.2
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_product launch on configs[2], parsed from the committed
+# `ncu --set full` capture of the benched kernel (the .md beside it names the command and the commit)
+PRODUCT_NCU_CSV = os.path.join(ROOT, "profiles", "r2_product_ncu.csv")
+
+
+def product_dram_traffic():
+    """(bytes per launch, source) from profiles/r2_product_ncu.csv, or (None, reason)."""
+    try:
+        rd = wr = None
+        with open(PRODUCT_NCU_CSV) as fh:
+            for line in fh:
+                cells = [c.strip().strip('"') for c in line.split(",")]
+                if len(cells) < 3:
+                    continue
+                name, unit, val = cells[0], cells[1].lower(), cells[2]
+                if name not in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    continue
+                scale = {"byte": 1.0, "kbyte": 1e3, "mbyte": 1e6, "gbyte": 1e9, "tbyte": 1e12}[unit]
+                if name.endswith("read.sum"):
+                    rd = float(val) * scale
+                else:
+                    wr = float(val) * scale
+        if rd is None or wr is None:
+            return None, "profiles/r2_product_ncu.csv has no dram__bytes rows"
+        return rd + wr, "profiles/r2_product_ncu.csv"
+    except OSError:
+        return None, "profiles/r2_product_ncu.csv missing"
 
 
 def parse():
@@ -45,7 +70,8 @@ def parse():
     ap.add_argument("--lattice", type=int, default=0, help="override L (debugging only; invalidates the metric)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--oracle-sample-L", type=int, default=5)
+    ap.add_argument("--oracle-sample-L", type=int, default=0,
+                    help="sub-lattice of the CPU oracle's timed sample (default: 6 for cpu_baseline, 8 for --impl reference)")
     return ap.parse_args()
 
 
@@ -94,27 +120,29 @@ def oracle_leg(sample_L: int, cfg_index: int, steps: int, warmup: int) -> dict:
     cfg = synth.CONFIGS[cfg_index]
     chans = O.channels52()
     V_full = cfg["L"] ** 3
-    times = []
+    times, cpu = [], []
     for i in range(warmup + steps):
         S = synth.config_slice(cfg, i % cfg["T"], L=sample_L)
+        c0 = os.times()
         t0 = time.perf_counter()
         B = O.all_blocks(S, O.sink_names(chans))
         F = O.correlator_fft(sample_L, B, chans)
         dt = time.perf_counter() - t0
+        c1 = os.times()
         assert np.isfinite(F).all()
         if i >= warmup:
             times.append(dt)
+            cpu.append((c1.user + c1.system) - (c0.user + c0.system))
     per_step = sum(times) / len(times)
     sites_per_s = sample_L ** 3 / per_step
-    try:
-        import threadpoolctl
-        cores = max([p["num_threads"] for p in threadpoolctl.threadpool_info()] + [1])
-    except Exception:
-        cores = 1
+    # threads the oracle actually kept busy: process CPU time / wall time of the timed samples
+    cores = max(1.0, round(sum(cpu) / sum(times), 1))
     return {"value": sites_per_s / V_full, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{sample_L}^3 sites of one slice (same flavour recipe, all 52 channels), "
-                      f"{per_step:.1f} s per sample, scaled by {sample_L ** 3}/{V_full} sites",
-            "ms_per_step": per_step * 1e3 * V_full / sample_L ** 3, "host_cpus": os.cpu_count()}
+            "sample": f"one step = the whole path on a periodic {sample_L}^3 sub-lattice ({sample_L ** 3} of the {V_full} sites "
+                      f"of a slice; same flavour recipe, all 52 channels): {per_step:.1f} s measured per step; the oracle's "
+                      f"cost is per site, so value = ({sample_L ** 3}/{V_full}) slices per step / measured seconds per step",
+            "ms_per_step": per_step * 1e3, "ms_per_slice_extrapolated": per_step * 1e3 * V_full / sample_L ** 3,
+            "host_cpus": os.cpu_count()}
 
 
 def main():
@@ -133,11 +161,11 @@ def main():
         if rank != 0:
             return
         steps, warm = max(1, min(args.steps, 3)), min(args.warmup, 1)
-        leg = oracle_leg(args.oracle_sample_L, args.config, steps, warm)
+        leg = oracle_leg(args.oracle_sample_L or 8, args.config, steps, warm)
         line = {"impl": "reference", "metric": METRIC, "value": leg["value"], "unit": UNIT, "n_gpus": args.gpus,
                 "steps": steps, "warmup": warm, "ms_per_step": leg["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": workload},
+                "config": {"workload": workload, "ms_per_slice_extrapolated": leg["ms_per_slice_extrapolated"]},
                 "cpu_baseline": {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample")},
                 "e2e": {"value": leg["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
         print(json.dumps(line))
@@ -201,6 +229,10 @@ def main():
     for i in range(W):
         step_resident(i)
     torch.cuda.synchronize()
+    # measured FP64 peaks of this device, in this process (nbs_probe_fp64): ~0.3 s per mix
+    probe = {name: ctx.probe_fp64(mode, 60000)["tflops"]
+             for name, mode in (("dmma", 0), ("dfma", 1), ("dadd", 2), ("mix_16x16_kstep", 3), ("mix_64x4_kstep", 4))}
+    torch.cuda.synchronize()
     ctx.set_timing(True)
     ctx.stage_times(reset=True)
     launches0 = ctx.kernel_launches()
@@ -229,14 +261,15 @@ def main():
         # Time slices are pipelined over two CUDA streams (the library keeps two
         # workspace slots, t % 2): the 7 GB device-to-host copy of slice i runs on the copy engine
         # while the kernels of slice i + 1 run.  Every slice still pays its own H2D and D2H.
-        streams2 = [stream, torch.cuda.Stream(device=dev)]
+        nslots = ctx.num_slots()  # one stream per workspace slot; with one slot the slices serialise on one stream
+        streams2 = [stream, torch.cuda.Stream(device=dev) if nslots > 1 else stream]
         outs_host = [torch.empty((nch, 256, V), dtype=torch.complex128).pin_memory() for _ in range(2)]
         out_host = outs_host[0]
 
         def step_e2e(i):
             t = pool_t[i % npool]
             h = host[i % npool]
-            st = streams2[t % 2]                                     # one stream per workspace slot (t % 2)
+            st = streams2[t % nslots]                                # one stream per workspace slot (t % nslots)
             ctx.load(t, h["u"], h["d"], h["s"], stream=st)          # H2D inside the library
             ctx.correlator(t, out=outs_host[t % 2], stream=st)      # D2H of F inside the library
         step_e2e(0)
@@ -246,12 +279,14 @@ def main():
         f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         Ke = max(2, min(K, 6))
         f0.record(stream)
-        streams2[1].wait_event(f0)
+        if nslots > 1:
+            streams2[1].wait_event(f0)
         for i in range(Ke):
             step_e2e(2 + i)
-        join = torch.cuda.Event()
-        join.record(streams2[1])
-        stream.wait_event(join)
+        if nslots > 1:
+            join = torch.cuda.Event()
+            join.record(streams2[1])
+            stream.wait_event(join)
         f1.record(stream)
         torch.cuda.synchronize()
         barrier()
@@ -274,6 +309,8 @@ def main():
     prod_avg_s = prod_ms * 1e-3 / max(prod_calls, 1)
     alg_flops = flops["product"] * V  # 256 * sum_d K_d cMAC x 8 flop per q, standard count
     achieved = alg_flops / prod_avg_s / 1e12
+    peak = probe["dmma"]
+    traffic, traffic_src = product_dram_traffic()
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -286,13 +323,16 @@ def main():
         "gpu_launches": int(launches),
         "stages_ms_per_step": {k: v[0] / max(v[1], 1) for k, v in stage.items()},
         "roofline": {"bound": "alu", "kernel": "product (effective blocks x product, eqs. 4.2-4.3)",
-                     "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": PRODUCT_DRAM_TRAFFIC_BYTES,
-                     "peak_source": "derived FP64 pipe peak 148 SM x 64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+                     "peak_source": "measured in this run: nbs_probe_fp64 mode 0 (register-resident DMMA.8x8x4, 16 warps per SM, "
+                                    "all SMs), executed flops / CUDA-event time",
+                     "peak_derived": FP64_PEAK_DERIVED_TFLOPS,
+                     "fp64_probe_tflops": probe,
                      "flops_per_launch_algorithmic": alg_flops,
                      "flops_per_launch_executed": flops["product_executed"] * V,
                      "achieved_executed": flops["product_executed"] * V / prod_avg_s / 1e12,
-                     "frac_executed": flops["product_executed"] * V / prod_avg_s / 1e12 / FP64_PEAK_TFLOPS,
+                     "frac_executed": flops["product_executed"] * V / prod_avg_s / 1e12 / peak,
                      "kernel_ms": prod_avg_s * 1e3,
                      "note": "achieved/frac use SURVEY 8(d)'s standard count (256 x sum K_d x 8 flop per site); the kernel "
                              "evaluates about half of it (shared elementary correlators, source- and sink-swap relations), "
@@ -303,7 +343,7 @@ def main():
         line["e2e"] = {"value": world * e2e["steps"] / (e2e["ms"] * 1e-3), "unit": UNIT,
                        "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
     if world == 1 and not args.no_cpu_baseline:
-        leg = oracle_leg(args.oracle_sample_L, args.config, 1, 0)
+        leg = oracle_leg(args.oracle_sample_L or 6, args.config, 1, 0)
         line["cpu_baseline"] = {k: leg[k] for k in ("value", "unit", "cores", "kind", "sample")}
     ctx.close()
     print(json.dumps(line))

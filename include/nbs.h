@@ -72,12 +72,16 @@ enum {
  * nbs_create -- build the diagram tables (the paper's CPU "diagramatical classification", SoA
  * tables copied to the device before the kernels) and allocate the workspace.
  *   out       : receives the context (library-owned; free with nbs_destroy).
- *   L, T      : spatial extent (2 <= L <= 64, FFT path: any L; radix-2 fast path for powers of 2)
- *               and number of time slices (labels only: slices are independent).
+ *   L, T      : spatial extent: 2 <= L <= 64, or L = 3 * 2^k <= 96 (in-register radix-2 FFT for powers of two up to
+ *               32, the same behind a radix-3 stage for 6, 12, 24, 48, 96, an O(L^2) transform per axis otherwise),
+ *               and number of time slices (labels only: slices are independent).  With the 52 channels the
+ *               resident plan needs 1.4 MB of workspace per site (46 GB at 32^3); larger lattices take the tile-wise
+ *               plan (nbs_tiled_info), which needs about 2 x 55.7 KB per site plus the channels of one sink pair.
  *   ch, nch   : channel list (host memory, copied).  ch == NULL selects the standard 52 channels
  *               "from NN to Xi-Xi" in the order of DESIGN.md reading A10.
  *   device    : CUDA device ordinal.
- *   workspace_budget_bytes : upper bound for library-owned device memory (0 = no bound).
+ *   workspace_budget_bytes : upper bound for library-owned device memory (0 = no bound).  Two workspaces (two time
+ *               slices in flight) if they fit, else one, else the tile-wise plan, else NBS_ENOMEM.
  * Errors: NBS_EINVAL (bad L/T/id, or a channel whose sink and source flavour content differ for
  * every elementary source term: F would vanish identically), NBS_ENOMEM, NBS_ECUDA.
  */
@@ -120,6 +124,27 @@ int nbs_correlator(nbs_ctx* ctx, int t, int ch_begin, int ch_end, void* out, siz
 
 /* nbs_destroy -- synchronise the device, free tables and workspace.  NULL is a no-op. */
 void nbs_destroy(nbs_ctx* ctx);
+
+/*
+ * nbs_num_slots -- number of workspace slots (time slices that can be in flight at once): 2 when two
+ * workspaces fit the budget / the free device memory and T >= 2, else 1.  Slice t uses slot t % nbs_num_slots.
+ * Sharing a slot is safe: every call that touches a slot on another stream than the previous call on that slot
+ * first makes its stream wait (cudaStreamWaitEvent) for that call, so slices that share a slot serialise; a
+ * caller that wants overlap uses one stream per slot.
+ */
+int nbs_num_slots(const nbs_ctx* ctx);
+
+/*
+ * nbs_tiled_info -- which plan nbs_create chose.  Returns 0 for the resident plan (the momentum-space normal blocks
+ * of a whole time slice live in device memory: every lattice up to 32^3 with the 52 channels on a B200) and 1 for
+ * the tile-wise plan (BASELINE.json configs[4], 96^3: "blocks must be contracted tile-wise"), taken when the
+ * resident workspace does not fit workspace_budget_bytes / the free device memory.  Tile-wise, the momentum-space
+ * blocks exist only as chunks of two sink-spin planes of one baryon (49 GB at 96^3), built on demand and cached in
+ * *chunk_slots buffers; nbs_correlator then runs sink pair by sink pair and plane pair by plane pair, and a channel
+ * range should cover whole sink pairs (consecutive channels of the standard list) to avoid recomputation.  Results
+ * are the same as with the resident plan.  *chunk_builds counts the chunks built so far.  Either pointer may be NULL.
+ */
+int nbs_tiled_info(const nbs_ctx* ctx, int* chunk_slots, long long* chunk_builds);
 
 /* Helpers. */
 const char* nbs_last_error(const nbs_ctx* ctx); /* never NULL; ctx == NULL -> last nbs_create error */
@@ -189,6 +214,17 @@ int nbs_set_direct(nbs_ctx* ctx, int enable);
 int nbs_stage_times(nbs_ctx* ctx, double* ms, long long* calls, int reset);
 
 int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);
+
+/*
+ * nbs_probe_fp64 -- FP64 throughput of this device for register-resident instruction mixes (DESIGN.md section 7:
+ * the measured denominator of the product kernel's roofline fraction).  Synchronous; runs `iters` iterations of
+ *   mode 0: 16 DMMA.8x8x4      mode 1: 16 DFMA      mode 2: 16 DADD
+ *   mode 3: 12 DMMA + 12 DADD  (one k-step of the 16x16 accumulator class of the product kernel)
+ *   mode 4: 16 DMMA + 24 DADD  (one k-step of the 64x4 class)
+ * per warp on 16 warps per SM, all SMs.  *tflops = executed FP64 flops per second / 1e12 (a DMMA counts
+ * 8*8*4*2 = 512, a DFMA 64, a DADD 32 per warp instruction); *ms = duration of the timed launch.  Either may be NULL.
+ */
+int nbs_probe_fp64(nbs_ctx* ctx, int mode, int iters, double* tflops, double* ms);
 int nbs_fft3d(nbs_ctx* ctx, void* data_dev, size_t R, int inverse, void* stream);
 long long nbs_kernel_launches(const nbs_ctx* ctx);
 

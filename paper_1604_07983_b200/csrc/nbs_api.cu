@@ -9,6 +9,7 @@
 
 #include "nbs_kernels.cuh"
 #include "nbs_product.cuh"
+#include "nbs_probe.cuh"
 #include "nbs_tables.hpp"
 
 using namespace nbs;
@@ -28,6 +29,11 @@ struct Slice {
     double2* Ft = nullptr; // [V][nch][256]
     double2* scratch = nullptr;            // [grid][PROD_NBUF][max_pair_units][256] unit results
     unsigned long long* counter = nullptr; // work-item counter of the persistent product kernel
+    // in-flight guard: `done` is recorded on the stream of the last call that touched this slot; a call
+    // that arrives on another stream first makes its stream wait for it (slices that share a slot serialise)
+    cudaEvent_t done = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool busy = false;
 };
 
 } // namespace
@@ -53,6 +59,20 @@ struct nbs_ctx {
     int* d_qorder = nullptr;
     int prod_grid = 0;
     bool direct = false; // nbs_set_direct: eq. 2.4 as a shifted sum in x-space (tiny lattices)
+    // Tile-wise plan (BASELINE.json configs[4], 96^3): chosen by nbs_create when the resident
+    // workspace does not fit.  A chunk = two sink-spin planes of one baryon for all momenta, [V][2 * SM_PLANE],
+    // built on demand (k_blocks in plane-pair mode, forward FFT, expansion) and cached; the product kernel runs
+    // once per (sink pair, plane pair of B~1, plane pair of B~2).
+    bool tiled = false;
+    struct Chunk { double2* buf = nullptr; int slot = -1, pp = -1; long long stamp = 0; };
+    std::vector<Chunk> chunks;
+    long long chunk_clock = 0, chunk_builds = 0;
+    int* d_gather_pp[2] = {nullptr, nullptr};
+    int* d_qorder_all = nullptr;  // every momentum, q and -q adjacent
+    int* d_qorder_half = nullptr; // the momenta q <= -q
+    long long ntasks_half = 0;
+    size_t ft_rows = 0;           // rows of Ft per momentum (tile-wise plan: most channels of one sink pair)
+    double2* stage_out = nullptr; // tile-wise plan, host output: one channel [256][V]
     long long ntasks = 0;   // entries of d_qorder
     long long nselfconj = 0; // momenta with q == -q
     int* d_baryon_of_slot = nullptr;
@@ -100,12 +120,18 @@ struct StageTimer { // brackets the launches of one stage with two events on `st
     static cudaEvent_t get(nbs_ctx* c) {
         if (!c->event_pool.empty()) { cudaEvent_t e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
         cudaEvent_t e = nullptr;
-        cudaEventCreate(&e);
+        if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
         return e;
     }
     StageTimer(nbs_ctx* c_, int stage_, cudaStream_t st_) : c(c_), stage(stage_), st(st_) {
         if (!c->timing) return;
         a = get(c); b = get(c);
+        if (!a || !b) { // no event: this stage execution is not timed
+            if (a) c->event_pool.push_back(a);
+            if (b) c->event_pool.push_back(b);
+            a = b = nullptr;
+            return;
+        }
         cudaEventRecord(a, st);
     }
     ~StageTimer() {
@@ -135,10 +161,34 @@ int dev_alloc(nbs_ctx* c, double2*& dst, size_t ncomplex) {
     return NBS_OK;
 }
 
+bool fft_r3(int L) { // 3 * 2^k, k = 1..5: the decimation-by-3 kernel
+    if (L % 3) return false;
+    const int m = L / 3;
+    return m == 2 || m == 4 || m == 8 || m == 16 || m == 32;
+}
+
+template <int L2, bool INV>
+void launch_r3(double2* data, size_t R, size_t Rn, int axis, const double2* tw, double scale, cudaStream_t st) {
+    dim3 grid((unsigned)((Rn + FFT_R3_COMPS - 1) / FFT_R3_COMPS), (unsigned)(9 * L2 * L2));
+    k_fft_axis_r3<L2, INV><<<grid, dim3(FFT_R3_COMPS, 3), fft_r3_smem_bytes<L2>(), st>>>(data, R, Rn, axis, tw, scale);
+}
+
 template <bool INV>
 int launch_fft_axis(nbs_ctx* c, double2* data, size_t R, int axis, double scale, cudaStream_t st, size_t Rn = 0) {
     const int L = c->L;
     if (Rn == 0) Rn = R; // Rn: number of (leading) components to transform; R: row length
+    if (fft_r3(L)) {
+        switch (L / 3) {
+        case 2: launch_r3<2, INV>(data, R, Rn, axis, c->d_tw, scale, st); break;
+        case 4: launch_r3<4, INV>(data, R, Rn, axis, c->d_tw, scale, st); break;
+        case 8: launch_r3<8, INV>(data, R, Rn, axis, c->d_tw, scale, st); break;
+        case 16: launch_r3<16, INV>(data, R, Rn, axis, c->d_tw, scale, st); break;
+        default: launch_r3<32, INV>(data, R, Rn, axis, c->d_tw, scale, st); break;
+        }
+        CU(c, cudaGetLastError());
+        ++c->launches;
+        return NBS_OK;
+    }
     dim3 grid((unsigned)((Rn + FFT_THREADS - 1) / FFT_THREADS), (unsigned)(L * L));
     switch (L) {
     case 2: k_fft_axis_pow2<2, INV><<<grid, FFT_THREADS, 0, st>>>(data, R, Rn, axis, c->d_tw, scale); break;
@@ -193,14 +243,147 @@ int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st, do
 }
 
 int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, const int2* d_info, int nslots, unsigned dq_mask,
-                  double2* out, size_t row_stride, cudaStream_t st) {
+                  double2* out, size_t row_stride, cudaStream_t st, int pp = -1) {
     int ndq = 0;
     for (int b = 0; b < 9; ++b) ndq += (dq_mask >> b) & 1u;
     if (nslots > BLOCKS_MAX_SLOTS) return fail(c, NBS_EINVAL, "too many block slots");
     k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, blocks_smem_bytes(ndq), st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask,
-                                                                          c->d_brec, c->d_bterm, d_info, out, row_stride);
+                                                                          c->d_brec, c->d_bterm, d_info, out, row_stride, pp);
     CU(c, cudaGetLastError());
     ++c->launches;
+    return NBS_OK;
+}
+
+// In-flight guard of a workspace slot (include/nbs.h, nbs_num_slots): order this call after whatever the slot
+// was last used for when that happened on another stream.
+int slot_acquire(nbs_ctx* c, Slice& sl, cudaStream_t st) {
+    if (sl.busy && sl.last_stream != st) CU(c, cudaStreamWaitEvent(st, sl.done, 0));
+    return NBS_OK;
+}
+int slot_release(nbs_ctx* c, Slice& sl, cudaStream_t st) {
+    CU(c, cudaEventRecord(sl.done, st));
+    sl.last_stream = st;
+    sl.busy = true;
+    return NBS_OK;
+}
+
+
+// ---- tile-wise plan ---------------------------------------------------------------------------
+// Chunk (slot, pp) of the loaded slice: k_blocks in plane-pair mode writes the two sink-spin planes (staged for a
+// block without antisymmetry, compact for an antisymmetric one) into rows of 2 * SM_PLANE entries, the forward
+// FFT transforms them in place, k_expand_chunk restores the mirror entries of an antisymmetric block in place.
+int get_chunk(nbs_ctx* c, Slice& sl, int slot, int pp, int protect, cudaStream_t st, int* index) {
+    for (size_t i = 0; i < c->chunks.size(); ++i)
+        if (c->chunks[i].slot == slot && c->chunks[i].pp == pp) {
+            c->chunks[i].stamp = ++c->chunk_clock;
+            *index = (int)i;
+            return NBS_OK;
+        }
+    int victim = -1;
+    for (size_t i = 0; i < c->chunks.size(); ++i) {
+        if ((int)i == protect) continue;
+        if (victim < 0 || c->chunks[i].slot < 0 ||
+            (c->chunks[victim].slot >= 0 && c->chunks[i].stamp < c->chunks[victim].stamp))
+            victim = (int)i;
+        if (c->chunks[victim].slot < 0) break;
+    }
+    nbs_ctx::Chunk& ck = c->chunks[victim];
+    const int baryon = c->plan.baryons[slot], kind = c->plan.slot_kind[slot];
+    const size_t R = 2 * SM_PLANE;
+    int rc;
+    {
+        StageTimer tm(c, NBS_STAGE_BLOCKS, st);
+        rc = launch_blocks(c, sl, c->d_one_baryon + baryon, c->d_one_slot_info + baryon, 1, c->dq_mask_of[baryon], ck.buf, R, st, pp);
+        if (rc) return rc;
+    }
+    {
+        StageTimer tm(c, NBS_STAGE_FFT_FWD, st);
+        rc = fft3d(c, ck.buf, R, false, st, nullptr, kind == BK_FULL ? R : (size_t)(2 * AS_PLANE));
+        if (rc) return rc;
+        if (kind != BK_FULL) {
+            k_expand_chunk<<<(unsigned)c->V, 256, 0, st>>>(ck.buf, c->d_gather_pp[kind - 1]);
+            CU(c, cudaGetLastError());
+            ++c->launches;
+        }
+    }
+    ck.slot = slot; ck.pp = pp; ck.stamp = ++c->chunk_clock;
+    ++c->chunk_builds;
+    *index = victim;
+    return NBS_OK;
+}
+
+// nbs_correlator with the tile-wise plan: sink pair by sink pair (in chain order, so that consecutive pairs share
+// chunks), each as up to four launches of the product kernel, one per (plane pair of B~1, plane pair of B~2);
+// then the inverse FFT of the pair's channels and their final layout in the caller's buffer.
+int correlator_tiled(nbs_ctx* c, Slice& sl, int ch_begin, int ch_end, void* out, int memloc, cudaStream_t st) {
+    const Plan& P = c->plan;
+    const size_t chan_elems = 256 * c->V;
+    if (memloc == NBS_MEM_HOST && !c->stage_out) {
+        int rc = dev_alloc(c, c->stage_out, chan_elems);
+        if (rc) return rc;
+    }
+    for (int ci = 0; ci < P.chain_full_n; ++ci) {
+        const int ip = P.chain[ci].pair;
+        const Pair3Rec& pr = P.pairs3[ip];
+        bool wanted = false;
+        for (int k = 0; k < pr.nchan; ++k) {
+            const int ch = P.pair_chans[pr.chan_begin + k].ch;
+            wanted = wanted || (ch >= ch_begin && ch < ch_end);
+        }
+        if (!wanted) continue;
+        // plane-pair tiles; for identical sink baryons (1,0) follows from (0,1) by the sink swap (reading A11)
+        static const int tiles[4][2] = {{0, 0}, {0, 1}, {1, 1}, {1, 0}};
+        const int ntiles = pr.self_swap ? 3 : 4;
+        for (int it = 0; it < ntiles; ++it) {
+            const int ti = tiles[it][0], tj = tiles[it][1];
+            int i1 = -1, i2 = -1;
+            int rc = get_chunk(c, sl, pr.slot1, ti, -1, st, &i1);
+            if (rc) return rc;
+            rc = get_chunk(c, sl, pr.slot2, tj, i1, st, &i2);
+            if (rc) return rc;
+            StageTimer tm(c, NBS_STAGE_PRODUCT, st);
+            CU(c, cudaMemsetAsync(sl.counter, 0, sizeof(unsigned long long), st));
+            ProdArgs pa;
+            pa.Bc = nullptr; pa.Rc = 0; pa.Be = nullptr; pa.Re = 0; pa.L = c->L;
+            pa.slot_src = reinterpret_cast<const int2*>(c->d_slot_src);
+            pa.chain_full_n = P.chain_full_n; pa.chain_half_n = P.chain_half_n;
+            const bool half = pr.self_swap && ti == tj; // the momenta q <= -q, mirrored to -q by the epilogue
+            pa.ntasks = half ? c->ntasks_half : (long long)c->V;
+            pa.qorder = half ? c->d_qorder_half : c->d_qorder_all;
+            pa.direct = 0;
+            pa.pairs = c->d_pairs3; pa.units = c->d_units3; pa.diags = c->d_diags3;
+            pa.tab = reinterpret_cast<const uint2*>(c->d_tab3);
+            pa.pair_chans = c->d_pair_chans; pa.chain = c->d_chain;
+            pa.scratch = sl.scratch; pa.max_pair_units = P.max_pair_units;
+            pa.Ft = sl.Ft; pa.ch_begin = 0; pa.nch_out = pr.nchan;
+            pa.counter = sl.counter;
+            pa.c1 = c->chunks[i1].buf; pa.c2 = c->chunks[i2].buf;
+            pa.tile_i = ti; pa.tile_j = tj; pa.chain_base = P.chain_single_begin + ip;
+            unsigned grid = (unsigned)std::min<long long>(c->prod_grid, pa.ntasks);
+            k_product_t<true><<<grid, PROD_THREADS, PROD_SMEM, st>>>(pa);
+            CU(c, cudaGetLastError());
+            ++c->launches;
+        }
+        const size_t ld = (size_t)pr.nchan * 256;
+        {
+            StageTimer tm(c, NBS_STAGE_FFT_INV, st);
+            int rc = fft3d(c, sl.Ft, ld, true, st);
+            if (rc) return rc;
+        }
+        StageTimer tm(c, NBS_STAGE_OUTPUT, st);
+        for (int k = 0; k < pr.nchan; ++k) {
+            const PairChanRec& pc = P.pair_chans[pr.chan_begin + k];
+            if (pc.ch < ch_begin || pc.ch >= ch_end) continue;
+            double2* dst = memloc == NBS_MEM_HOST ? c->stage_out : (double2*)out + (size_t)(pc.ch - ch_begin) * chan_elems;
+            dim3 tg((unsigned)((c->V + 31) / 32), 8);
+            k_transpose_out<<<tg, 256, 0, st>>>(sl.Ft + (size_t)pc.local * 256, c->V, 256, ld, dst);
+            CU(c, cudaGetLastError());
+            ++c->launches;
+            if (memloc == NBS_MEM_HOST)
+                CU(c, cudaMemcpyAsync((double2*)out + (size_t)(pc.ch - ch_begin) * chan_elems, dst, chan_elems * sizeof(double2),
+                                      cudaMemcpyDeviceToHost, st));
+        }
+    }
     return NBS_OK;
 }
 
@@ -230,7 +413,8 @@ int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long lo
 int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int device, size_t budget) {
     if (!out) return fail(nullptr, NBS_EINVAL, "out is NULL");
     *out = nullptr;
-    if (L < 2 || L > FFT_MAXL) return fail(nullptr, NBS_EINVAL, "L must be in [2, 64]");
+    if (L < 2 || (L > FFT_MAXL && !fft_r3(L)))
+        return fail(nullptr, NBS_EINVAL, "L must be in [2, 64] or 3 * 2^k <= 96");
     if (T < 1) return fail(nullptr, NBS_EINVAL, "T must be >= 1");
     if (ch && nch < 1) return fail(nullptr, NBS_EINVAL, "nch must be >= 1");
     std::vector<nbs_channel> chans = ch ? std::vector<nbs_channel>(ch, ch + nch) : standard_channels();
@@ -310,6 +494,19 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         c->nselfconj = 0;
         for (size_t q = 0; q < c->V; ++q) c->nselfconj += neg(q) == q;
         CUC(upload(c, c->d_qorder, qorder));
+        std::vector<int> qall, qhalf;
+        std::fill(seen.begin(), seen.end(), 0);
+        for (size_t q = 0; q < c->V; ++q) {
+            if (seen[q]) continue;
+            const size_t m = neg(q);
+            qall.push_back((int)q); qhalf.push_back((int)q); seen[q] = 1;
+            if (!seen[m]) { qall.push_back((int)m); seen[m] = 1; }
+        }
+        c->ntasks_half = (long long)qhalf.size();
+        CUC(upload(c, c->d_qorder_all, qall));
+        CUC(upload(c, c->d_qorder_half, qhalf));
+        CUC(upload(c, c->d_gather_pp[0], c->plan.gather_pp[0]));
+        CUC(upload(c, c->d_gather_pp[1], c->plan.gather_pp[1]));
     }
     {
         cudaDeviceProp prop;
@@ -351,22 +548,48 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     size_t avail = (size_t)(0.92 * (double)free_b);
     if (budget && budget < avail + c->workspace) avail = budget > c->workspace ? budget - c->workspace : 0;
     c->nslices = (T >= 2 && 2 * per_slice <= avail) ? 2 : 1;
+    c->ft_rows = nchan;
+    size_t chunk_elems = 0;
     if (per_slice > avail) {
-        g_create_error = "workspace of " + std::to_string(per_slice) + " bytes per time slice does not fit (" +
-                         std::to_string(avail) + " available)";
-        nbs_destroy(c);
-        return NBS_ENOMEM;
+        // tile-wise plan: chunks of two sink-spin planes, Ft for the channels of one sink pair, at least two chunks
+        size_t maxchan = 1;
+        for (auto& pr : c->plan.pairs3) maxchan = std::max<size_t>(maxchan, (size_t)pr.nchan);
+        chunk_elems = c->V * (size_t)(2 * SM_PLANE);
+        const size_t fixed = (c->V * maxchan * 256 + scratch_elems + 1) * sizeof(double2);
+        const size_t chunk_bytes = chunk_elems * sizeof(double2);
+        const size_t nfit = avail > fixed ? (avail - fixed) / chunk_bytes : 0;
+        if (nfit < 2) {
+            g_create_error = "neither the resident workspace (" + std::to_string(per_slice) + " bytes per time slice) nor the "
+                             "tile-wise plan (" + std::to_string(fixed + 2 * chunk_bytes) + " bytes) fits (" +
+                             std::to_string(avail) + " available)";
+            nbs_destroy(c);
+            return NBS_ENOMEM;
+        }
+        c->tiled = true;
+        c->nslices = 1;
+        c->ft_rows = maxchan;
+        c->chunks.resize(std::min<size_t>(nfit, 2 * c->plan.baryons.size()));
     }
     for (int i = 0; i < c->nslices; ++i) {
-        CUC(dev_alloc(c, c->slice[i].B, c->V * c->R));
-        CUC(dev_alloc(c, c->slice[i].Be, std::max<size_t>(c->V * c->Re, 1)));
-        CUC(dev_alloc(c, c->slice[i].Ft, c->V * nchan * 256));
+        if (!c->tiled) {
+            CUC(dev_alloc(c, c->slice[i].B, c->V * c->R));
+            CUC(dev_alloc(c, c->slice[i].Be, std::max<size_t>(c->V * c->Re, 1)));
+        } else {
+            for (auto& ck : c->chunks) CUC(dev_alloc(c, ck.buf, chunk_elems));
+        }
+        CUC(dev_alloc(c, c->slice[i].Ft, c->V * c->ft_rows * 256));
         CUC(dev_alloc(c, c->slice[i].scratch, scratch_elems));
         double2* cnt = nullptr;
         CUC(dev_alloc(c, cnt, 1));
         c->slice[i].counter = (unsigned long long*)cnt;
+        CUX(cudaEventCreateWithFlags(&c->slice[i].done, cudaEventDisableTiming));
     }
-    CUX(cudaFuncSetAttribute(k_product, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
+    CUX(cudaFuncSetAttribute(k_product_t<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
+    CUX(cudaFuncSetAttribute(k_product_t<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
+    CUX(cudaFuncSetAttribute(k_fft_axis_r3<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<32>()));
+    CUX(cudaFuncSetAttribute(k_fft_axis_r3<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<32>()));
+    CUX(cudaFuncSetAttribute(k_fft_axis_r3<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<16>()));
+    CUX(cudaFuncSetAttribute(k_fft_axis_r3<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<16>()));
     CUX(cudaFuncSetAttribute(k_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)blocks_smem_bytes(9)));
     CUX(cudaFuncSetAttribute(k_fft_xy<32, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_xy_smem_bytes<32>()));
     CUX(cudaFuncSetAttribute(k_fft_xy<16, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_xy_smem_bytes<16>()));
@@ -385,6 +608,10 @@ int nbs_load_propagators(nbs_ctx* c, int t, const void* u, const void* d, const 
     cudaStream_t st = (cudaStream_t)stream;
     Slice& sl = c->slice[t % c->nslices];
     const void* src[3] = {u, d, s};
+    {
+        int rc = slot_acquire(c, sl, st);
+        if (rc) return rc;
+    }
     if (memloc == NBS_MEM_DEVICE) {
         for (int f = 0; f < 3; ++f) sl.S[f] = (const double2*)src[f];
     } else {
@@ -403,8 +630,11 @@ int nbs_load_propagators(nbs_ctx* c, int t, const void* u, const void* d, const 
         }
     }
     sl.t = t;
-    return NBS_OK;
+    for (auto& ck : c->chunks) ck.slot = ck.pp = -1; // chunks of the previous slice are stale
+    return slot_release(c, sl, st);
 }
+
+int nbs_num_slots(const nbs_ctx* c) { return c ? c->nslices : NBS_EINVAL; }
 
 int nbs_blocks_x(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes, void* stream) {
     if (!c) return NBS_EINVAL;
@@ -419,18 +649,22 @@ int nbs_blocks_x(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes,
     cudaStream_t st = (cudaStream_t)stream;
     double2* tmp = nullptr;
     const int kind = block_kind(baryon);
-    CU(c, cudaMalloc((void**)&tmp, c->V * (size_t)block_elems(kind) * sizeof(double2)));
-    int rc = launch_blocks(c, sl, c->d_one_baryon + baryon, c->d_one_slot_info + baryon, 1, c->dq_mask_of[baryon], tmp,
-                           (size_t)block_elems(kind), st);
+    int rc = slot_acquire(c, sl, st);
+    if (rc) return rc;
+    // stream-ordered temporary: no device-wide synchronisation, freed when the stream has passed the kernels
+    CU(c, cudaMallocAsync((void**)&tmp, c->V * (size_t)block_elems(kind) * sizeof(double2), st));
+    rc = launch_blocks(c, sl, c->d_one_baryon + baryon, c->d_one_slot_info + baryon, 1, c->dq_mask_of[baryon], tmp,
+                       (size_t)block_elems(kind), st);
     if (rc == NBS_OK) {
         const size_t n = c->V * (size_t)BLOCK_ELEMS;
         k_unstage<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(tmp, c->V, kind, (double2*)out_dev);
         ++c->launches;
-        cudaError_t e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(c, e, "nbs_blocks_x"); }
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) rc = cuda_fail(c, e, "nbs_blocks_x");
     }
-    cudaFree(tmp);
-    return rc;
+    CU(c, cudaFreeAsync(tmp, st));
+    if (rc) return rc;
+    return slot_release(c, sl, st);
 }
 
 int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_t out_bytes, int memloc, void* stream) {
@@ -447,6 +681,25 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     if (sl.t != t) return fail(c, NBS_ESTATE, "time slice not loaded");
     CU(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)stream;
+    // host output: the result is staged in a block buffer (free again after the product) and copied back; the
+    // range must fit BEFORE anything is enqueued
+    if (c->tiled) {
+        int rc0 = slot_acquire(c, sl, st);
+        if (rc0) return rc0;
+        rc0 = correlator_tiled(c, sl, ch_begin, ch_end, out, memloc, st);
+        if (rc0) return rc0;
+        return slot_release(c, sl, st);
+    }
+    double2* dst = (double2*)out;
+    if (memloc == NBS_MEM_HOST) {
+        if (need <= c->V * c->R * sizeof(double2)) dst = sl.B;
+        else if (need <= c->V * c->Re * sizeof(double2)) dst = sl.Be;
+        else return fail(c, NBS_ENOMEM, "channel range too large for the device staging of a host output; use a smaller range");
+    }
+    {
+        int rc0 = slot_acquire(c, sl, st);
+        if (rc0) return rc0;
+    }
 
     // isospin-limit fast path: the caller passed the same array for u and d
     const bool iso = sl.S[0] == sl.S[1] && c->plan.n_slots_iso < (int)c->plan.baryons.size();
@@ -488,17 +741,12 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         pa.Ft = sl.Ft; pa.ch_begin = ch_begin; pa.nch_out = (int)nout;
         pa.counter = sl.counter;
         unsigned grid = (unsigned)std::min<long long>(c->prod_grid, pa.ntasks);
-        k_product<<<grid, PROD_THREADS, PROD_SMEM, st>>>(pa);
+        pa.c1 = pa.c2 = nullptr; pa.tile_i = pa.tile_j = 0; pa.chain_base = 0;
+        k_product_t<false><<<grid, PROD_THREADS, PROD_SMEM, st>>>(pa);
         CU(c, cudaGetLastError());
         ++c->launches;
     }
     // inverse FFT and final layout F[ch][a1 a2 a3 a4][r]
-    double2* dst = (double2*)out;
-    if (memloc == NBS_MEM_HOST) { // a block buffer is free again: device staging for the host copy
-        if (need <= c->V * c->R * sizeof(double2)) dst = sl.B;
-        else if (need <= c->V * c->Re * sizeof(double2)) dst = sl.Be;
-        else return fail(c, NBS_ENOMEM, "channel range too large for the device staging of a host output; use a smaller range");
-    }
     const bool fused = fft_fused(c) && !c->direct;
     if (!c->direct) {
         StageTimer tm(c, NBS_STAGE_FFT_INV, st);
@@ -508,17 +756,18 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     if (!fused) {
         StageTimer tm(c, NBS_STAGE_OUTPUT, st);
         dim3 tg((unsigned)((c->V + 31) / 32), (unsigned)((nout * 256 + 31) / 32));
-        k_transpose_out<<<tg, 256, 0, st>>>(sl.Ft, c->V, nout * 256, dst);
+        k_transpose_out<<<tg, 256, 0, st>>>(sl.Ft, c->V, nout * 256, nout * 256, dst);
         CU(c, cudaGetLastError());
         ++c->launches;
     }
     if (memloc == NBS_MEM_HOST) CU(c, cudaMemcpyAsync(out, dst, need, cudaMemcpyDeviceToHost, st));
-    return NBS_OK;
+    return slot_release(c, sl, st);
 }
 
 int nbs_set_direct(nbs_ctx* c, int enable) {
     if (!c) return NBS_EINVAL;
     if (enable && c->L > 8) return fail(c, NBS_EINVAL, "the direct shifted sum is O(V^2): allowed for L <= 8 only");
+    if (enable && c->tiled) return fail(c, NBS_EINVAL, "the direct shifted sum is not available with the tile-wise plan");
     c->direct = enable != 0;
     return NBS_OK;
 }
@@ -557,6 +806,7 @@ void nbs_destroy(nbs_ctx* c) {
         for (void* p : c->allocs) cudaFree(p);
         for (auto& p : c->pending) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
         for (cudaEvent_t e : c->event_pool) cudaEventDestroy(e);
+        for (auto& sl : c->slice) if (sl.done) cudaEventDestroy(sl.done);
     }
     delete c;
 }
@@ -605,5 +855,50 @@ int nbs_fft3d(nbs_ctx* c, void* data_dev, size_t R, int inverse, void* stream) {
 }
 
 long long nbs_kernel_launches(const nbs_ctx* c) { return c ? c->launches : 0; }
+
+int nbs_tiled_info(const nbs_ctx* c, int* chunk_slots, long long* chunk_builds) {
+    if (!c) return NBS_EINVAL;
+    if (chunk_slots) *chunk_slots = (int)c->chunks.size();
+    if (chunk_builds) *chunk_builds = c->chunk_builds;
+    return c->tiled ? 1 : 0;
+}
+
+int nbs_probe_fp64(nbs_ctx* c, int mode, int iters, double* tflops, double* ms_out) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    if (mode < 0 || mode > 4 || iters < 1) return fail(c, NBS_EINVAL, "nbs_probe_fp64: mode in [0, 4], iters >= 1");
+    CU(c, cudaSetDevice(c->device));
+    cudaEvent_t a = nullptr, b = nullptr;
+    CU(c, cudaEventCreate(&a));
+    CU(c, cudaEventCreate(&b));
+    double* sink = reinterpret_cast<double*>(c->slice[0].scratch); // never written (the guard in the kernel is false)
+    const unsigned grid = (unsigned)c->prod_grid;
+    auto launch = [&](int n) {
+        switch (mode) {
+        case 0: k_probe_fp64<0><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        case 1: k_probe_fp64<1><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        case 2: k_probe_fp64<2><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        case 3: k_probe_fp64<3><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        default: k_probe_fp64<4><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        }
+    };
+    launch(iters / 8 + 1); // warm-up
+    CU(c, cudaEventRecord(a, 0));
+    launch(iters);
+    CU(c, cudaEventRecord(b, 0));
+    cudaError_t e = cudaEventSynchronize(b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    if (e != cudaSuccess) return cuda_fail(c, e, "nbs_probe_fp64");
+    c->launches += 2;
+    // per warp instruction: DMMA.8x8x4 = 8*8*4 FMA = 512 flop, DFMA = 32 lanes x 2, DADD = 32 lanes x 1
+    const double per_iter = 512.0 * probe_dmma(mode) + 64.0 * probe_dfma(mode) + 32.0 * probe_dadd(mode);
+    const double warps = (double)grid * (PROBE_THREADS / 32);
+    if (tflops) *tflops = per_iter * warps * (double)iters / ((double)ms * 1e-3) / 1e12;
+    if (ms_out) *ms_out = (double)ms;
+    return NBS_OK;
+}
 
 } // extern "C"

@@ -67,7 +67,11 @@ inline size_t blocks_smem_bytes(int ndq) { return (size_t)(3 * 144 + ndq * DQ_SI
 // acc[a][e0][e1][e2] += coef * sum_c D_c(xi_P0, xi_P1) * S[(c, a0 + a), xi_P2] over the thread's tile
 template <int P0, int P1, int P2>
 __device__ __forceinline__ void blocks_term(double2 (&acc)[2][2][2][2], const double2* __restrict__ Dq,
-                                            const double2* __restrict__ S2, double coef, int a0, const int (&x)[3]) {
+                                            const double2* __restrict__ S2, double coef, int a0, int x0, int x1, int x2) {
+    // tile origins as scalars selected at compile time (an int[3] indexed through the run-time switch below
+    // was placed in local memory)
+    const int xP0 = P0 == 0 ? x0 : P0 == 1 ? x1 : x2, xP1 = P1 == 0 ? x0 : P1 == 1 ? x1 : x2,
+              xP2 = P2 == 0 ? x0 : P2 == 1 ? x1 : x2;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double2 Dv[2][2], Sv[2][2];
@@ -75,12 +79,12 @@ __device__ __forceinline__ void blocks_term(double2 (&acc)[2][2][2][2], const do
         for (int ja = 0; ja < 2; ++ja)
 #pragma unroll
             for (int jb = 0; jb < 2; ++jb) // x even: dq_rank(x + j) = 6 j + x / 2
-                Dv[ja][jb] = Dq[c * DQ_C + (6 * ja + (x[P0] >> 1)) * DQ_ROW + 6 * jb + (x[P1] >> 1)];
+                Dv[ja][jb] = Dq[c * DQ_C + (6 * ja + (xP0 >> 1)) * DQ_ROW + 6 * jb + (xP1 >> 1)];
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                const double2 v = S2[(c + 3 * (a0 + a)) * 12 + 6 * j + (x[P2] >> 1)];
+                const double2 v = S2[(c + 3 * (a0 + a)) * 12 + 6 * j + (xP2 >> 1)];
                 Sv[a][j] = make_double2(coef * v.x, coef * v.y);
             }
 #pragma unroll
@@ -101,7 +105,9 @@ __global__ void __launch_bounds__(BLOCKS_THREADS, 2)
 k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const double2* __restrict__ Ss,
          const int* __restrict__ baryon_of_slot, int nslots, unsigned dq_mask,
          const BlockRec* __restrict__ brec, const BTermRec* __restrict__ bterm,
-         const int2* __restrict__ slot_info, double2* __restrict__ out, size_t row_stride) {
+         const int2* __restrict__ slot_info, double2* __restrict__ out, size_t row_stride, int pp) {
+    // pp < 0: whole blocks.  pp = 0, 1 (tile-wise plan, one slot): only the sink-spin planes {2 pp, 2 pp + 1},
+    // written as a two-plane chunk row (staged planes for a full-kind block, compact planes for an antisymmetric one)
     extern __shared__ double2 smem[];
     const int ndq = __popc(dq_mask);
     double2* sS = smem;                  // [3][144]
@@ -156,21 +162,22 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
         // one pass, 2 x 126 tiles on or above the diagonal of the antisymmetric slot pair
         const int npass = (kind == BK_FULL) ? 2 : 1;
         for (int pass = 0; pass < npass; ++pass) {
-            int x[3], a0 = 2 * pass;
+            if (pp >= 0 && kind == BK_FULL && pass != pp) continue; // uniform over the CTA
+            int x0, x1, x2, a0 = 2 * pass;
             bool active;
             if (kind == BK_FULL) {
                 active = tid < BLOCKS_TILES;
-                x[0] = 2 * (tid / 36); x[1] = 2 * ((tid / 6) % 6); x[2] = 2 * (tid % 6);
+                x0 = 2 * (tid / 36); x1 = 2 * ((tid / 6) % 6); x2 = 2 * (tid % 6);
             } else {
-                active = tid < 252;
                 const int h = tid / 126, tt = tid - h * 126;
+                active = tid < 252 && (pp < 0 || h == pp);
                 int ia = 0, rem = tt / 6;
                 while (rem >= 6 - ia) { rem -= 6 - ia; ++ia; }
                 const int ib = ia + rem, ic = tt % 6;
                 a0 = 2 * h;
-                x[2] = 2 * ib;
-                if (kind == BK_ASYM13) { x[0] = 2 * ia; x[1] = 2 * ic; }
-                else { x[1] = 2 * ia; x[0] = 2 * ic; }
+                x2 = 2 * ib;
+                if (kind == BK_ASYM13) { x0 = 2 * ia; x1 = 2 * ic; }
+                else { x1 = 2 * ia; x0 = 2 * ic; }
             }
             double2 acc[2][2][2][2];
             if (active) {
@@ -184,12 +191,12 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                     const double2* S2 = sS + bt.f2 * 144;
                     const int perm = bt.p0 * 3 + bt.p1; // (p0, p1) fixes the permutation
                     switch (perm) {
-                    case 1: blocks_term<0, 1, 2>(acc, Dq, S2, bt.coef, a0, x); break;
-                    case 2: blocks_term<0, 2, 1>(acc, Dq, S2, bt.coef, a0, x); break;
-                    case 3: blocks_term<1, 0, 2>(acc, Dq, S2, bt.coef, a0, x); break;
-                    case 5: blocks_term<1, 2, 0>(acc, Dq, S2, bt.coef, a0, x); break;
-                    case 6: blocks_term<2, 0, 1>(acc, Dq, S2, bt.coef, a0, x); break;
-                    default: blocks_term<2, 1, 0>(acc, Dq, S2, bt.coef, a0, x); break;
+                    case 1: blocks_term<0, 1, 2>(acc, Dq, S2, bt.coef, a0, x0, x1, x2); break;
+                    case 2: blocks_term<0, 2, 1>(acc, Dq, S2, bt.coef, a0, x0, x1, x2); break;
+                    case 3: blocks_term<1, 0, 2>(acc, Dq, S2, bt.coef, a0, x0, x1, x2); break;
+                    case 5: blocks_term<1, 2, 0>(acc, Dq, S2, bt.coef, a0, x0, x1, x2); break;
+                    case 6: blocks_term<2, 0, 1>(acc, Dq, S2, bt.coef, a0, x0, x1, x2); break;
+                    default: blocks_term<2, 1, 0>(acc, Dq, S2, bt.coef, a0, x0, x1, x2); break;
                     }
                 }
             }
@@ -210,7 +217,7 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                         for (int e1 = 0; e1 < 2; ++e1)
 #pragma unroll
                             for (int e2 = 0; e2 < 2; ++e2) {
-                                const int xi0 = x[0] + e0, xi1 = x[1] + e1, xi2 = x[2] + e2;
+                                const int xi0 = x0 + e0, xi1 = x1 + e1, xi2 = x2 + e2;
                                 if (kind == BK_FULL) {
                                     sO[a * SM_PLANE + sm_index(xi0, xi1, xi2)] = acc[a][e0][e1][e2];
                                 } else {
@@ -223,10 +230,11 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncthreads();
             if (tid == 0) {
-                const int n = (kind == BK_FULL) ? BLOCKS_HALF : AS_BLOCK;
-                double2* dst = orow + info.x + ((kind == BK_FULL) ? pass * BLOCKS_HALF : 0);
+                const int n = (kind == BK_FULL) ? BLOCKS_HALF : (pp < 0 ? AS_BLOCK : 2 * AS_PLANE);
+                double2* dst = orow + info.x + ((kind == BK_FULL && pp < 0) ? pass * BLOCKS_HALF : 0);
+                const double2* src = sO + ((kind != BK_FULL && pp > 0) ? 2 * AS_PLANE : 0);
                 asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n\tcp.async.bulk.commit_group;"
-                             :: "l"(dst), "r"((uint32_t)__cvta_generic_to_shared(sO)), "r"((uint32_t)(n * sizeof(double2))) : "memory");
+                             :: "l"(dst), "r"((uint32_t)__cvta_generic_to_shared(src)), "r"((uint32_t)(n * sizeof(double2))) : "memory");
             }
         }
     }
@@ -248,6 +256,25 @@ k_expand(const double2* __restrict__ compact, size_t Rc, const int* __restrict__
             if (g & (1 << 30)) { v.x = -v.x; v.y = -v.y; }
         }
         dst[j] = v;
+    }
+}
+
+// Tile-wise plan: the same expansion for a two-plane chunk, in place inside the chunk row (the compact plane pair
+// sits at the start of the row of 2 * SM_PLANE entries; Plan::gather_pp).  One CTA per site.
+__global__ void __launch_bounds__(256)
+k_expand_chunk(double2* __restrict__ chunk, const int* __restrict__ gather) {
+    __shared__ double2 buf[2 * AS_PLANE];
+    double2* row = chunk + (size_t)blockIdx.x * (2 * SM_PLANE);
+    for (int j = threadIdx.x; j < 2 * AS_PLANE; j += 256) buf[j] = row[j];
+    __syncthreads();
+    for (int j = threadIdx.x; j < 2 * SM_PLANE; j += 256) {
+        const int g = __ldg(gather + j);
+        double2 v = make_double2(0.0, 0.0);
+        if (g >= 0) {
+            v = buf[g & 0x3fffffff];
+            if (g & (1 << 30)) { v.x = -v.x; v.y = -v.y; }
+        }
+        row[j] = v;
     }
 }
 
@@ -348,6 +375,66 @@ k_fft_axis_pow2(double2* __restrict__ data, size_t R, size_t Rn, int axis, const
         double2 v = a[j];
         if (INV) { v.x *= scale; v.y *= scale; }
         data[(s0 + j * st) * R + r] = v;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// L = 3 * L2 with L2 a power of two <= 32 (6, 12, 24, 48 and the 96 of BASELINE.json configs[4]): decimation in
+// time by 3.  Three threads share one line: thread s transforms the L2 points x[3 n + s] in registers (the same
+// in-register radix-2 code), multiplies by the twiddles w_L^{s k}, and the three partial spectra meet in shared
+// memory for the radix-3 butterfly  X[k + L2 m] = sum_s w_3^{s m} (w_L^{s k} Y_s[k]); thread m writes its third
+// of the spectrum.  Lanes on consecutive components as in the power-of-two kernel: every access is coalesced.
+// tw[m] = exp(-2 pi i m / L), computed in long double on the host.
+// ---------------------------------------------------------------------------------------------
+constexpr int FFT_R3_COMPS = 64;
+template <int L2>
+constexpr size_t fft_r3_smem_bytes() { return (size_t)3 * L2 * FFT_R3_COMPS * sizeof(double2); }
+
+template <int L2, bool INV>
+__global__ void __launch_bounds__(3 * FFT_R3_COMPS, 2)
+k_fft_axis_r3(double2* __restrict__ data, size_t R, size_t Rn, int axis, const double2* __restrict__ tw, double scale) {
+    constexpr int L = 3 * L2;
+    extern __shared__ double2 smem[]; // [s][k][component]
+    const int c = threadIdx.x, s = threadIdx.y;
+    const size_t r = (size_t)blockIdx.x * FFT_R3_COMPS + c;
+    const bool live = r < Rn;
+    size_t s0, st;
+    line_geometry(L, axis, blockIdx.y, s0, st);
+    double2 a[L2];
+    if (live) {
+#pragma unroll
+        for (int n = 0; n < L2; ++n) a[n] = data[(s0 + (size_t)(3 * n + s) * st) * R + r];
+        fft_inreg<L2, INV>(a, nullptr);
+#pragma unroll
+        for (int k = 0; k < L2; ++k) {
+            double2 v = a[k];
+            if (s > 0 && k > 0) {
+                double2 w = __ldg(tw + s * k); // s k < 2 L2 < L
+                if (INV) w.y = -w.y;
+                v = cmul(v, w);
+            }
+            smem[(s * L2 + k) * FFT_R3_COMPS + c] = v;
+        }
+    }
+    __syncthreads();
+    if (!live) return;
+    // thread m = s: X[k + L2 m] = Z0 + w3^m Z1 + w3^{2m} Z2,  w3 = exp(-+ 2 pi i / 3) = -1/2 -+ i sqrt(3)/2
+    constexpr double H = 0.86602540378443864676372317075294; // sqrt(3) / 2
+    const double sg = (s == 0) ? 0.0 : ((s == 1) != INV ? -1.0 : 1.0); // sign of the i sqrt(3)/2 (Z1 - Z2) term
+#pragma unroll
+    for (int k = 0; k < L2; ++k) {
+        const double2 z0 = smem[(0 * L2 + k) * FFT_R3_COMPS + c];
+        const double2 z1 = smem[(1 * L2 + k) * FFT_R3_COMPS + c];
+        const double2 z2 = smem[(2 * L2 + k) * FFT_R3_COMPS + c];
+        const double2 t1 = cadd(z1, z2), t2 = csub(z1, z2);
+        double2 v;
+        if (s == 0) v = cadd(z0, t1);
+        else { // z0 - t1 / 2 + sg * i * H * t2,   i * t2 = (-t2.y, t2.x)
+            v.x = z0.x - 0.5 * t1.x - sg * H * t2.y;
+            v.y = z0.y - 0.5 * t1.y + sg * H * t2.x;
+        }
+        if (INV) { v.x *= scale; v.y *= scale; }
+        data[(s0 + (size_t)(k + L2 * s) * st) * R + r] = v;
     }
 }
 
@@ -453,15 +540,16 @@ k_fft_axis_generic(double2* __restrict__ data, size_t R, size_t Rn, int L, int a
     }
 }
 
-// Final layout change: Fr[r][comp] (site-major) -> out[comp][r] (r fastest), 32x32 tiles.
+// Final layout change: Fr[r][ld] (site-major, the first ncomp components of every row) -> out[comp][r]
+// (r fastest), 32x32 tiles.
 __global__ void __launch_bounds__(256)
-k_transpose_out(const double2* __restrict__ Fr, size_t V, size_t ncomp, double2* __restrict__ out) {
+k_transpose_out(const double2* __restrict__ Fr, size_t V, size_t ncomp, size_t ld, double2* __restrict__ out) {
     __shared__ double2 tile[32][33];
     const size_t r0 = (size_t)blockIdx.x * 32, c0 = (size_t)blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     for (int i = ty; i < 32; i += 8) {
         size_t r = r0 + i, c = c0 + tx;
-        if (r < V && c < ncomp) tile[i][tx] = Fr[r * ncomp + c];
+        if (r < V && c < ncomp) tile[i][tx] = Fr[r * ld + c];
     }
     __syncthreads();
     for (int i = ty; i < 32; i += 8) {

@@ -1,0 +1,78 @@
+// FP64 peak probe (nbs_probe_fp64, include/nbs.h): register-resident instruction mixes on every SM, timed with
+// CUDA events.  bench.py runs it in the same process and under the same clock sampler as the timed steps; the
+// DMMA-only figure is the denominator of `roofline.frac` for the product kernel.
+//   mode 0: DMMA.8x8x4 only            mode 1: DFMA only            mode 2: DADD only
+//   mode 3: 12 DMMA + 12 DADD  (one k-step of the 16x16 accumulator class of k_product: 8 gather subtractions,
+//           4 Gauss sums, 12 MMAs)
+//   mode 4: 16 DMMA + 24 DADD  (one k-step of the 64x4 class)
+#pragma once
+#include <cuda_runtime.h>
+
+#include "nbs_product.cuh"
+
+namespace nbs {
+
+constexpr int PROBE_THREADS = 512; // 16 warps per CTA, one CTA per SM: 4 warps per SM sub-partition
+__host__ __device__ constexpr int probe_dmma(int mode) { return mode == 0 ? 16 : mode == 3 ? 12 : mode == 4 ? 16 : 0; }
+__host__ __device__ constexpr int probe_dfma(int mode) { return mode == 1 ? 16 : 0; }
+__host__ __device__ constexpr int probe_dadd(int mode) { return mode == 2 ? 16 : mode == 3 ? 12 : mode == 4 ? 24 : 0; }
+
+template <int MODE>
+__global__ void __launch_bounds__(PROBE_THREADS, 1) k_probe_fp64(int iters, double delta, double* __restrict__ sink) {
+    const int lane = threadIdx.x & 31;
+    double acc[16][2];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { acc[i][0] = 0.0; acc[i][1] = 0.0; }
+    double v[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = 1.0 + 1e-3 * (lane + i);
+    double w[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) w[i] = 0.5 + 1e-3 * (lane - i);
+    for (int it = 0; it < iters; ++it) {
+        if (MODE == 0) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) dmma884(acc[i][0], acc[i][1], v[i & 7], v[8 + (i & 7)]);
+        } else if (MODE == 1) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) acc[i][0] = fma(v[i], delta, acc[i][0]);
+        } else if (MODE == 2) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) acc[i][0] += delta;
+        } else if (MODE == 3) {
+            // A[2], B[2] complex: 8 subtractions (eq. 4.2 gathers), 4 Gauss sums, 12 MMAs (mma_square)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = v[i] - delta;
+            const double sA0 = v[0] + v[1], sA1 = v[2] + v[3], sB0 = v[4] + v[5], sB1 = v[6] + v[7];
+            const double Ar[2] = {v[0], v[2]}, Ai[2] = {v[1], v[3]}, Br[2] = {v[4], v[6]}, Bi[2] = {v[5], v[7]};
+            const double sA[2] = {sA0, sA1}, sB[2] = {sB0, sB1};
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    dmma884(acc[(i * 2 + j) * 3 + 0][0], acc[(i * 2 + j) * 3 + 0][1], Ar[i], Br[j]);
+                    dmma884(acc[(i * 2 + j) * 3 + 1][0], acc[(i * 2 + j) * 3 + 1][1], Ai[i], Bi[j]);
+                    dmma884(acc[(i * 2 + j) * 3 + 2][0], acc[(i * 2 + j) * 3 + 2][1], sA[i], sB[j]);
+                }
+        } else {
+            // A[4][2] complex (16 subtractions), B entry (8 adds), 16 MMAs (mma_wide)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) v[i] = v[i] - delta;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) w[i] = w[i] + delta;
+            const double b1 = (w[0] + w[1]) + w[4], b2 = (w[2] + w[3]) + w[5]; // 4 + 4 adds: the 8-term B entry
+#pragma unroll
+            for (int i = 0; i < 8; ++i) dmma884(acc[i][0], acc[i][1], v[2 * i], b1);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) dmma884(acc[i][0], acc[i][1], v[2 * i + 1], b2);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += acc[i][0] + acc[i][1];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += v[i];
+    if (s == 1.2345e-300) sink[blockIdx.x * PROBE_THREADS + threadIdx.x] = s; // keeps the arithmetic alive
+}
+
+} // namespace nbs

@@ -117,16 +117,20 @@ __device__ __forceinline__ void sub_pair(const double2 (&u)[NP], const double2 (
 // Complex products with three real multiplications (Gauss): with P1 = sum Ar Br, P2 = sum Ai Bi and
 // P3 = sum (Ar + Ai)(Br + Bi), Re = P1 - P2 and Im = P3 - P1 - P2.  12 DMMAs per k-step instead of 16
 // for 4 more FP64 adds: the FP64 units (shared by DMMA and DADD) do 13 % less per k-step.
+// NT = MMA tiles per side: 2 (whole blocks staged: a1, a2 = 0..3) or 1 (tile-wise plan: one plane pair per side).
+template <int NT>
 struct AccSquare {
-    double p1[2][2][2], p2[2][2][2], p3[2][2][2];
+    double p1[NT][NT][2], p2[NT][NT][2], p3[NT][NT][2];
 };
-__device__ __forceinline__ void mma_square(AccSquare& c, const double2 (&A)[2], const double2 (&B)[2]) {
-    const double sA[2] = {A[0].x + A[0].y, A[1].x + A[1].y};
-    const double sB[2] = {B[0].x + B[0].y, B[1].x + B[1].y};
+template <int NT>
+__device__ __forceinline__ void mma_square(AccSquare<NT>& c, const double2 (&A)[NT], const double2 (&B)[NT]) {
+    double sA[NT], sB[NT];
 #pragma unroll
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < NT; ++i) { sA[i] = A[i].x + A[i].y; sB[i] = B[i].x + B[i].y; }
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
+    for (int i = 0; i < NT; ++i)
+#pragma unroll
+        for (int j = 0; j < NT; ++j) {
             dmma884(c.p1[i][j][0], c.p1[i][j][1], A[i].x, B[j].x);
             dmma884(c.p2[i][j][0], c.p2[i][j][1], A[i].y, B[j].y);
             dmma884(c.p3[i][j][0], c.p3[i][j][1], sA[i], sB[j]);
@@ -143,12 +147,14 @@ __device__ __forceinline__ Diag3Rec load_diag(const Diag3Rec* p) { // p: shared 
     return d;
 }
 
+template <bool TILE>
 __device__ __forceinline__ void run_unit_square(const Unit3Rec u, const Diag3Rec* diags,
                                                 const uint2* __restrict__ tab, const char* s1, const char* s2,
-                                                double2* __restrict__ out, int lane) {
+                                                double2* __restrict__ out, int lane, int ti, int tj) {
     const int r = lane >> 2, kk = lane & 3;
     constexpr uint32_t PS = 2 * PLANE_BYTES;
-    AccSquare acc = {};
+    constexpr int NT = TILE ? 1 : 2;
+    AccSquare<NT> acc = {};
     for (int d = u.diag_begin; d < u.diag_end; ++d) {
         const Diag3Rec dr = load_diag(diags + d);
         const int nsteps = dr.send - dr.sbeg;
@@ -158,50 +164,50 @@ __device__ __forceinline__ void run_unit_square(const Unit3Rec u, const Diag3Rec
             const uint2* tB = tab + dr.offB + (dr.sbeg * 4 + kk) * 8 + r;
             uint2 wa = __ldg(tA), wb = __ldg(tB);
             uint2 na = __ldg(tA + 32), nb = __ldg(tB + 32);
-            double2 A[2], B[2], ua[2], va[2], ub[2], vb[2];
-            ld_pair<2, PS>(s1, wa, ua, va);
-            ld_pair<2, PS>(s2, wb, ub, vb);
-            sub_pair<2, true>(ua, va, A);
-            sub_pair<2, true>(ub, vb, B);
+            double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
+            ld_pair<NT, PS>(s1, wa, ua, va);
+            ld_pair<NT, PS>(s2, wb, ub, vb);
+            sub_pair<NT, true>(ua, va, A);
+            sub_pair<NT, true>(ub, vb, B);
             for (int s = 0; s < nsteps; ++s) {
                 tA += 32; tB += 32;
                 wa = na; wb = nb;
-                ld_pair<2, PS>(s1, wa, ua, va); // one step past the end reads a valid (unused) entry
-                ld_pair<2, PS>(s2, wb, ub, vb);
+                ld_pair<NT, PS>(s1, wa, ua, va); // one step past the end reads a valid (unused) entry
+                ld_pair<NT, PS>(s2, wb, ub, vb);
                 na = __ldg(tA + 32); nb = __ldg(tB + 32);
                 prefetch_l1(tA + 5 * 32); prefetch_l1(tB + 5 * 32); // L2 latency > 2 k-steps: pull the words into L1 early
                 mma_square(acc, A, B);
-                sub_pair<2, true>(ua, va, A);
-                sub_pair<2, true>(ub, vb, B);
+                sub_pair<NT, true>(ua, va, A);
+                sub_pair<NT, true>(ub, vb, B);
             }
         } else {
             const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry)
             const uint2* tA = tab + dr.offA + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
             const uint2* tB = tab + dr.offB + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
             for (int s = 0; s < nsteps; ++s, tA += 32 * nw, tB += 32 * nw) {
-                double2 A[2], B[2], ua[2], va[2], ub[2], vb[2];
-                ld_pair<2, PS>(s1, __ldg(tA), ua, va);
-                ld_pair<2, PS>(s2, __ldg(tB), ub, vb);
-                sub_pair<2, true>(ua, va, A);
-                sub_pair<2, true>(ub, vb, B);
+                double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
+                ld_pair<NT, PS>(s1, __ldg(tA), ua, va);
+                ld_pair<NT, PS>(s2, __ldg(tB), ub, vb);
+                sub_pair<NT, true>(ua, va, A);
+                sub_pair<NT, true>(ub, vb, B);
                 for (int j = 1; j < nw; ++j) {
-                    ld_pair<2, PS>(s1, __ldg(tA + j), ua, va);
-                    ld_pair<2, PS>(s2, __ldg(tB + j), ub, vb);
-                    sub_pair<2, false>(ua, va, A);
-                    sub_pair<2, false>(ub, vb, B);
+                    ld_pair<NT, PS>(s1, __ldg(tA + j), ua, va);
+                    ld_pair<NT, PS>(s2, __ldg(tB + j), ub, vb);
+                    sub_pair<NT, false>(ua, va, A);
+                    sub_pair<NT, false>(ub, vb, B);
                 }
                 mma_square(acc, A, B);
             }
         }
     }
 #pragma unroll
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < NT; ++i)
 #pragma unroll
-        for (int j = 0; j < 2; ++j)
+        for (int j = 0; j < NT; ++j)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const int a1 = 2 * i + (r & 1), c1 = r >> 1;
-                const int cc = 2 * kk + e, a2 = 2 * j + (cc & 1), c2 = cc >> 1;
+                const int a1 = 2 * (TILE ? ti : i) + (r & 1), c1 = r >> 1;
+                const int cc = 2 * kk + e, a2 = 2 * (TILE ? tj : j) + (cc & 1), c2 = cc >> 1;
                 const int a3 = u.cls == 0 ? c1 : c2, a4 = u.cls == 0 ? c2 : c1;
                 out[((a1 * 4 + a2) * 4 + a3) * 4 + a4] =
                     make_double2(acc.p1[i][j][e] - acc.p2[i][j][e], acc.p3[i][j][e] - acc.p1[i][j][e] - acc.p2[i][j][e]);
@@ -213,26 +219,28 @@ __device__ __forceinline__ void run_unit_square(const Unit3Rec u, const Diag3Rec
 // (j, g) holds aX in {2j, 2j+1}, cX in {4g .. 4g+3}; MMA row = 2*(cX & 3) + (aX & 1).  Operand B =
 // the other effective block (n = aY).  The 8 MMA columns hold [Re | Im] of the 4 outputs:
 //   C += Ar [Br | Bi];  C += Ai [-Bi | Br].
-__device__ __forceinline__ void mma_wide(double (&acc)[8][2], const double2 (&A)[4][2], double2 Bv, int hi) {
+template <int NJ>
+__device__ __forceinline__ void mma_wide(double (&acc)[NJ * 4][2], const double2 (&A)[4][NJ], double2 Bv, int hi) {
     const double b1 = hi ? Bv.y : Bv.x;
     const double b2 = hi ? Bv.x : dneg(Bv.y);
 #pragma unroll
     for (int g = 0; g < 4; ++g)
 #pragma unroll
-        for (int j = 0; j < 2; ++j) dmma884(acc[j * 4 + g][0], acc[j * 4 + g][1], A[g][j].x, b1);
+        for (int j = 0; j < NJ; ++j) dmma884(acc[j * 4 + g][0], acc[j * 4 + g][1], A[g][j].x, b1);
 #pragma unroll
     for (int g = 0; g < 4; ++g)
 #pragma unroll
-        for (int j = 0; j < 2; ++j) dmma884(acc[j * 4 + g][0], acc[j * 4 + g][1], A[g][j].y, b2);
+        for (int j = 0; j < NJ; ++j) dmma884(acc[j * 4 + g][0], acc[j * 4 + g][1], A[g][j].y, b2);
 }
 
 // Table words of one k-step of one lane: 4 A entries (g) and the 4 term pairs of the B entry.
-__device__ __forceinline__ void wide_loads_A(const char* sA, uint4 a01, uint4 a23, double2 (&ua)[4][2], double2 (&va)[4][2]) {
+template <int NJ>
+__device__ __forceinline__ void wide_loads_A(const char* sA, uint4 a01, uint4 a23, double2 (&ua)[4][NJ], double2 (&va)[4][NJ]) {
     constexpr uint32_t PS = 2 * PLANE_BYTES;
-    ld_pair<2, PS>(sA, make_uint2(a01.x, a01.y), ua[0], va[0]);
-    ld_pair<2, PS>(sA, make_uint2(a01.z, a01.w), ua[1], va[1]);
-    ld_pair<2, PS>(sA, make_uint2(a23.x, a23.y), ua[2], va[2]);
-    ld_pair<2, PS>(sA, make_uint2(a23.z, a23.w), ua[3], va[3]);
+    ld_pair<NJ, PS>(sA, make_uint2(a01.x, a01.y), ua[0], va[0]);
+    ld_pair<NJ, PS>(sA, make_uint2(a01.z, a01.w), ua[1], va[1]);
+    ld_pair<NJ, PS>(sA, make_uint2(a23.x, a23.y), ua[2], va[2]);
+    ld_pair<NJ, PS>(sA, make_uint2(a23.z, a23.w), ua[3], va[3]);
 }
 // B entry (8 gather terms = 4 pairs): the lanes hi = 0 and hi = 1 of one (aY, k) need the same entry, so
 // each gathers two of the four pairs and the halves are exchanged with a shuffle (lane ^ 16 flips hi):
@@ -249,13 +257,18 @@ __device__ __forceinline__ void wide_fold_B(const double2 (&ub)[2][1], const dou
     Bv[0] = make_double2(part[0].x + ox, part[0].y + oy);
 }
 
+// Tile-wise plan (TILE): each side holds one plane pair.  The A side then has one MMA row tile per g (NJ = 1); the
+// lanes of the B side with aY = 2, 3 gather from planes that are not staged, and their two output columns (columns
+// of an MMA do not mix) are dropped at the flush.
+template <bool TILE>
 __device__ __forceinline__ void run_unit_wide(const Unit3Rec u, const Diag3Rec* diags,
                                               const uint2* __restrict__ tab, const char* s1, const char* s2,
-                                              double2* __restrict__ out, int lane) {
+                                              double2* __restrict__ out, int lane, int ti, int tj) {
     const int r = lane >> 2, kk = lane & 3, aY = r & 3, hi = r >> 2;
     const char* sA = (u.cls == 2) ? s1 : s2;
     const char* sB = (u.cls == 2) ? s2 : s1;
-    double acc[8][2] = {};
+    constexpr int NJ = TILE ? 1 : 2;
+    double acc[NJ * 4][2] = {};
     for (int d = u.diag_begin; d < u.diag_end; ++d) {
         const Diag3Rec dr = load_diag(diags + d); // nwA == 1, nwB == 4 (checked by the table generator)
         const int nsteps = dr.send - dr.sbeg;
@@ -265,34 +278,37 @@ __device__ __forceinline__ void run_unit_wide(const Unit3Rec u, const Diag3Rec* 
         // software pipeline: table words one k-step ahead; the A gathers of step s+1 fly under the
         // MMAs of step s, the (8-term) B gather of step s+1 is issued after them and folded at the
         // top of step s+1 (keeps the live registers under the 168 available per thread)
-        double2 A[4][2], Bv[1], ua[4][2], va[4][2], ub[2][1], vb[2][1];
-        wide_loads_A(sA, __ldg(tA), __ldg(tA + 1), ua, va);
+        double2 A[4][NJ], Bv[1], ua[4][NJ], va[4][NJ], ub[2][1], vb[2][1];
+        wide_loads_A<NJ>(sA, __ldg(tA), __ldg(tA + 1), ua, va);
         wide_loads_B(sB, __ldg(tB + hi), ub, vb);
         uint4 na01 = __ldg(tA + 64), na23 = __ldg(tA + 65), nbw = __ldg(tB + 32 + hi);
 #pragma unroll
-        for (int g = 0; g < 4; ++g) sub_pair<2, true>(ua[g], va[g], A[g]);
+        for (int g = 0; g < 4; ++g) sub_pair<NJ, true>(ua[g], va[g], A[g]);
         for (int s = 0; s < nsteps; ++s) {
             tA += 64; tB += 32;
             wide_fold_B(ub, vb, Bv);
-            wide_loads_A(sA, na01, na23, ua, va); // one step past the end reads valid (unused) entries
+            wide_loads_A<NJ>(sA, na01, na23, ua, va); // one step past the end reads valid (unused) entries
             na01 = __ldg(tA + 64); na23 = __ldg(tA + 65);
             prefetch_l1(tA + 3 * 64); prefetch_l1(tB + 3 * 32); // L2 latency > 1 k-step: pull the words into L1 early
-            mma_wide(acc, A, Bv[0], hi);
+            mma_wide<NJ>(acc, A, Bv[0], hi);
 #pragma unroll
-            for (int g = 0; g < 4; ++g) sub_pair<2, true>(ua[g], va[g], A[g]);
+            for (int g = 0; g < 4; ++g) sub_pair<NJ, true>(ua[g], va[g], A[g]);
             wide_loads_B(sB, nbw, ub, vb);
             nbw = __ldg(tB + 32 + hi);
         }
     }
     double* o = reinterpret_cast<double*>(out);
+    const int tX = (u.cls == 2) ? ti : tj, tY = (u.cls == 2) ? tj : ti; // plane pairs of the A and the B side
 #pragma unroll
-    for (int j = 0; j < 2; ++j)
+    for (int j = 0; j < NJ; ++j)
 #pragma unroll
         for (int g = 0; g < 4; ++g)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const int aX = 2 * j + (r & 1), cX = 4 * g + (r >> 1);
-                const int cc = 2 * kk + e, part = cc >> 2, ay = cc & 3;
+                const int aX = 2 * (TILE ? tX : j) + (r & 1), cX = 4 * g + (r >> 1);
+                const int cc = 2 * kk + e, part = cc >> 2;
+                if (TILE && (cc & 3) >= 2) continue; // columns of the planes that are not staged
+                const int ay = TILE ? 2 * tY + (cc & 3) : (cc & 3);
                 const int a1 = u.cls == 2 ? aX : ay, a2 = u.cls == 2 ? ay : aX;
                 o[2 * ((a1 * 4 + a2) * 16 + cX) + part] = acc[j * 4 + g][e];
             }
@@ -325,6 +341,14 @@ struct ProdArgs {
     // direct mode (tiny-L path, eq. 2.4 as a shifted sum): Bc / Be hold the x-space blocks, a task is
     // a displacement r, its items are (X, sink pair) with B1 at X + r and B2 at X, and Ft[r] accumulates over X
     int direct;
+    // tile-wise plan (k_product_t<true>; BASELINE.json configs[4]): one sink pair per launch (chain[chain_base]),
+    // sink spins a1 in {2 tile_i, 2 tile_i + 1}, a2 in {2 tile_j, 2 tile_j + 1}; B~1 / B~2 are staged from the
+    // two-plane chunks c1[V][2 * SM_PLANE] / c2[V][2 * SM_PLANE]; Ft[q][channel of the pair (PairChanRec::local)][256].
+    // For identical sink baryons the launch with tile_i != tile_j also writes the tile (tile_j, tile_i) by the
+    // sink-swap relation (reading A11), at -q.
+    const double2* c1;
+    const double2* c2;
+    int tile_i, tile_j, chain_base;
 };
 
 __device__ __forceinline__ size_t minus_q(int L, size_t q) {
@@ -343,6 +367,7 @@ __device__ __forceinline__ size_t shifted_site(int L, size_t X, size_t r) { // X
 // correlators = real combinations of them (eqs. 2.2-2.3) -> Ft[q][ch][256].  The pair record and
 // the channel coefficients are first copied to shared memory (one L2 round trip for the item
 // instead of one per use); thread et owns the spin components et + 64 m.
+template <bool TILE>
 __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q, bool accumulate,
                                              const double2* __restrict__ scr, int et, char* s_epi) {
     Pair3Rec* pr = reinterpret_cast<Pair3Rec*>(s_epi);
@@ -354,7 +379,10 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
     named_sync(BAR_EPI, PROD_ETHREADS);
     const int nelem = pr->nelem, nchan = pr->nchan, swap_mask = pr->swap_mask;
     const size_t mq = minus_q(a.L, q);
-    const bool mirror = !a.direct && pr->self_swap && mq != q;
+    const bool mirror = !a.direct && pr->self_swap && (mq != q || (TILE && a.tile_i != a.tile_j));
+    // tile-wise plan: this launch holds the components with a1 = m in pair tile_i, a2 = et >> 4 in pair tile_j
+    const bool col_ok = !TILE || ((et >> 5) == a.tile_j);
+    const int nrows = TILE ? nchan : a.nch_out;
     for (int c0 = 0; c0 < nchan; c0 += EPI_CG) {
         const int nc = min(EPI_CG, nchan - c0);
         {
@@ -426,23 +454,25 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
 #pragma unroll
         for (int c = 0; c < EPI_CG; ++c) {
             if (c < nc) {
-                const int ch = pcs[c].ch - a.ch_begin;
-                if (ch >= 0 && ch < a.nch_out) {
+                const int ch = TILE ? pcs[c].local : pcs[c].ch - a.ch_begin;
+                if (ch >= 0 && ch < nrows && col_ok) {
                     if (accumulate) { // direct mode, X > 0: the same thread wrote this entry for the previous X
 #pragma unroll
                         for (int m = 0; m < 4; ++m) {
-                            const double2 old = __ldcg(a.Ft + (q * a.nch_out + ch) * 256 + et + 64 * m);
+                            const double2 old = __ldcg(a.Ft + (q * nrows + ch) * 256 + et + 64 * m);
                             acc[c][m].x += old.x;
                             acc[c][m].y += old.y;
                         }
                     }
 #pragma unroll
-                    for (int m = 0; m < 4; ++m) __stcs(a.Ft + (q * a.nch_out + ch) * 256 + et + 64 * m, acc[c][m]);
+                    for (int m = 0; m < 4; ++m)
+                        if (!TILE || (m >> 1) == a.tile_i) __stcs(a.Ft + (q * nrows + ch) * 256 + et + 64 * m, acc[c][m]);
                     if (mirror) { // sink swap: F~(-q)_{a2 a1 a3 a4} = - F~(q)_{a1 a2 a3 a4}; here a1 = m, a2 = et >> 4
 #pragma unroll
                         for (int m = 0; m < 4; ++m)
-                            __stcs(a.Ft + (mq * a.nch_out + ch) * 256 + ((et >> 4) * 4 + m) * 16 + (et & 15),
-                                   make_double2(-acc[c][m].x, -acc[c][m].y));
+                            if (!TILE || (m >> 1) == a.tile_i)
+                                __stcs(a.Ft + (mq * nrows + ch) * 256 + ((et >> 4) * 4 + m) * 16 + (et & 15),
+                                       make_double2(-acc[c][m].x, -acc[c][m].y));
                     }
                 }
             }
@@ -465,7 +495,8 @@ __device__ __forceinline__ void prefetch_unit(const Unit3Rec* urec, const Diag3R
     }
 }
 
-__global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
+template <bool TILE>
+__global__ void __launch_bounds__(PROD_THREADS, 1) k_product_t(const ProdArgs a) {
     extern __shared__ __align__(128) char prod_smem[];
     char* smem = prod_smem;
     char* s1 = smem + SMO_S1;
@@ -497,7 +528,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
-            combine_item(a, ip, q, ctl->meta_acc[b] != 0, scr0 + b * scr_stride, et, smem + SMO_EPI);
+            combine_item<TILE>(a, ip, q, ctl->meta_acc[b] != 0, scr0 + b * scr_stride, et, smem + SMO_EPI);
             named_arrive(BAR_EMPTY0 + b, PROD_THREADS);
         }
         return;
@@ -519,7 +550,12 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
         if (pos == 0) {
             if (!a.direct || xs == 0) qt = ctl->qtask[ntask & 1]; // new task
             if (qt < a.ntasks) {
-                if (a.direct) { // task = displacement r = qt; this pass of the chain: site X = xs
+                if (TILE) { // one sink pair, every momentum of the list
+                    q = (size_t)__ldg(a.qorder + qt);
+                    mq = minus_q(a.L, q);
+                    cbase = a.chain_base;
+                    clen = 1;
+                } else if (a.direct) { // task = displacement r = qt; this pass of the chain: site X = xs
                     mq = xs;
                     q = shifted_site(a.L, xs, (size_t)qt);
                     cbase = 0;
@@ -555,17 +591,20 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             const uint32_t ubytes = (uint32_t)nunits * (uint32_t)sizeof(Unit3Rec);
             const uint32_t dbytes = (uint32_t)h1.y * (uint32_t)sizeof(Diag3Rec);
             void* rbar = load1 ? mbar1 : mbar2;
-            if (load1) mbar_expect_tx(mbar1, BLOCK_BYTES + ubytes + dbytes);
-            if (load2) mbar_expect_tx(mbar2, BLOCK_BYTES + (load1 ? 0u : ubytes + dbytes));
+            constexpr int NPL = TILE ? 2 : 4; // staged sink-spin planes per side
+            if (load1) mbar_expect_tx(mbar1, NPL * PLANE_BYTES + ubytes + dbytes);
+            if (load2) mbar_expect_tx(mbar2, NPL * PLANE_BYTES + (load1 ? 0u : ubytes + dbytes));
             if (load1) {
-                const char* g1 = reinterpret_cast<const char*>((h2.x ? a.Be + q * a.Re : a.Bc + q * a.Rc) + h2.y);
+                const char* g1 = TILE ? reinterpret_cast<const char*>(a.c1 + q * (size_t)(2 * SM_PLANE))
+                                      : reinterpret_cast<const char*>((h2.x ? a.Be + q * a.Re : a.Bc + q * a.Rc) + h2.y);
 #pragma unroll
-                for (int p = 0; p < 4; ++p) bulk_g2s(s1 + p * PLANE_BYTES, g1 + p * PLANE_BYTES, PLANE_BYTES, mbar1);
+                for (int p = 0; p < NPL; ++p) bulk_g2s(s1 + p * PLANE_BYTES, g1 + p * PLANE_BYTES, PLANE_BYTES, mbar1);
             }
             if (load2) {
-                const char* g2 = reinterpret_cast<const char*>((h2.z ? a.Be + mq * a.Re : a.Bc + mq * a.Rc) + h2.w);
+                const char* g2 = TILE ? reinterpret_cast<const char*>(a.c2 + mq * (size_t)(2 * SM_PLANE))
+                                      : reinterpret_cast<const char*>((h2.z ? a.Be + mq * a.Re : a.Bc + mq * a.Rc) + h2.w);
 #pragma unroll
-                for (int p = 0; p < 4; ++p) bulk_g2s(s2 + p * PLANE_BYTES, g2 + p * PLANE_BYTES, PLANE_BYTES, mbar2);
+                for (int p = 0; p < NPL; ++p) bulk_g2s(s2 + p * PLANE_BYTES, g2 + p * PLANE_BYTES, PLANE_BYTES, mbar2);
             }
             bulk_g2s(s_units, a.units + h1.x, ubytes, rbar);
             bulk_g2s(s_diags, a.diags + h1.z, dbytes, rbar);
@@ -593,8 +632,8 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product(const ProdArgs a) {
             u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
             if (i + PROD_CWARPS < nunits) prefetch_unit(s_units + i + PROD_CWARPS, s_diags, a.tab, lane);
             double2* out = scr + (size_t)u.slot * 256;
-            if (u.cls < 2) run_unit_square(u, s_diags, a.tab, s1, s2, out, lane);
-            else run_unit_wide(u, s_diags, a.tab, s1, s2, out, lane);
+            if (u.cls < 2) run_unit_square<TILE>(u, s_diags, a.tab, s1, s2, out, lane, a.tile_i, a.tile_j);
+            else run_unit_wide<TILE>(u, s_diags, a.tab, s1, s2, out, lane, a.tile_i, a.tile_j);
             i = grab();
         }
         __threadfence_block();

@@ -556,7 +556,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         for (size_t ic = 0; ic < channels.size(); ++ic) {
             if (plan.chan_pair[ic] != (int)ip) continue;
             PairChanRec pc;
-            pc.ch = (int)ic; pc.pad = 0;
+            pc.ch = (int)ic; pc.local = (int)plan.pair_chans.size() - pr.chan_begin;
             bool any = false;
             for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = pc.coefS[e] = 0.0;
             for (auto& ct : chan_ct[ic])
@@ -638,6 +638,21 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         plan.chain_full_n = (int)plan.chain.size();
         make_chain(half);
         plan.chain_half_n = (int)plan.chain.size() - plan.chain_full_n;
+        plan.chain_single_begin = (int)plan.chain.size();
+        for (int i = 0; i < (int)plan.pairs3.size(); ++i) make_chain(std::vector<int>{i});
+    }
+    // tile-wise plan: expansion map of a two-plane chunk of an antisymmetric block
+    for (int kind = BK_ASYM13; kind <= BK_ASYM23; ++kind) {
+        std::vector<int>& g = plan.gather_pp[kind - 1];
+        g.assign(2 * SM_PLANE, -1);
+        for (int al = 0; al < 2; ++al)
+            for (int x1 = 0; x1 < NXI; ++x1)
+                for (int x2 = 0; x2 < NXI; ++x2)
+                    for (int x3 = 0; x3 < NXI; ++x3) {
+                        if ((kind == BK_ASYM13 ? x1 : x2) == x3) continue; // diagonal: zero
+                        const Located loc = locate(kind, x1, x2, x3);
+                        g[al * SM_PLANE + sm_index(x1, x2, x3)] = (al * AS_PLANE + loc.idx) | (loc.sign < 0 ? (1 << 30) : 0);
+                    }
     }
     return "";
 }

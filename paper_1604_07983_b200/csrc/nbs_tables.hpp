@@ -123,7 +123,7 @@ struct Pair3Rec {
     int self_swap;           // 1: identical sink baryons; computed for q <= -q only, mirrored to -q by the epilogue
 };
 struct PairChanRec {
-    int ch, pad;
+    int ch, local; // channel index; position of the channel among the channels of its sink pair (row of the tile-wise plan's Ft)
     double coef[MAX_PAIR_ELEMS];  // channel = sum_e coef[e] * E_e + coefS[e] * (E_e with a3 <-> a4), eqs. 2.2-2.3;
     double coefS[MAX_PAIR_ELEMS]; // coefS carries the minus sign of the source swap (reading A11)
 };
@@ -174,8 +174,13 @@ struct Plan {
     std::vector<Diag3Rec> diags3;
     std::vector<uint2x> tab3;
     std::vector<PairChanRec> pair_chans;
-    std::vector<ChainRec> chain; // full chain, then the half chain
+    std::vector<ChainRec> chain; // full chain, then the half chain, then one single-pair chain per sink pair
     int chain_full_n = 0, chain_half_n = 0;
+    int chain_single_begin = 0; // chain[chain_single_begin + p]: sink pair p alone, both blocks loaded (tile-wise plan)
+    // Tile-wise plan (configs[4], 96^3): a chunk holds two sink-spin planes of one baryon for all sites.  Expansion
+    // map of a chunk of an antisymmetric block, [kind - 1][2 * SM_PLANE]: expanded element j takes compact element
+    // gather_pp[j] & 0x3fffffff of the same site's compact plane pair [2][AS_PLANE], negated if bit 30 is set; -1 = zero.
+    std::vector<int> gather_pp[2];
     int max_pair_units = 0;
     double sumKp_exec = 0; // executed k-steps x 4 (padding included)
 };

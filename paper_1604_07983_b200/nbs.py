@@ -27,7 +27,8 @@ BARYON_NAME = {v: k for k, v in BARYON_ID.items()}
 EXPORTS = ["nbs_create", "nbs_load_propagators", "nbs_correlator", "nbs_destroy", "nbs_last_error",
            "nbs_workspace_bytes", "nbs_num_channels", "nbs_channel_info", "nbs_std_channels",
            "nbs_diagram_stats", "nbs_blocks_x", "nbs_model_flops", "nbs_exec_flops", "nbs_fft3d",
-           "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct"]
+           "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_num_slots",
+           "nbs_probe_fp64", "nbs_tiled_info"]
 
 
 class nbs_channel(ctypes.Structure):
@@ -71,6 +72,9 @@ def lib() -> ctypes.CDLL:
         L.nbs_set_direct.argtypes = [c_void_p, c_int]
         L.nbs_stage_times.argtypes = [c_void_p, POINTER(c_double), POINTER(c_longlong), c_int]
         L.nbs_kernel_launches.argtypes = [c_void_p]
+        L.nbs_num_slots.argtypes = [c_void_p]
+        L.nbs_tiled_info.argtypes = [c_void_p, POINTER(c_int), POINTER(c_longlong)]
+        L.nbs_probe_fp64.argtypes = [c_void_p, c_int, c_int, POINTER(c_double), POINTER(c_double)]
         L.nbs_kernel_launches.restype = c_longlong
         _lib = L
     return _lib
@@ -237,6 +241,21 @@ class Nbs:
         calls = (c_longlong * len(self.STAGES))()
         _check(self.ctx, lib().nbs_stage_times(self.ctx, ms, calls, 1 if reset else 0))
         return {name: (ms[i], calls[i]) for i, name in enumerate(self.STAGES)}
+
+    def tiled_info(self) -> dict:
+        """nbs_tiled_info: {tiled, chunk_slots, chunk_builds}."""
+        n, b = c_int(), c_longlong()
+        t = _check(self.ctx, lib().nbs_tiled_info(self.ctx, byref(n), byref(b)))
+        return dict(tiled=bool(t), chunk_slots=n.value, chunk_builds=b.value)
+
+    def num_slots(self) -> int:
+        return _check(self.ctx, lib().nbs_num_slots(self.ctx))
+
+    def probe_fp64(self, mode: int, iters: int = 20000) -> dict:
+        """nbs_probe_fp64: {tflops, ms} of a register-resident FP64 instruction mix (see include/nbs.h)."""
+        tf, ms = c_double(), c_double()
+        _check(self.ctx, lib().nbs_probe_fp64(self.ctx, mode, iters, byref(tf), byref(ms)))
+        return dict(tflops=tf.value, ms=ms.value)
 
     def workspace_bytes(self) -> int:
         return lib().nbs_workspace_bytes(self.ctx)

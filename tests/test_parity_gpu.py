@@ -79,11 +79,12 @@ def test_normal_blocks_match_oracle(torch_cuda, nbs, oracle, L):
 
 
 # ------------------------------------------------------------------------------ rows a2, a5: FFT
-@pytest.mark.parametrize("L", [2, 4, 6, 8, 12, 16, 32])
+@pytest.mark.parametrize("L", [2, 4, 5, 6, 8, 12, 16, 24, 32, 48, 96])
 def test_fft3d_matches_numpy(torch_cuda, nbs, L):
-    """B~(q) = sum_x B(x) exp(-i q.x) and its inverse (eq. 2.6), ragged component count."""
+    """B~(q) = sum_x B(x) exp(-i q.x) and its inverse (eq. 2.6), ragged component count.  Powers of two: in-register
+    radix 2; 6, 12, 24, 48, 96 (configs[4]): the same behind a radix-3 stage; 5: the O(L^2) transform."""
     torch = torch_cuda
-    R = 37 if L < 32 else 5
+    R = 37 if L < 32 else (70 if L == 48 else 5)  # 70 > 64: two component groups of the radix-3 kernel, ragged
     rng = np.random.default_rng(L)
     a = rng.standard_normal((L, L, L, R)) + 1j * rng.standard_normal((L, L, L, R))  # [z][y][x][R]
     with nbs.Nbs(L, 1, [("p", "n", "p", "n")]) as ctx:
@@ -318,19 +319,6 @@ def test_full_size_32cubed_isospin_relations_config3(torch_cuda, nbs):
     assert rel(F[10], -F[10].transpose(0, 1)[..., minus_r]) <= RTOL
 
 
-def test_16cubed_config1_lattice_selected_channels(torch_cuda, nbs, oracle):
-    """BASELINE.json configs[1] lattice (16^3, u = d, s; time slice 7 of 32): element-by-element parity
-    on the whole volume for five channels that cover every accumulator layout, a Lambda/Sigma0 source
-    (shared elementary correlators, source swap) and an identical-baryon sink (sink swap)."""
-    L, t = 16, 7
-    S = synth.config_slice(synth.CONFIGS[1], t)
-    chans = [("p", "n", "p", "n"), ("p", "L", "S0", "p"), ("L", "L", "S0", "S0"), ("Sm", "X0", "Xm", "L"),
-             ("Xm", "X0", "Xm", "X0")]
-    F = run_gpu(torch_cuda, nbs, L, S, chans, t=t, T=32)
-    B = oracle.all_blocks(S, oracle.sink_names(chans))
-    assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
-
-
 def test_direct_shifted_sum_path(torch_cuda, nbs, oracle):
     """Row a7: eq. 2.4 as a shifted sum in x-space (nbs_set_direct), no FFT.  configs[0] (4^3, NN, u = d)
     against the oracle's direct tier A, and all 52 channels on 3^3 against tier B and the FFT path."""
@@ -416,3 +404,250 @@ def test_smallest_lattice(torch_cuda, nbs, oracle):
     assert_parity(F_dir, Fo, chans)
     with pytest.raises(nbs.NbsError):
         nbs.Nbs(1, 1)
+
+
+# ------------------------------------------------------------------------------ full-size dense parity (g2)
+def _momentum_parity(torch, nbs, oracle, cfg, t, nq=6, seed=0):
+    """All 52 channels of one dense full-size slice, in the launch configuration bench.py times, compared with the
+    oracle at sampled momenta: the oracle builds its x-space blocks of every site, projects them on the sampled
+    q and -q by the definition B~(q) = sum_x exp(-i q.x) B(x) and evaluates eq. 2.6's integrand
+    sum_P sigma_P B~1^(P)(q) B~2^(P)(-q) there (`fourpt_momentum`); the GPU's F(r) is projected on the same q by
+    the inverse of eq. 2.6, F~(q) = sum_r exp(-i q.r) F(r) (test-side DFT of the library's output).
+    Returns the worst per-channel max-norm error relative to the channel's max |F~|."""
+    import oracle_pool
+    L, T = cfg["L"], cfg["T"]
+    V = L ** 3
+    S = synth.config_slice(cfg, t)
+    chans = oracle.channels52()
+    rng = np.random.default_rng(seed + t)
+    qs = rng.choice(V, size=nq, replace=False)
+    qs[0] = 1 + L * (L - 1) + L * L * 5  # one hand-picked asymmetric momentum: (1, L-1, 5)
+    mq = oracle.minus_q_index(L)[qs]
+    allq = np.concatenate([qs, mq])
+    Bq = oracle_pool.blocks_at_momenta(L, S, oracle.sink_names(chans), allq)
+    ref = np.stack([oracle.fourpt_momentum(Bq[ch[0]][:nq], Bq[ch[1]][nq:], ch).reshape(nq, 256) for ch in chans])
+    with nbs.Nbs(L, T) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(t, d["u"], d["d"], d["s"])
+        F = ctx.correlator(t).reshape(len(chans) * 256, V)
+        torch.cuda.synchronize()
+        r = torch.arange(V, device="cuda")
+        rxyz = torch.stack([r % L, (r // L) % L, r // (L * L)]).to(torch.float64)           # [3, V]
+        q = torch.from_numpy(qs).cuda()
+        qxyz = torch.stack([q % L, (q // L) % L, q // (L * L)], dim=1).to(torch.float64)    # [nq, 3]
+        ang = (-2.0 * np.pi / L) * (qxyz @ rxyz)
+        phase = torch.complex(torch.cos(ang), torch.sin(ang))                                # [nq, V]
+        Fq = (F @ phase.T).reshape(len(chans), 256, nq).permute(0, 2, 1).cpu().numpy()       # [ch, nq, 256]
+    scale = np.abs(ref).max(axis=(1, 2))
+    assert scale.min() > 0
+    err = np.abs(Fq - ref).max(axis=(1, 2)) / scale
+    return err
+
+
+def test_config1_16cubed_all_52_channels_two_slices(torch_cuda, nbs, oracle):
+    """BASELINE.json configs[1] (16^3 x 32, u = d -> the isospin fast path, s): ALL 52 channels, dense Gaussian
+    propagators, element by element over the whole volume against the oracle's tier B, on the first and the last
+    time slice (F falls by exp(-1.4 * 31) ~ 1e-19 between them; the bar is relative per channel, reading A13)."""
+    import oracle_pool
+    torch = torch_cuda
+    cfg = synth.CONFIGS[1]
+    L, T, ts = cfg["L"], cfg["T"], [0, 31]
+    chans = oracle.channels52()
+    Ss = [synth.config_slice(cfg, t) for t in ts]
+    assert all(S["d"] is S["u"] for S in Ss)
+    Fo = oracle_pool.tierB_channels([(L, S, chans) for S in Ss])
+    with nbs.Nbs(L, T) as ctx:
+        for t, S, ref in zip(ts, Ss, Fo):
+            d = to_dev(torch, S)
+            ctx.load(t, d["u"], d["d"], d["s"])
+            F = ctx.correlator(t)
+            torch.cuda.synchronize()
+            assert_parity(F.cpu().numpy(), ref, chans)
+
+
+def test_config2_32cubed_dense_selected_channels_whole_volume(torch_cuda, nbs, oracle):
+    """BASELINE.json configs[2] (32^3 x 64, u != d != s, dense Gaussian propagators, all 52 channels computed as
+    bench.py launches them): three channels compared element by element over all 32768 displacements with the
+    oracle's tier B -- pn <- pn (two antisymmetric blocks), p Lambda <- Sigma0 p (a block without antisymmetry, a
+    Sigma0 source: shared elementary correlators and the source swap) and Lambda Lambda <- p Xi- (identical sink
+    baryons: half of the momenta computed, the rest mirrored).  Each covers the four accumulator layouts."""
+    import oracle_pool
+    torch = torch_cuda
+    cfg = synth.CONFIGS[2]
+    L, T, t = cfg["L"], cfg["T"], 31
+    S = synth.config_slice(cfg, t)
+    sel = [("p", "n", "p", "n"), ("p", "L", "S0", "p"), ("L", "L", "p", "Xm")]
+    chans = oracle.channels52()
+    idx = [chans.index(ch) for ch in sel]
+    ref = oracle_pool.tierB_channels([(L, S, sel)])[0]
+    with nbs.Nbs(L, T) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(t, d["u"], d["d"], d["s"])
+        F = ctx.correlator(t)
+        torch.cuda.synchronize()
+        got = np.stack([F[i].cpu().numpy() for i in idx])
+    assert_parity(got, ref, sel)
+
+
+@pytest.mark.parametrize("t", [0, 31, 63])
+def test_config2_32cubed_dense_all_52_channels_sampled_momenta(torch_cuda, nbs, oracle, t):
+    """configs[2], dense, all 52 channels, time slices 0, 31 and 63 (see _momentum_parity)."""
+    err = _momentum_parity(torch_cuda, nbs, oracle, synth.CONFIGS[2], t)
+    assert err.max() <= RTOL, (int(err.argmax()), float(err.max()))
+
+
+def test_config3_32cubed_su3_dense_against_oracle(torch_cuda, nbs, oracle):
+    """configs[3] (32^3, u = d = s, one array aliased three times: isospin fast path) against the oracle at sampled
+    momenta, all 52 channels."""
+    err = _momentum_parity(torch_cuda, nbs, oracle, synth.CONFIGS[3], 5, seed=7)
+    assert err.max() <= RTOL, (int(err.argmax()), float(err.max()))
+
+
+def test_blocks_dense_32cubed_sampled_sites(torch_cuda, nbs, oracle):
+    """eq. 4.1 at full size with dense input: the x-space blocks of configs[2] on 48 random sites (large site
+    indices included) against the oracle's blocks of those sites, one baryon of each block kind."""
+    torch = torch_cuda
+    cfg = synth.CONFIGS[2]
+    L, T, t = cfg["L"], cfg["T"], 9
+    V = L ** 3
+    S = synth.config_slice(cfg, t)
+    rng = np.random.default_rng(3)
+    sites = np.unique(np.concatenate([rng.choice(V, size=46, replace=False), [0, V - 1]]))
+    Ssub = {f: np.ascontiguousarray(S[f][sites]) for f in "uds"}
+    with nbs.Nbs(L, T) as ctx:
+        d = to_dev(torch, S)
+        ctx.load(t, d["u"], d["d"], d["s"])
+        for name in ("p", "n", "L", "S0"):
+            got = ctx.blocks_x(t, name)[torch.from_numpy(sites).cuda()].cpu().numpy()
+            ref = oracle.block(Ssub, name)
+            assert np.abs(got - ref).max() <= RTOL * np.abs(ref).max(), name
+
+
+# ------------------------------------------------------------------------------ hardening
+def test_workspace_budget_slots_and_guard(torch_cuda, nbs):
+    """workspace_budget_bytes: two slots when two workspaces fit, one when only one does, NBS_ENOMEM when none
+    does; with ONE slot, slices loaded alternately on two streams must still give the serial results (the
+    library orders the calls that share a slot, include/nbs.h nbs_num_slots)."""
+    torch = torch_cuda
+    L = 4
+    chans = [("p", "n", "p", "n"), ("L", "L", "L", "L"), ("Xm", "L", "S0", "Xm")]
+    with nbs.Nbs(L, 4, chans) as a, nbs.Nbs(L, 1, chans) as b:
+        assert a.num_slots() == 2 and b.num_slots() == 1
+        ws2, ws1 = a.workspace_bytes(), b.workspace_bytes()
+    per_slice = ws2 - ws1
+    tables = ws1 - per_slice
+    assert per_slice > 0 and tables > 0
+    with pytest.raises(nbs.NbsError) as e:
+        nbs.Nbs(L, 4, chans, workspace_budget_bytes=tables + per_slice // 2)
+    assert e.value.code == nbs.NBS_ENOMEM
+    Ss = [props(L, seed=40, t=t) for t in range(4)]
+    serial = [run_gpu(torch, nbs, L, Ss[t], chans, t=t, T=4) for t in range(4)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    with nbs.Nbs(L, 4, chans, workspace_budget_bytes=tables + per_slice * 3 // 2) as ctx:
+        assert ctx.num_slots() == 1
+        devs = [to_dev(torch, S) for S in Ss]
+        torch.cuda.synchronize()
+        outs = []
+        for rep in range(3):  # repeat: a race would not show on every run
+            outs = []
+            for t in range(4):
+                st = streams[t % 2]
+                ctx.load(t, devs[t]["u"], devs[t]["d"], devs[t]["s"], stream=st)
+                outs.append(ctx.correlator(t, stream=st))
+            torch.cuda.synchronize()
+            for t in range(4):
+                assert np.array_equal(outs[t].cpu().numpy(), serial[t]), (rep, t)
+
+
+def test_host_output_range_checked_before_launch(torch_cuda, nbs):
+    """A host output larger than the device staging is refused (NBS_ENOMEM) before any kernel is enqueued."""
+    L = 2
+    chans = [("p", "n", "p", "n")] * 1 + [("p", "p", "p", "p"), ("n", "n", "n", "n"), ("p", "n", "p", "n")] * 40
+    S = props(L, seed=41)
+    with nbs.Nbs(L, 1, chans) as ctx:
+        ctx.load(0, S["u"], S["d"], S["s"])
+        n0 = ctx.kernel_launches()
+        host = np.empty((len(chans), 4, 4, 4, 4, L ** 3), dtype=np.complex128)
+        with pytest.raises(nbs.NbsError) as e:
+            ctx.correlator(0, out=host)
+        assert e.value.code == nbs.NBS_ENOMEM
+        assert ctx.kernel_launches() == n0
+
+
+def test_fp64_probe(torch_cuda, nbs):
+    """nbs_probe_fp64: the register-resident mixes run and report plausible FP64 rates on a B200."""
+    with nbs.Nbs(2, 1, [("p", "n", "p", "n")]) as ctx:
+        dmma = ctx.probe_fp64(0, 20000)["tflops"]
+        assert 10.0 < dmma < 60.0, dmma
+        for mode in (1, 2, 3, 4):
+            assert ctx.probe_fp64(mode, 5000)["tflops"] > 1.0
+        with pytest.raises(nbs.NbsError):
+            ctx.probe_fp64(7, 10)
+
+
+# ------------------------------------------------------------------------------ tile-wise plan (configs[4], g1)
+@pytest.mark.parametrize("L", [4, 6])
+def test_tilewise_plan_equals_resident_plan_and_oracle(torch_cuda, nbs, oracle, L):
+    """The plan of BASELINE.json configs[4] ("blocks must be contracted tile-wise, never materialised") forced on a
+    small lattice by a tiny workspace budget: two-plane chunks built on demand (2 or 3 chunk buffers: evictions and
+    rebuilds), one product launch per (sink pair, plane pair, plane pair), all 52 channels -- against the oracle and
+    against the resident plan.  L = 6 also takes the radix-3 FFT (96 = 3 * 32).  Device and host output, and a
+    channel range that cuts through sink pairs."""
+    torch = torch_cuda
+    V = L ** 3
+    S = props(L, seed=61)
+    chans = oracle.channels52()
+    with nbs.Nbs(L, 1) as ctx:
+        assert not ctx.tiled_info()["tiled"]
+        ws_res = ctx.workspace_bytes()
+        d = to_dev(torch, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        F_res = ctx.correlator(0).cpu().numpy()
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    Fo = oracle.correlator_fft(L, B, chans)
+    assert_parity(F_res, Fo, chans)
+    # resident: B [V][33216] + Be [V][6 * 6960] + Ft [V][52][256]; tile-wise: n chunks [V][3480] + Ft [V][6][256]
+    base = ws_res - V * (33216 + 6 * 6960 + 52 * 256) * 16
+    for nchunks in (2, 3):
+        budget = base + V * (nchunks * 3480 + 6 * 256) * 16 + V * 3480 * 8  # half a chunk of slack
+        with nbs.Nbs(L, 1, workspace_budget_bytes=budget) as ctx:
+            info = ctx.tiled_info()
+            assert info["tiled"] and info["chunk_slots"] == nchunks, info
+            d = to_dev(torch, S)
+            ctx.load(0, d["u"], d["d"], d["s"])
+            F = ctx.correlator(0).cpu().numpy()
+            assert_parity(F, Fo, chans)
+            assert_parity(F, F_res, chans)
+            builds = ctx.tiled_info()["chunk_builds"]
+            assert builds >= 16  # 8 baryons x 2 plane pairs at least once
+            part = ctx.correlator(0, 9, 13).cpu().numpy()  # cuts the pairs (Sigma0 p) and (Lambda Lambda)
+            assert np.array_equal(part, F[9:13])
+            host = np.empty((3, 4, 4, 4, 4, V), dtype=np.complex128)
+            ctx.correlator(0, 40, 43, out=host)
+            torch.cuda.synchronize()
+            assert np.array_equal(host, F[40:43])
+            with pytest.raises(nbs.NbsError):
+                ctx.set_direct(True)
+    with pytest.raises(nbs.NbsError) as e:
+        nbs.Nbs(L, 1, workspace_budget_bytes=base + V * (1 * 3480 + 6 * 256) * 16)
+    assert e.value.code == nbs.NBS_ENOMEM
+
+
+def test_tilewise_plan_user_channels_identical_sinks(torch_cuda, nbs, oracle):
+    """Tile-wise plan on a user channel list made of identical-baryon sinks (the (0,1) tile on every momentum and its
+    mirror, reading A11) and an elementary-operator channel, odd L (one self-conjugate momentum)."""
+    torch = torch_cuda
+    L = 3
+    V = L ** 3
+    S = props(L, seed=62)
+    chans = [("L", "L", "L", "L"), ("L", "L", "S0", "S0"), ("S0", "S0", "Sp", "Sm"), ("p", "p", "p", "p"), ("p", "L", "p", "Xu")]
+    with nbs.Nbs(L, 1, chans) as ctx:
+        ws_res = ctx.workspace_bytes()
+    # a budget well below the resident workspace but above two chunks + Ft + tables
+    with nbs.Nbs(L, 1, chans, workspace_budget_bytes=ws_res - V * 6960 * 16) as ctx:
+        assert ctx.tiled_info()["tiled"]
+        d = to_dev(torch, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        F = ctx.correlator(0).cpu().numpy()
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
