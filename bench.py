@@ -26,7 +26,11 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "nbs_correlator_time_slices_per_s_52ch_32c64_fp64"
+METRIC = "nbs_correlator_time_slices_per_s_52ch_32c64_fp64"  # configs[2]; other --config values rename it (metric_name)
+
+
+def metric_name(cfg_index: int, cfg: dict, L: int) -> str:
+    return METRIC if cfg_index == 2 else f"nbs_correlator_time_slices_per_s_52ch_{L}c{cfg['T']}_fp64"
 UNIT = "time-slices/s"
 # Cross-check only: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz.  The roofline denominator is
 # MEASURED in this process by nbs_probe_fp64 (register-resident DMMA.8x8x4 on all SMs, include/nbs.h).
@@ -156,13 +160,14 @@ def main():
     L = args.lattice or cfg["L"]
     V = L ** 3
     workload = f"BASELINE.json configs[{args.config}]: {L}^3 x {cfg['T']}, 52 channels, complex128, {cfg['name']}"
+    metric = metric_name(args.config, cfg, L)
 
     if args.impl == "reference":
         if rank != 0:
             return
         steps, warm = max(1, min(args.steps, 3)), min(args.warmup, 1)
         leg = oracle_leg(args.oracle_sample_L or 8, args.config, steps, warm)
-        line = {"impl": "reference", "metric": METRIC, "value": leg["value"], "unit": UNIT, "n_gpus": args.gpus,
+        line = {"impl": "reference", "metric": metric, "value": leg["value"], "unit": UNIT, "n_gpus": args.gpus,
                 "steps": steps, "warmup": warm, "ms_per_step": leg["ms_per_step"], "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": workload, "ms_per_slice_extrapolated": leg["ms_per_slice_extrapolated"]},
@@ -189,7 +194,7 @@ def main():
 
     K, W = args.steps, max(args.warmup, 3)
     T = cfg["T"]
-    npool = min(4, K + W)
+    npool = min(4 if L <= 32 else 2, K + W, T)
     # this rank's time slices: T-parallel replicas (t = rank, rank + world, ...)
     pool_t = replicas.rank_slices(rank, world, T, count=npool)
     host = []
@@ -213,22 +218,33 @@ def main():
             d[f] = d[spec] if isinstance(spec, str) else h[f].to(dev)
         resident.append(d)
 
-    ctx = nbs.Nbs(L, T, None, device=local)
+    # configs[4] (96^3): the result of one slice is 188 GB, so it is produced sink pair by sink pair into one buffer
+    # (include/nbs.h: channel ranges, nbs_pair_order); the library takes its tile-wise plan there
+    big = 52 * 256 * V * 16 > 40e9
+    ctx = nbs.Nbs(L, T, None, device=local,
+                  workspace_budget_bytes=0 if not big else int(0.92 * torch.cuda.mem_get_info(dev)[0]) - 6 * 256 * V * 16)
     nch = ctx.nch
     flops = ctx.model_flops()
-    out_dev = torch.empty((nch, 256, V), dtype=torch.complex128, device=dev)
+    tiled = ctx.tiled_info()
+    ranges = ctx.pair_order() if big else [(0, nch)]
+    nmax = max(hi - lo for lo, hi in ranges)
+    out_dev = torch.empty((nmax, 256, V), dtype=torch.complex128, device=dev)
     stream = torch.cuda.Stream(device=dev)
 
     def step_resident(i):
         t = pool_t[i % npool]
         r = resident[i % npool]
         ctx.load(t, r["u"], r["d"], r["s"], stream=stream)
-        ctx.correlator(t, out=out_dev, stream=stream)
+        for lo, hi in ranges:
+            ctx.correlator(t, lo, hi, out=out_dev[:hi - lo], stream=stream)
 
     # ---------------- device-resident leg (value, roofline) ----------------
     for i in range(W):
         step_resident(i)
     torch.cuda.synchronize()
+    # clocks are sampled from here on: the probes and the timed steps keep the GPU loaded without a gap
+    sampler = ClockSampler(local)
+    sampler.start()
     # measured FP64 peaks of this device, in this process (nbs_probe_fp64): ~0.3 s per mix
     probe = {name: ctx.probe_fp64(mode, 60000)["tflops"]
              for name, mode in (("dmma", 0), ("dfma", 1), ("dadd", 2), ("mix_16x16_kstep", 3), ("mix_64x4_kstep", 4))}
@@ -236,10 +252,9 @@ def main():
     ctx.set_timing(True)
     ctx.stage_times(reset=True)
     launches0 = ctx.kernel_launches()
-    sampler = ClockSampler(local)
+    builds0 = ctx.tiled_info()["chunk_builds"]
     barrier()
     torch.cuda.synchronize()
-    sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for i in range(K):
@@ -252,6 +267,7 @@ def main():
     stage = ctx.stage_times(reset=True)
     ctx.set_timing(False)
     launches = ctx.kernel_launches() - launches0
+    builds = ctx.tiled_info()["chunk_builds"] - builds0
     checksum = float(out_dev.view(torch.float64).abs().max().item())
     assert np.isfinite(checksum) and checksum > 0
 
@@ -263,7 +279,8 @@ def main():
         # while the kernels of slice i + 1 run.  Every slice still pays its own H2D and D2H.
         nslots = ctx.num_slots()  # one stream per workspace slot; with one slot the slices serialise on one stream
         streams2 = [stream, torch.cuda.Stream(device=dev) if nslots > 1 else stream]
-        outs_host = [torch.empty((nch, 256, V), dtype=torch.complex128).pin_memory() for _ in range(2)]
+        del out_dev
+        outs_host = [torch.empty((nmax, 256, V), dtype=torch.complex128).pin_memory() for _ in range(2 if not big else 1)]
         out_host = outs_host[0]
 
         def step_e2e(i):
@@ -271,13 +288,14 @@ def main():
             h = host[i % npool]
             st = streams2[t % nslots]                                # one stream per workspace slot (t % nslots)
             ctx.load(t, h["u"], h["d"], h["s"], stream=st)          # H2D inside the library
-            ctx.correlator(t, out=outs_host[t % 2], stream=st)      # D2H of F inside the library
+            for lo, hi in ranges:                                    # D2H of F inside the library
+                ctx.correlator(t, lo, hi, out=outs_host[t % len(outs_host)][:hi - lo], stream=st)
         step_e2e(0)
         step_e2e(1)
         torch.cuda.synchronize()
         barrier()
         f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        Ke = max(2, min(K, 6))
+        Ke = max(2, min(K, 6 if not big else 2))
         f0.record(stream)
         if nslots > 1:
             streams2[1].wait_event(f0)
@@ -306,22 +324,25 @@ def main():
 
     value = replicas.aggregate_throughput(K, world, ms)
     prod_ms, prod_calls = stage["product"]
-    prod_avg_s = prod_ms * 1e-3 / max(prod_calls, 1)
+    prod_avg_s = prod_ms * 1e-3 / K  # per slice (the tile-wise plan launches the kernel up to 4 times per sink pair)
     alg_flops = flops["product"] * V  # 256 * sum_d K_d cMAC x 8 flop per q, standard count
     achieved = alg_flops / prod_avg_s / 1e12
     peak = probe["dmma"]
     traffic, traffic_src = product_dram_traffic()
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload, "channels": nch, "lattice": [L, L, L, T],
-                   "l2_policy": "inputs (226 MB) and intermediates (tens of GB per slice) exceed the 126 MB L2",
+                   "l2_policy": "inputs (%.0f MB per slice) and intermediates (%.1f GB per slice) exceed the 126 MB L2"
+                                % (len({id(v) for v in host[0].values()}) * V * 144 * 16 / 1e6, V * 1.4e6 / 1e9),
                    "parallelism": "replicas only (T-parallel), no collective" if world > 1 else "1 GPU",
+                   "plan": ("tile-wise: %d chunk buffers, %.1f chunk builds per slice, %d channel ranges per slice"
+                            % (tiled["chunk_slots"], builds / K, len(ranges))) if tiled["tiled"] else "resident",
                    "channel_sites_per_s": value * nch * V},
         "clocks": clocks,
         "gpu_launches": int(launches),
-        "stages_ms_per_step": {k: v[0] / max(v[1], 1) for k, v in stage.items()},
+        "stages_ms_per_step": {k: v[0] / K for k, v in stage.items()},
         "roofline": {"bound": "alu", "kernel": "product (effective blocks x product, eqs. 4.2-4.3)",
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                      "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
@@ -333,7 +354,7 @@ def main():
                      "flops_per_launch_executed": flops["product_executed"] * V,
                      "achieved_executed": flops["product_executed"] * V / prod_avg_s / 1e12,
                      "frac_executed": flops["product_executed"] * V / prod_avg_s / 1e12 / peak,
-                     "kernel_ms": prod_avg_s * 1e3,
+                     "kernel_ms": prod_avg_s * 1e3, "kernel_launches_per_step": prod_calls / K,
                      "note": "achieved/frac use SURVEY 8(d)'s standard count (256 x sum K_d x 8 flop per site); the kernel "
                              "evaluates about half of it (shared elementary correlators, source- and sink-swap relations), "
                              "so frac can exceed 1; achieved_executed/frac_executed count 8 flop per complex MAC actually "

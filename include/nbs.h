@@ -146,6 +146,15 @@ int nbs_num_slots(const nbs_ctx* ctx);
  */
 int nbs_tiled_info(const nbs_ctx* ctx, int* chunk_slots, long long* chunk_builds);
 
+/*
+ * nbs_pair_order -- the sink pairs (B1 B2) of the channel list in the order in which the library walks them
+ * (consecutive pairs share a baryon block), each as the smallest channel range [ch_begin[i], ch_end[i]) that holds
+ * its channels (in the standard 52-channel list the channels of a sink pair are consecutive).  With the tile-wise
+ * plan, calling nbs_correlator once per range in this order builds the fewest chunks.  Returns the number of sink
+ * pairs; writes at most `cap` entries; either array may be NULL.
+ */
+int nbs_pair_order(const nbs_ctx* ctx, int* ch_begin, int* ch_end, int cap);
+
 /* Helpers. */
 const char* nbs_last_error(const nbs_ctx* ctx); /* never NULL; ctx == NULL -> last nbs_create error */
 size_t nbs_workspace_bytes(const nbs_ctx* ctx); /* library-owned device bytes */

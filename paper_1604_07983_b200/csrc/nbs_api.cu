@@ -856,6 +856,24 @@ int nbs_fft3d(nbs_ctx* c, void* data_dev, size_t R, int inverse, void* stream) {
 
 long long nbs_kernel_launches(const nbs_ctx* c) { return c ? c->launches : 0; }
 
+int nbs_pair_order(const nbs_ctx* c, int* ch_begin, int* ch_end, int cap) {
+    if (!c) return NBS_EINVAL;
+    const Plan& P = c->plan;
+    for (int ci = 0; ci < P.chain_full_n; ++ci) {
+        const Pair3Rec& pr = P.pairs3[P.chain[ci].pair];
+        int lo = 1 << 30, hi = -1;
+        for (int k = 0; k < pr.nchan; ++k) {
+            const int ch = P.pair_chans[pr.chan_begin + k].ch;
+            lo = std::min(lo, ch); hi = std::max(hi, ch + 1);
+        }
+        if (ci < cap) {
+            if (ch_begin) ch_begin[ci] = lo;
+            if (ch_end) ch_end[ci] = hi;
+        }
+    }
+    return P.chain_full_n;
+}
+
 int nbs_tiled_info(const nbs_ctx* c, int* chunk_slots, long long* chunk_builds) {
     if (!c) return NBS_EINVAL;
     if (chunk_slots) *chunk_slots = (int)c->chunks.size();

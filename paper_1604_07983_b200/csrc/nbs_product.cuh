@@ -380,8 +380,13 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
     const int nelem = pr->nelem, nchan = pr->nchan, swap_mask = pr->swap_mask;
     const size_t mq = minus_q(a.L, q);
     const bool mirror = !a.direct && pr->self_swap && (mq != q || (TILE && a.tile_i != a.tile_j));
-    // tile-wise plan: this launch holds the components with a1 = m in pair tile_i, a2 = et >> 4 in pair tile_j
-    const bool col_ok = !TILE || ((et >> 5) == a.tile_j);
+    // Components of this thread.  Whole blocks: et + 64 m, m = a1 = 0..3 (et = a2 a3 a4).  Tile-wise plan: the launch
+    // holds a1 in pair tile_i, a2 in pair tile_j, 64 components, one per thread (et = low bit of a1, low bit of a2, a3 a4).
+    constexpr int NM = TILE ? 1 : 4;
+    const int t_a1 = 2 * a.tile_i + (et >> 5), t_a2 = 2 * a.tile_j + ((et >> 4) & 1);
+    auto comp = [&](int m) { return TILE ? (t_a1 * 4 + t_a2) * 16 + (et & 15) : et + 64 * m; };
+    // sink swap: F~(-q)_{a2 a1 a3 a4} = - F~(q)_{a1 a2 a3 a4}
+    auto mirror_comp = [&](int m) { return TILE ? (t_a2 * 4 + t_a1) * 16 + (et & 15) : ((et >> 4) * 4 + m) * 16 + (et & 15); };
     const int nrows = TILE ? nchan : a.nch_out;
     for (int c0 = 0; c0 < nchan; c0 += EPI_CG) {
         const int nc = min(EPI_CG, nchan - c0);
@@ -391,30 +396,30 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
             for (int i = et; i < nwords; i += PROD_ETHREADS) reinterpret_cast<double*>(pcs)[i] = __ldg(src + i);
         }
         named_sync(BAR_EPI, PROD_ETHREADS);
-        double2 acc[EPI_CG][4];
+        double2 acc[EPI_CG][NM];
 #pragma unroll
         for (int c = 0; c < EPI_CG; ++c)
 #pragma unroll
-            for (int m = 0; m < 4; ++m) acc[c][m] = make_double2(0.0, 0.0);
+            for (int m = 0; m < NM; ++m) acc[c][m] = make_double2(0.0, 0.0);
         for (int e = 0; e < nelem; ++e) {
-            double2 s[4];
+            double2 s[NM];
 #pragma unroll
-            for (int m = 0; m < 4; ++m) s[m] = make_double2(0.0, 0.0);
+            for (int m = 0; m < NM; ++m) s[m] = make_double2(0.0, 0.0);
             const int ub = pr->elem_unit_begin[e], ue = pr->elem_unit_begin[e + 1];
             // rows in groups of EG with all loads of a group in flight (an elementary correlator has
             // ~5 unit rows: a plain unrolled loop would run them one by one through its remainder)
             constexpr int EG = 4;
             for (int ul = ub; ul < ue; ul += EG) {
-                double2 v[EG][4];
+                double2 v[EG][NM];
 #pragma unroll
                 for (int j = 0; j < EG; ++j)
 #pragma unroll
-                    for (int m = 0; m < 4; ++m)
-                        v[j][m] = (ul + j < ue) ? __ldcg(scr + (size_t)(ul + j) * 256 + et + 64 * m) : make_double2(0.0, 0.0);
+                    for (int m = 0; m < NM; ++m)
+                        v[j][m] = (ul + j < ue) ? __ldcg(scr + (size_t)(ul + j) * 256 + comp(m)) : make_double2(0.0, 0.0);
 #pragma unroll
                 for (int j = 0; j < EG; ++j)
 #pragma unroll
-                    for (int m = 0; m < 4; ++m) {
+                    for (int m = 0; m < NM; ++m) {
                         s[m].x += v[j][m].x;
                         s[m].y += v[j][m].y;
                     }
@@ -422,11 +427,11 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
             // source swap (reading A11): the same sums at the component with a3 <-> a4
             // exchanged live in another lane of the same 16-lane group
             const bool sw = (swap_mask >> e) & 1;
-            double2 ss[4];
+            double2 ss[NM];
             if (sw) {
                 const int src_lane = (et & 0x10) | ((et & 3) << 2) | ((et >> 2) & 3);
 #pragma unroll
-                for (int m = 0; m < 4; ++m) {
+                for (int m = 0; m < NM; ++m) {
                     ss[m].x = __shfl_sync(0xffffffffu, s[m].x, src_lane);
                     ss[m].y = __shfl_sync(0xffffffffu, s[m].y, src_lane);
                 }
@@ -436,14 +441,14 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
                 if (c < nc) {
                     const double k = pcs[c].coef[e];
 #pragma unroll
-                    for (int m = 0; m < 4; ++m) {
+                    for (int m = 0; m < NM; ++m) {
                         acc[c][m].x = fma(k, s[m].x, acc[c][m].x);
                         acc[c][m].y = fma(k, s[m].y, acc[c][m].y);
                     }
                     if (sw) {
                         const double ks = pcs[c].coefS[e];
 #pragma unroll
-                        for (int m = 0; m < 4; ++m) {
+                        for (int m = 0; m < NM; ++m) {
                             acc[c][m].x = fma(ks, ss[m].x, acc[c][m].x);
                             acc[c][m].y = fma(ks, ss[m].y, acc[c][m].y);
                         }
@@ -455,24 +460,21 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
         for (int c = 0; c < EPI_CG; ++c) {
             if (c < nc) {
                 const int ch = TILE ? pcs[c].local : pcs[c].ch - a.ch_begin;
-                if (ch >= 0 && ch < nrows && col_ok) {
+                if (ch >= 0 && ch < nrows) {
                     if (accumulate) { // direct mode, X > 0: the same thread wrote this entry for the previous X
 #pragma unroll
-                        for (int m = 0; m < 4; ++m) {
-                            const double2 old = __ldcg(a.Ft + (q * nrows + ch) * 256 + et + 64 * m);
+                        for (int m = 0; m < NM; ++m) {
+                            const double2 old = __ldcg(a.Ft + (q * nrows + ch) * 256 + comp(m));
                             acc[c][m].x += old.x;
                             acc[c][m].y += old.y;
                         }
                     }
 #pragma unroll
-                    for (int m = 0; m < 4; ++m)
-                        if (!TILE || (m >> 1) == a.tile_i) __stcs(a.Ft + (q * nrows + ch) * 256 + et + 64 * m, acc[c][m]);
-                    if (mirror) { // sink swap: F~(-q)_{a2 a1 a3 a4} = - F~(q)_{a1 a2 a3 a4}; here a1 = m, a2 = et >> 4
+                    for (int m = 0; m < NM; ++m) __stcs(a.Ft + (q * nrows + ch) * 256 + comp(m), acc[c][m]);
+                    if (mirror) {
 #pragma unroll
-                        for (int m = 0; m < 4; ++m)
-                            if (!TILE || (m >> 1) == a.tile_i)
-                                __stcs(a.Ft + (mq * nrows + ch) * 256 + ((et >> 4) * 4 + m) * 16 + (et & 15),
-                                       make_double2(-acc[c][m].x, -acc[c][m].y));
+                        for (int m = 0; m < NM; ++m)
+                            __stcs(a.Ft + (mq * nrows + ch) * 256 + mirror_comp(m), make_double2(-acc[c][m].x, -acc[c][m].y));
                     }
                 }
             }

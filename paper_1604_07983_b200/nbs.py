@@ -28,7 +28,7 @@ EXPORTS = ["nbs_create", "nbs_load_propagators", "nbs_correlator", "nbs_destroy"
            "nbs_workspace_bytes", "nbs_num_channels", "nbs_channel_info", "nbs_std_channels",
            "nbs_diagram_stats", "nbs_blocks_x", "nbs_model_flops", "nbs_exec_flops", "nbs_fft3d",
            "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_num_slots",
-           "nbs_probe_fp64", "nbs_tiled_info"]
+           "nbs_probe_fp64", "nbs_tiled_info", "nbs_pair_order"]
 
 
 class nbs_channel(ctypes.Structure):
@@ -73,6 +73,7 @@ def lib() -> ctypes.CDLL:
         L.nbs_stage_times.argtypes = [c_void_p, POINTER(c_double), POINTER(c_longlong), c_int]
         L.nbs_kernel_launches.argtypes = [c_void_p]
         L.nbs_num_slots.argtypes = [c_void_p]
+        L.nbs_pair_order.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), c_int]
         L.nbs_tiled_info.argtypes = [c_void_p, POINTER(c_int), POINTER(c_longlong)]
         L.nbs_probe_fp64.argtypes = [c_void_p, c_int, c_int, POINTER(c_double), POINTER(c_double)]
         L.nbs_kernel_launches.restype = c_longlong
@@ -247,6 +248,12 @@ class Nbs:
         n, b = c_int(), c_longlong()
         t = _check(self.ctx, lib().nbs_tiled_info(self.ctx, byref(n), byref(b)))
         return dict(tiled=bool(t), chunk_slots=n.value, chunk_builds=b.value)
+
+    def pair_order(self) -> list:
+        """nbs_pair_order: [(ch_begin, ch_end)] per sink pair, in the library's walking order."""
+        lo, hi = (c_int * 64)(), (c_int * 64)()
+        n = _check(self.ctx, lib().nbs_pair_order(self.ctx, lo, hi, 64))
+        return [(lo[i], hi[i]) for i in range(min(n, 64))]
 
     def num_slots(self) -> int:
         return _check(self.ctx, lib().nbs_num_slots(self.ctx))

@@ -435,7 +435,7 @@ def _momentum_parity(torch, nbs, oracle, cfg, t, nq=6, seed=0):
         rxyz = torch.stack([r % L, (r // L) % L, r // (L * L)]).to(torch.float64)           # [3, V]
         q = torch.from_numpy(qs).cuda()
         qxyz = torch.stack([q % L, (q // L) % L, q // (L * L)], dim=1).to(torch.float64)    # [nq, 3]
-        ang = (-2.0 * np.pi / L) * (qxyz @ rxyz)
+        ang = (-2.0 * np.pi / L) * torch.remainder(qxyz @ rxyz, L)  # q.r mod L: exact in float64
         phase = torch.complex(torch.cos(ang), torch.sin(ang))                                # [nq, V]
         Fq = (F @ phase.T).reshape(len(chans), 256, nq).permute(0, 2, 1).cpu().numpy()       # [ch, nq, 256]
     scale = np.abs(ref).max(axis=(1, 2))
@@ -465,28 +465,109 @@ def test_config1_16cubed_all_52_channels_two_slices(torch_cuda, nbs, oracle):
             assert_parity(F.cpu().numpy(), ref, chans)
 
 
-def test_config2_32cubed_dense_selected_channels_whole_volume(torch_cuda, nbs, oracle):
+CFG2_SELECTED = [("p", "n", "p", "n"), ("p", "L", "S0", "p"), ("L", "L", "p", "Xm")]
+
+
+@pytest.fixture(scope="module")
+def cfg2_t31_reference(oracle):
+    """configs[2], time slice 31: the propagators and the oracle's tier B for three channels over the whole 32^3
+    volume (shared by the 32^3 and the 96^3 test below; ~90 s on 16 host cores)."""
+    import oracle_pool
+    cfg = synth.CONFIGS[2]
+    S = synth.config_slice(cfg, 31)
+    ref = oracle_pool.tierB_channels([(cfg["L"], S, CFG2_SELECTED)])[0]
+    return S, ref
+
+
+def test_config2_32cubed_dense_selected_channels_whole_volume(torch_cuda, nbs, oracle, cfg2_t31_reference):
     """BASELINE.json configs[2] (32^3 x 64, u != d != s, dense Gaussian propagators, all 52 channels computed as
     bench.py launches them): three channels compared element by element over all 32768 displacements with the
     oracle's tier B -- pn <- pn (two antisymmetric blocks), p Lambda <- Sigma0 p (a block without antisymmetry, a
     Sigma0 source: shared elementary correlators and the source swap) and Lambda Lambda <- p Xi- (identical sink
     baryons: half of the momenta computed, the rest mirrored).  Each covers the four accumulator layouts."""
-    import oracle_pool
     torch = torch_cuda
     cfg = synth.CONFIGS[2]
     L, T, t = cfg["L"], cfg["T"], 31
-    S = synth.config_slice(cfg, t)
-    sel = [("p", "n", "p", "n"), ("p", "L", "S0", "p"), ("L", "L", "p", "Xm")]
+    S, ref = cfg2_t31_reference
     chans = oracle.channels52()
-    idx = [chans.index(ch) for ch in sel]
-    ref = oracle_pool.tierB_channels([(L, S, sel)])[0]
+    idx = [chans.index(ch) for ch in CFG2_SELECTED]
     with nbs.Nbs(L, T) as ctx:
         d = to_dev(torch, S)
         ctx.load(t, d["u"], d["d"], d["s"])
         F = ctx.correlator(t)
         torch.cuda.synchronize()
         got = np.stack([F[i].cpu().numpy() for i in idx])
-    assert_parity(got, ref, sel)
+    assert_parity(got, ref, CFG2_SELECTED)
+
+
+def test_config4_96cubed_tilewise_against_oracle_by_tiling(torch_cuda, nbs, oracle, cfg2_t31_reference):
+    """BASELINE.json configs[4] size (96^3, 52-channel plan, tile-wise: the resident workspace would need 1.2 TB):
+    the propagators are the 32^3 field of the test above repeated 3 x 3 x 3 times, for which
+    F_96(r) = 27 F_32(r mod 32) (the tiling identity, pinned on the oracle in tests/test_oracle_pins.py), so the
+    oracle's 32^3 tier B gives the expected value at every one of the 884736 displacements.  Channel ranges that
+    hold pn <- pn, p Lambda <- Sigma0 p and Lambda Lambda <- p Xi- (an identical-baryon sink)."""
+    torch = torch_cuda
+    L, L0, T, t = 96, 32, 4, 1
+    V = L ** 3
+    S32, ref = cfg2_t31_reference
+    chans = oracle.channels52()
+    x = np.arange(V)
+    small = (x % L) % L0 + L0 * (((x // L) % L) % L0 + L0 * ((x // (L * L)) % L0))
+    d = {f: torch.from_numpy(S32[f][small]).cuda() for f in "uds"}
+    small_dev = torch.from_numpy(small).cuda()
+    with nbs.Nbs(L, T) as ctx:
+        info = ctx.tiled_info()
+        assert info["tiled"] and info["chunk_slots"] >= 2, info
+        ctx.load(t, d["u"], d["d"], d["s"])
+        for ch, r32 in zip(CFG2_SELECTED, ref):
+            i = chans.index(ch)
+            F = ctx.correlator(t, i, i + 1).reshape(256, V)
+            torch.cuda.synchronize()
+            want = torch.from_numpy(r32.reshape(256, L0 ** 3)).cuda()
+            scale = float(want.abs().max()) * 27.0
+            err = 0.0
+            for a in range(0, 256, 64):  # in slabs: the gathered reference of a whole channel would be 3.6 GB more
+                err = max(err, float((F[a:a + 64] - 27.0 * want[a:a + 64][:, small_dev]).abs().max()))
+            assert err <= RTOL * scale, (ch, err / scale)
+            del F
+
+
+def test_config4_96cubed_dense_sampled_momenta(torch_cuda, nbs, oracle):
+    """configs[4] itself (96^3, u = d and s, seed 5, dense): the three channels of the sink pair p Lambda on one time
+    slice against the oracle at sampled momenta (see _momentum_parity: the oracle's blocks of all 884736 sites
+    projected on q and -q, eq. 2.6's integrand there; the library's F(r) projected on the same q)."""
+    import oracle_pool
+    torch = torch_cuda
+    cfg = synth.CONFIGS[4]
+    L, T, t, nq = cfg["L"], cfg["T"], 2, 4
+    V = L ** 3
+    S = synth.config_slice(cfg, t)
+    chans = oracle.channels52()
+    lo, hi = 1, 4
+    sel = chans[lo:hi]
+    assert all(ch[:2] == ("p", "L") for ch in sel)
+    rng = np.random.default_rng(96)
+    qs = rng.choice(V, size=nq, replace=False)
+    qs[0] = 1 + L * (L - 1) + L * L * 37
+    mq = oracle.minus_q_index(L)[qs]
+    Bq = oracle_pool.blocks_at_momenta(L, S, ["p", "L"], np.concatenate([qs, mq]), chunk=4096)
+    ref = np.stack([oracle.fourpt_momentum(Bq[ch[0]][:nq], Bq[ch[1]][nq:], ch).reshape(nq, 256) for ch in sel])
+    dd = to_dev(torch, S)
+    with nbs.Nbs(L, T) as ctx:
+        assert ctx.tiled_info()["tiled"]
+        ctx.load(t, dd["u"], dd["d"], dd["s"])
+        F = ctx.correlator(t, lo, hi).reshape((hi - lo) * 256, V)
+        torch.cuda.synchronize()
+        r = torch.arange(V, device="cuda")
+        rxyz = torch.stack([r % L, (r // L) % L, r // (L * L)]).to(torch.float64)
+        q = torch.from_numpy(qs).cuda()
+        qxyz = torch.stack([q % L, (q // L) % L, q // (L * L)], dim=1).to(torch.float64)
+        ang = (-2.0 * np.pi / L) * torch.remainder(qxyz @ rxyz, L)  # q.r mod L: exact in float64
+        phase = torch.complex(torch.cos(ang), torch.sin(ang))
+        Fq = (F @ phase.T).reshape(hi - lo, 256, nq).permute(0, 2, 1).cpu().numpy()
+    scale = np.abs(ref).max(axis=(1, 2))
+    err = np.abs(Fq - ref).max(axis=(1, 2)) / scale
+    assert err.max() <= RTOL, (int(err.argmax()), float(err.max()))
 
 
 @pytest.mark.parametrize("t", [0, 31, 63])
