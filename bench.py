@@ -70,7 +70,12 @@ def parse():
     ap.add_argument("--steps", type=int, default=8)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (2 = 32^3 x 64)")
+    ap.add_argument("--config", type=int, default=2,
+                    help="index into BASELINE.json configs (2 = 32^3 x 64, the metric; 1 = 16^3 x 32, the paper's Fig. 1-2 "
+                         "lattice; 3 = 32^3 u=d=s; 4 = 96^3, tile-wise plan)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1 (T-parallel replicas, PAPER.md:133-137): weak = K slices per rank; strong = the K slices "
+                         "of the job are divided over the ranks (K must be a multiple of N)")
     ap.add_argument("--lattice", type=int, default=0, help="override L (debugging only; invalidates the metric)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -193,6 +198,10 @@ def main():
             dist.barrier()
 
     K, W = args.steps, max(args.warmup, 3)
+    if args.scaling == "strong":
+        if K % world:
+            raise SystemExit("--scaling strong needs --steps to be a multiple of the number of ranks")
+        K //= world  # slices of THIS rank; the job's total stays args.steps
     T = cfg["T"]
     npool = min(4 if L <= 32 else 2, K + W, T)
     # this rank's time slices: T-parallel replicas (t = rank, rank + world, ...)
@@ -330,8 +339,9 @@ def main():
     peak = probe["dmma"]
     traffic, traffic_src = product_dram_traffic()
     line = {
-        "metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
+        "ms_per_step": ms / (K * world if args.scaling == "strong" else K), "higher_is_better": True,
+        "scaling": args.scaling, "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload, "channels": nch, "lattice": [L, L, L, T],
                    "l2_policy": "inputs (%.0f MB per slice) and intermediates (%.1f GB per slice) exceed the 126 MB L2"

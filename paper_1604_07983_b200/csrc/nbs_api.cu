@@ -419,7 +419,11 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     if (ch && nch < 1) return fail(nullptr, NBS_EINVAL, "nch must be >= 1");
     std::vector<nbs_channel> chans = ch ? std::vector<nbs_channel>(ch, ch + nch) : standard_channels();
     nbs_ctx* c = new nbs_ctx();
+#if defined(NBS_UNIT_SPLIT) && defined(NBS_UNIT_COST)
+    std::string err = build_plan(chans, c->plan, NBS_UNIT_SPLIT, NBS_UNIT_COST);
+#else
     std::string err = build_plan(chans, c->plan);
+#endif
     if (!err.empty()) { delete c; return fail(nullptr, NBS_EINVAL, err); }
     c->L = L; c->T = T; c->device = device;
     c->V = (size_t)L * L * L;

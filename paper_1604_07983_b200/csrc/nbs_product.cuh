@@ -90,6 +90,9 @@ static_assert(3 + 2 * PROD_NBUF <= 16, "named barriers");
 static_assert(sizeof(Pair3Rec) % 4 == 0 && sizeof(PairChanRec) % 8 == 0 && SMO_CTRL % 8 == 0, "record alignment");
 
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void bulk_prefetch_l2(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
 
 // ---- gathers (eq. 4.2) ----------------------------------------------------------------------
 // One table word = one (+, -) pair of byte offsets into a staged block.  ld_pair issues the
@@ -612,6 +615,22 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_t(const ProdArgs a)
             bulk_g2s(s_diags, a.diags + h1.z, dbytes, rbar);
             if (pos == 0 && (!a.direct || xs == 0)) ctl->qtask[(ntask + 1) & 1] = (long long)atomicAdd(a.counter, 1ull); // next task
             if (pos + 1 < clen) nh2 = __ldg(crec + 5);
+            // the blocks the NEXT item will stage are pulled into L2 now, one item ahead of their bulk copy (69.8 -> 69.3 ms)
+            if (!TILE && !a.direct) {
+                if (pos + 1 < clen) {
+                    const int4 n0 = __ldg(crec + 3);
+                    if (n0.y) bulk_prefetch_l2((nh2.x ? a.Be + q * a.Re : a.Bc + q * a.Rc) + nh2.y, BLOCK_BYTES);
+                    if (n0.z) bulk_prefetch_l2((nh2.z ? a.Be + mq * a.Re : a.Bc + mq * a.Rc) + nh2.w, BLOCK_BYTES);
+                } else {
+                    const long long nqt = ctl->qtask[(ntask + 1) & 1];
+                    if (nqt < a.ntasks) {
+                        const size_t q2 = (size_t)__ldg(a.qorder + nqt), mq2 = minus_q(a.L, q2);
+                        const int4 f2 = __ldg(reinterpret_cast<const int4*>(a.chain + ((mq2 < q2) ? a.chain_full_n : 0)) + 2);
+                        bulk_prefetch_l2((f2.x ? a.Be + q2 * a.Re : a.Bc + q2 * a.Rc) + f2.y, BLOCK_BYTES);
+                        bulk_prefetch_l2((f2.z ? a.Be + mq2 * a.Re : a.Bc + mq2 * a.Rc) + f2.w, BLOCK_BYTES);
+                    }
+                }
+            }
         }
         if (pos + 1 < clen) { nh0 = __ldg(crec + 3); nh1 = __ldg(crec + 4); }
         // while the copies fly: table heads of the unit this warp will probably start with
