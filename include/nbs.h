@@ -173,6 +173,10 @@ int nbs_channel_info(const nbs_ctx* ctx, int i, nbs_channel* out);
  *             Returns NBS_EINVAL for an invalid channel.
  */
 int nbs_std_channels(nbs_channel* out, int cap);
+/*   nbs_plan_selfcheck: host-only bounds check of the tables the kernels index with (gather offsets inside the staged
+ *             blocks, table extents including the software pipeline's look-ahead, unit / diagram / chain / channel record
+ *             ranges, expansion maps); ch == NULL checks the standard 52 channels.  Returns 0 or a negative check number. */
+int nbs_plan_selfcheck(const nbs_channel* ch, int nch);
 int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long long* literal_terms);
 
 /*

@@ -410,6 +410,70 @@ int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long lo
     return (int)d.size();
 }
 
+int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
+    // Host-side bounds check of everything the kernels index with table data (compute-sanitizer is not available on
+    // the target pool): returns 0, or the negative number of the first violated invariant.
+    std::vector<nbs_channel> chans = ch ? std::vector<nbs_channel>(ch, ch + nch) : standard_channels();
+    Plan P;
+    std::string err = build_plan(chans, P);
+    if (!err.empty()) { g_create_error = err; return NBS_EINVAL; }
+    const size_t ntab = P.tab3.size();
+    for (auto& w : P.tab3) // 1: gather offsets are 16-byte aligned positions inside a staged block
+        if (w.x % 16 || w.y % 16 || w.x >= BLOCK_BYTES || w.y >= BLOCK_BYTES) return -101;
+    for (auto& d : P.diags3) { // 2: a diagram's tables, one k-step past its range (software pipeline), lie inside tab3
+        const size_t rowsA = 8, stepA = 4 * rowsA * d.nwA, stepB4 = 4 * 4 * d.nwB, stepB8 = 4 * 8 * d.nwB;
+        if (d.send <= d.sbeg || d.send > (d.K + 3) / 4) return -102;
+        if (d.offA + (size_t)(d.send + 1) * std::max<size_t>(stepA, 4 * 8 * 4) > ntab) return -103;
+        if (d.offB + (size_t)(d.send + 1) * std::max(stepB4, stepB8) > ntab) return -104;
+        if (d.offA % 2 || d.offB % 2) return -105; // 16-byte aligned tables (uint4 reads)
+    }
+    if (P.max_pair_units > MAX_PAIR_UNITS) return -106;
+    for (auto& pr : P.pairs3) {
+        if (pr.nunits < 1 || pr.nunits > MAX_PAIR_UNITS || pr.ndiags > MAX_PAIR_DIAGS || pr.nelem > MAX_PAIR_ELEMS) return -107;
+        if (pr.unit_begin + pr.nunits > (int)P.units3.size() || pr.diag_begin + pr.ndiags > (int)P.diags3.size()) return -108;
+        if (pr.slot1 < 0 || pr.slot1 >= (int)P.baryons.size() || pr.slot2 < 0 || pr.slot2 >= (int)P.baryons.size()) return -109;
+        std::vector<char> seen(pr.nunits, 0);
+        for (int u = 0; u < pr.nunits; ++u) {
+            const Unit3Rec& ur = P.units3[pr.unit_begin + u];
+            if (ur.diag_begin < 0 || ur.diag_end > pr.ndiags || ur.diag_begin >= ur.diag_end) return -110;
+            if (ur.slot < 0 || ur.slot >= pr.nunits || seen[ur.slot] || ur.cls < 0 || ur.cls > 3) return -111;
+            seen[ur.slot] = 1; // every scratch row written by exactly one unit
+        }
+        for (int e = 0; e < MAX_PAIR_ELEMS; ++e)
+            if (pr.elem_unit_begin[e] > pr.elem_unit_begin[e + 1] || pr.elem_unit_begin[e + 1] > pr.nunits) return -112;
+        if (pr.chan_begin + pr.nchan > (int)P.pair_chans.size()) return -113;
+        for (int k = 0; k < pr.nchan; ++k) {
+            const PairChanRec& pc = P.pair_chans[pr.chan_begin + k];
+            if (pc.ch < 0 || pc.ch >= (int)chans.size() || pc.local != k) return -114;
+        }
+    }
+    if ((int)P.chain.size() != P.chain_full_n + P.chain_half_n + (int)P.pairs3.size()) return -115;
+    for (auto& cr : P.chain) {
+        if (cr.pair < 0 || cr.pair >= (int)P.pairs3.size()) return -116;
+        const Pair3Rec& pr = P.pairs3[cr.pair];
+        if (cr.nunits != pr.nunits || cr.unit_begin != pr.unit_begin || cr.ndiags != pr.ndiags || cr.diag_begin != pr.diag_begin) return -117;
+        const size_t lim1 = cr.buf1 ? (size_t)P.n_asym * SM_BLOCK : (size_t)P.row_elems;
+        const size_t lim2 = cr.buf2 ? (size_t)P.n_asym * SM_BLOCK : (size_t)P.row_elems;
+        if ((size_t)cr.off1 + SM_BLOCK > lim1 || (size_t)cr.off2 + SM_BLOCK > lim2) return -118;
+    }
+    for (int i = 0; i < P.chain_full_n + P.chain_half_n; ++i) { // 3: a reused staged block really is the one staged before
+        if (i == 0 || i == P.chain_full_n) { if (!P.chain[i].load1 || !P.chain[i].load2) return -119; continue; }
+        const Pair3Rec &a = P.pairs3[P.chain[i - 1].pair], &b = P.pairs3[P.chain[i].pair];
+        if ((!P.chain[i].load1 && a.slot1 != b.slot1) || (!P.chain[i].load2 && a.slot2 != b.slot2)) return -120;
+    }
+    for (size_t j = 0; j < P.gather.size(); ++j) // 4: expansion maps stay inside the compact row / chunk
+        if (P.gather[j] >= 0 && (size_t)(P.gather[j] & 0x3fffffff) >= (size_t)P.row_elems) return -121;
+    for (size_t j = 0; j < P.gather_iso.size(); ++j)
+        if (P.gather_iso[j] >= 0 && (size_t)(P.gather_iso[j] & 0x3fffffff) >= (size_t)P.row_elems_iso) return -122;
+    for (int k = 0; k < 2; ++k) {
+        if (P.gather_pp[k].size() != (size_t)(2 * SM_PLANE)) return -123;
+        for (int g : P.gather_pp[k])
+            if (g >= 0 && (g & 0x3fffffff) >= 2 * AS_PLANE) return -124;
+    }
+    if ((size_t)P.row_elems != (size_t)P.slot_off.back() + block_elems(P.slot_kind.back())) return -125;
+    return NBS_OK;
+}
+
 int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int device, size_t budget) {
     if (!out) return fail(nullptr, NBS_EINVAL, "out is NULL");
     *out = nullptr;

@@ -28,7 +28,7 @@ EXPORTS = ["nbs_create", "nbs_load_propagators", "nbs_correlator", "nbs_destroy"
            "nbs_workspace_bytes", "nbs_num_channels", "nbs_channel_info", "nbs_std_channels",
            "nbs_diagram_stats", "nbs_blocks_x", "nbs_model_flops", "nbs_exec_flops", "nbs_fft3d",
            "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_num_slots",
-           "nbs_probe_fp64", "nbs_tiled_info", "nbs_pair_order"]
+           "nbs_probe_fp64", "nbs_tiled_info", "nbs_pair_order", "nbs_plan_selfcheck"]
 
 
 class nbs_channel(ctypes.Structure):
@@ -73,6 +73,7 @@ def lib() -> ctypes.CDLL:
         L.nbs_stage_times.argtypes = [c_void_p, POINTER(c_double), POINTER(c_longlong), c_int]
         L.nbs_kernel_launches.argtypes = [c_void_p]
         L.nbs_num_slots.argtypes = [c_void_p]
+        L.nbs_plan_selfcheck.argtypes = [POINTER(nbs_channel), c_int]
         L.nbs_pair_order.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), c_int]
         L.nbs_tiled_info.argtypes = [c_void_p, POINTER(c_int), POINTER(c_longlong)]
         L.nbs_probe_fp64.argtypes = [c_void_p, c_int, c_int, POINTER(c_double), POINTER(c_double)]
@@ -102,6 +103,14 @@ def nbs_std_channels() -> list[tuple[str, str, str, str]]:
     buf = (nbs_channel * 64)()
     n = lib().nbs_std_channels(buf, 64)
     return [tuple(BARYON_NAME[x] for x in (buf[i].b1, buf[i].b2, buf[i].b3, buf[i].b4)) for i in range(n)]
+
+
+def nbs_plan_selfcheck(channels=None) -> int:
+    """Host-only bounds check of the kernel tables (0 = all invariants hold)."""
+    if channels is None:
+        return lib().nbs_plan_selfcheck(None, 0)
+    arr = _as_channels(channels)
+    return lib().nbs_plan_selfcheck(arr, len(channels))
 
 
 def nbs_diagram_stats(channel) -> dict:

@@ -78,3 +78,14 @@ def test_no_cpu_fallback_without_gpu():
     with pytest.raises(nbs.NbsError) as e:
         nbs.nbs_create(4, 1)
     assert e.value.code == nbs.NBS_ECUDA
+
+
+def test_plan_tables_stay_in_bounds():
+    """compute-sanitizer is closed on the target pool, so the indices the kernels take from tables are bounds-checked on
+    the host: gather offsets inside the staged blocks, table extents including the pipeline's look-ahead, unit / diagram
+    / chain / channel record ranges, expansion maps -- for the standard 52 channels and for user lists."""
+    from paper_1604_07983_b200 import nbs
+    assert nbs.nbs_plan_selfcheck() == 0
+    assert nbs.nbs_plan_selfcheck([("p", "n", "p", "n")]) == 0
+    assert nbs.nbs_plan_selfcheck([("L", "L", "L", "L"), ("S0", "S0", "Sp", "Sm"), ("p", "L", "p", "Xu"), ("Xu", "Xs", "Xd", "Xs")]) == 0
+    assert nbs.nbs_plan_selfcheck([("p", "p", "p", "p"), ("n", "n", "n", "n"), ("p", "n", "p", "n")] * 40) == 0
