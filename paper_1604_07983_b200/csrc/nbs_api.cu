@@ -9,6 +9,7 @@
 
 #include "nbs_kernels.cuh"
 #include "nbs_product.cuh"
+#include "nbs_product_c.cuh"
 #include "nbs_probe.cuh"
 #include "nbs_tables.hpp"
 
@@ -58,6 +59,18 @@ struct nbs_ctx {
     PairChanRec* d_pair_chans = nullptr;
     int* d_qorder = nullptr;
     int prod_grid = 0;
+    // pipelined product kernel (nbs_product_c.cuh): compact antisymmetric blocks staged as they are, no expansion
+    bool use_c = false;
+    uint2x* d_tabc = nullptr;
+    Diag3Rec* d_diagsc = nullptr;
+    CItem* d_cprog = nullptr;
+    CLoad* d_cloads = nullptr;
+    int* d_slot_off = nullptr;      // block staged for a slot: its own ...
+    int* d_slot_off_iso = nullptr;  // ... or, in the isospin limit, its partner's
+    double* d_pair_sign = nullptr;  // all +1
+    double* d_pair_sign_iso = nullptr;
+    uint32_t c_rec_stride = 0, c_units_bytes = 0;
+    size_t c_smem = 0;
     bool direct = false; // nbs_set_direct: eq. 2.4 as a shifted sum in x-space (tiny lattices)
     // Tile-wise plan (BASELINE.json configs[4], 96^3): chosen by nbs_create when the resident
     // workspace does not fit.  A chunk = two sink-spin planes of one baryon for all momenta, [V][2 * SM_PLANE],
@@ -428,6 +441,50 @@ int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
         if (d.offA % 2 || d.offB % 2) return -105; // 16-byte aligned tables (uint4 reads)
     }
     if (P.max_pair_units > MAX_PAIR_UNITS) return -106;
+    if (P.diagsc.size() != P.diags3.size()) return -130;
+    {   // 5: compact gather tables and the program of the pipelined kernel
+        const size_t ntabc = P.tabc.size();
+        for (auto& w : P.tabc) {
+            const uint32_t x = w.x & 0x7fffffffu, y = w.y & 0x7fffffffu;
+            if (x % 16 || y % 16 || x >= BLOCK_BYTES || y >= BLOCK_BYTES) return -131;
+        }
+        for (size_t i = 0; i < P.diagsc.size(); ++i) {
+            const Diag3Rec &d = P.diagsc[i], &o = P.diags3[i];
+            if (d.sbeg != o.sbeg || d.send != o.send || d.nwA != o.nwA || d.nwB != o.nwB || d.K != o.K) return -132;
+            const size_t stepA = 4 * 8 * (size_t)d.nwA, stepB4 = 4 * 4 * (size_t)d.nwB, stepB8 = 4 * 8 * (size_t)d.nwB;
+            if (d.offA + (size_t)(d.send + 1) * std::max<size_t>(stepA, 4 * 8 * 4) > ntabc) return -133;
+            if (d.offB + (size_t)(d.send + 1) * std::max(stepB4, stepB8) > ntabc) return -134;
+            if (d.offA % 2 || d.offB % 2) return -135;
+        }
+        if (P.cprog_ok) {
+            if ((int)P.cprog.size() != P.chain_full_n + P.chain_half_n || (int)P.cprog.size() < C_NREC) return -136;
+            std::vector<int> fresh(C_NSLOT, 0), loaded(C_NSLOT, 0);
+            for (size_t i = 0; i < P.cprog.size(); ++i) {
+                const CItem& it = P.cprog[i];
+                const Pair3Rec& pr = P.pairs3[it.pair];
+                const uint32_t n1 = (uint32_t)block_elems(P.slot_kind[pr.slot1]) * 16u, n2 = (uint32_t)block_elems(P.slot_kind[pr.slot2]) * 16u;
+                if (it.off1 % C_SLOT_BYTES || it.off2 % C_SLOT_BYTES) return -137;
+                if (it.off1 + n1 > C_NSLOT * C_SLOT_BYTES || it.off2 + n2 > C_NSLOT * C_SLOT_BYTES) return -138;
+                if (it.off1 < it.off2 + n2 && it.off2 < it.off1 + n1) return -139; // the two blocks of an item do not overlap
+                if (it.ps1 != 2u * (uint32_t)plane_elems(P.slot_kind[pr.slot1]) * 16u || it.ps2 != 2u * (uint32_t)plane_elems(P.slot_kind[pr.slot2]) * 16u) return -140;
+                if (it.rel_begin > it.rel_end || it.rel_end > (int)P.cloads.size()) return -141;
+                for (int side = 0; side < 2; ++side) {
+                    const int w = (it.flags >> (3 * side)) & 7;
+                    if (w > C_NSLOT) return -142;
+                    if (w && (uint32_t)(w - 1) * C_SLOT_BYTES != (side ? it.off2 : it.off1)) return -143;
+                    if (w) ++fresh[w - 1];
+                }
+            }
+            for (auto& ld : P.cloads) {
+                if ((ld.src & 255) >= (int)P.baryons.size() || ld.bar < 0 || ld.bar >= C_NSLOT) return -144;
+                if (ld.dst != (uint32_t)ld.bar * C_SLOT_BYTES || ld.bytes != (uint32_t)block_elems(P.slot_kind[ld.src & 255]) * 16u) return -145;
+                if (ld.dst + ld.bytes > C_NSLOT * C_SLOT_BYTES || ld.bytes % 64) return -146;
+                ++loaded[ld.bar];
+            }
+            for (int s = 0; s < C_NSLOT; ++s)
+                if (fresh[s] != loaded[s]) return -147; // every load is waited for by exactly one item (barrier phases stay in step)
+        }
+    }
     for (auto& pr : P.pairs3) {
         if (pr.nunits < 1 || pr.nunits > MAX_PAIR_UNITS || pr.ndiags > MAX_PAIR_DIAGS || pr.nelem > MAX_PAIR_ELEMS) return -107;
         if (pr.unit_begin + pr.nunits > (int)P.units3.size() || pr.diag_begin + pr.ndiags > (int)P.diags3.size()) return -108;
@@ -585,6 +642,34 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
             return NBS_ECUDA;
         }
         c->prod_grid = prop.multiProcessorCount;
+        // pipelined kernel: needs a program (Plan::cprog_ok) and room for three record buffers
+        c->c_units_bytes = (uint32_t)c->plan.max_pair_units * (uint32_t)sizeof(Unit3Rec);
+        c->c_rec_stride = c->c_units_bytes + (uint32_t)c->plan.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
+        c->c_smem = cprod_smem_bytes(c->c_rec_stride);
+        c->use_c = c->plan.cprog_ok && c->c_smem <= (size_t)prop.sharedMemPerBlockOptin && c->plan.baryons.size() < 256;
+#ifdef NBS_NO_PIPELINE
+        c->use_c = false;
+#endif
+    }
+    if (c->use_c) {
+        CUC(upload(c, c->d_tabc, c->plan.tabc));
+        CUC(upload(c, c->d_diagsc, c->plan.diagsc));
+        CUC(upload(c, c->d_cprog, c->plan.cprog));
+        CUC(upload(c, c->d_cloads, c->plan.cloads));
+        std::vector<int> off, off_iso;
+        std::vector<double> sg, sg_iso;
+        for (size_t i = 0; i < c->plan.baryons.size(); ++i) {
+            off.push_back(c->plan.slot_off[i]);
+            off_iso.push_back(c->plan.slot_off[c->plan.slot_partner_iso[i]]);
+        }
+        for (auto& pr : c->plan.pairs3) {
+            sg.push_back(1.0);
+            sg_iso.push_back((double)(c->plan.slot_sign_iso[pr.slot1] * c->plan.slot_sign_iso[pr.slot2]));
+        }
+        CUC(upload(c, c->d_slot_off, off));
+        CUC(upload(c, c->d_slot_off_iso, off_iso));
+        CUC(upload(c, c->d_pair_sign, sg));
+        CUC(upload(c, c->d_pair_sign_iso, sg_iso));
     }
     CUC(upload(c, c->d_baryon_of_slot, c->plan.baryons));
     CUC(upload(c, c->d_one_baryon, std::vector<int>(NBS_NUM_BARYONS, 0)));
@@ -610,7 +695,10 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     // workspace: per slice in flight, blocks + elementary correlators + channel correlators
     size_t nchan = c->plan.channels.size();
     size_t scratch_elems = (size_t)c->prod_grid * PROD_NBUF * c->plan.max_pair_units * 256;
-    size_t per_slice = (c->V * (c->R + c->Re + nchan * 256) + scratch_elems) * sizeof(double2);
+    // the expanded antisymmetric blocks (Be) exist only where the one-buffer kernel runs: without a program for the
+    // pipelined kernel, and for the direct shifted sum (allocated by nbs_set_direct)
+    const size_t Re_res = c->use_c ? 0 : c->Re;
+    size_t per_slice = (c->V * (c->R + Re_res + nchan * 256) + scratch_elems) * sizeof(double2);
     size_t free_b = 0, total_b = 0;
     CUX(cudaMemGetInfo(&free_b, &total_b));
     size_t avail = (size_t)(0.92 * (double)free_b);
@@ -641,7 +729,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     for (int i = 0; i < c->nslices; ++i) {
         if (!c->tiled) {
             CUC(dev_alloc(c, c->slice[i].B, c->V * c->R));
-            CUC(dev_alloc(c, c->slice[i].Be, std::max<size_t>(c->V * c->Re, 1)));
+            if (!c->use_c) CUC(dev_alloc(c, c->slice[i].Be, std::max<size_t>(c->V * c->Re, 1)));
         } else {
             for (auto& ck : c->chunks) CUC(dev_alloc(c, ck.buf, chunk_elems));
         }
@@ -654,6 +742,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     }
     CUX(cudaFuncSetAttribute(k_product_t<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
     CUX(cudaFuncSetAttribute(k_product_t<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
+    if (c->use_c) CUX(cudaFuncSetAttribute(k_product_c, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->c_smem));
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<32>()));
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<32>()));
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<16>()));
@@ -761,7 +850,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     double2* dst = (double2*)out;
     if (memloc == NBS_MEM_HOST) {
         if (need <= c->V * c->R * sizeof(double2)) dst = sl.B;
-        else if (need <= c->V * c->Re * sizeof(double2)) dst = sl.Be;
+        else if (sl.Be && need <= c->V * c->Re * sizeof(double2)) dst = sl.Be;
         else return fail(c, NBS_ENOMEM, "channel range too large for the device staging of a host output; use a smaller range");
     }
     {
@@ -785,7 +874,8 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
             rc = fft3d(c, sl.B, c->R, false, st, nullptr, iso ? (size_t)c->plan.row_elems_iso : 0);
             if (rc) return rc;
         }
-        if (c->Re) { // antisymmetric blocks: mirror halves restored for the gathers of the product kernel
+        const bool pipelined = c->use_c && !c->direct;
+        if (c->Re && !pipelined) { // antisymmetric blocks: mirror halves restored for the gathers of the one-buffer kernel
             k_expand<<<(unsigned)c->V, 256, 0, st>>>(sl.B, c->R, iso ? c->d_gather_iso : c->d_gather, (int)c->Re, sl.Be);
             CU(c, cudaGetLastError());
             ++c->launches;
@@ -795,6 +885,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     {
         StageTimer tm(c, NBS_STAGE_PRODUCT, st);
         CU(c, cudaMemsetAsync(sl.counter, 0, sizeof(unsigned long long), st));
+        const bool pipelined = c->use_c && !c->direct;
         ProdArgs pa;
         pa.Bc = sl.B; pa.Rc = c->R; pa.Be = sl.Be; pa.Re = c->Re; pa.L = c->L;
         pa.slot_src = reinterpret_cast<const int2*>(c->d_slot_src);
@@ -810,6 +901,19 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
         pa.counter = sl.counter;
         unsigned grid = (unsigned)std::min<long long>(c->prod_grid, pa.ntasks);
         pa.c1 = pa.c2 = nullptr; pa.tile_i = pa.tile_j = 0; pa.chain_base = 0;
+        if (pipelined) {
+            CProdArgs ca;
+            ca.base = pa;
+            ca.B = sl.B; ca.R = c->R;
+            ca.slot_off = iso ? c->d_slot_off_iso : c->d_slot_off;
+            ca.pair_sign = iso ? c->d_pair_sign_iso : c->d_pair_sign;
+            ca.ntasks = c->ntasks_half; ca.qhalf = c->d_qorder_half;
+            ca.prog = c->d_cprog; ca.nitems = (int)c->plan.cprog.size(); ca.loads = c->d_cloads;
+            ca.units = c->d_units3; ca.diags = c->d_diagsc; ca.tab = reinterpret_cast<const uint2*>(c->d_tabc);
+            ca.rec_stride = c->c_rec_stride; ca.units_bytes = c->c_units_bytes;
+            grid = (unsigned)std::min<long long>(c->prod_grid, ca.ntasks);
+            k_product_c<<<grid, PROD_THREADS, c->c_smem, st>>>(ca);
+        } else
         k_product_t<false><<<grid, PROD_THREADS, PROD_SMEM, st>>>(pa);
         CU(c, cudaGetLastError());
         ++c->launches;
@@ -836,6 +940,13 @@ int nbs_set_direct(nbs_ctx* c, int enable) {
     if (!c) return NBS_EINVAL;
     if (enable && c->L > 8) return fail(c, NBS_EINVAL, "the direct shifted sum is O(V^2): allowed for L <= 8 only");
     if (enable && c->tiled) return fail(c, NBS_EINVAL, "the direct shifted sum is not available with the tile-wise plan");
+    if (enable && c->Re) // the direct sum runs the one-buffer kernel on expanded x-space blocks
+        for (int i = 0; i < c->nslices; ++i)
+            if (!c->slice[i].Be) {
+                CU(c, cudaSetDevice(c->device));
+                int rc = dev_alloc(c, c->slice[i].Be, c->V * c->Re);
+                if (rc) return rc;
+            }
     c->direct = enable != 0;
     return NBS_OK;
 }

@@ -206,7 +206,13 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
             if (kind == BK_FULL) {
                 if (tid < 24) sO[(tid / 12) * SM_PLANE + (tid % 12) * SM_STRIDE1 + 144] = make_double2(0.0, 0.0);
             } else {
-                if (tid < 48) sO[(tid / 12) * AS_PLANE + (tid % 12) * AS_ROW + 66] = make_double2(0.0, 0.0);
+                // unused positions of every row (read as the vanishing diagonal by the product kernel) and plane pads
+                for (int i = tid; i < 4 * (12 * AS_ROW_PADS + 4); i += BLOCKS_THREADS) {
+                    const int pl = i / (12 * AS_ROW_PADS + 4), j = i % (12 * AS_ROW_PADS + 4);
+                    const int c = j / AS_ROW_PADS, pos = j < 12 * AS_ROW_PADS ? c * AS_ROW + (as_pad_pos(j % AS_ROW_PADS) + c) % AS_ROW
+                                                                              : 12 * AS_ROW + (j - 12 * AS_ROW_PADS);
+                    sO[pl * AS_PLANE + pos] = make_double2(0.0, 0.0);
+                }
             }
             if (active) {
 #pragma unroll
@@ -222,7 +228,7 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                                     sO[a * SM_PLANE + sm_index(xi0, xi1, xi2)] = acc[a][e0][e1][e2];
                                 } else {
                                     const int xa = (kind == BK_ASYM13) ? xi0 : xi1, xc = (kind == BK_ASYM13) ? xi1 : xi0;
-                                    if (xa < xi2) sO[(a0 + a) * AS_PLANE + as_row_rank(xc) * AS_ROW + as_pair_index(xa, xi2)] = acc[a][e0][e1][e2];
+                                    if (xa < xi2) sO[(a0 + a) * AS_PLANE + as_index(xa, xi2, xc)] = acc[a][e0][e1][e2];
                                 }
                             }
             }

@@ -35,6 +35,7 @@ constexpr int PROD_CTHREADS = PROD_CWARPS * 32, PROD_ETHREADS = PROD_EWARPS * 32
 constexpr int PROD_THREADS = PROD_CTHREADS + PROD_ETHREADS;
 constexpr uint32_t PLANE_BYTES = SM_PLANE * 16u;  // 27 840
 constexpr uint32_t BLOCK_BYTES = SM_BLOCK * 16u;  // 111 360
+// osign of combine_item: only the pipelined kernel (nbs_product_c.cuh) passes a value other than 1.
 // shared-memory map (bytes)
 constexpr uint32_t SMO_S1 = 0, SMO_S2 = BLOCK_BYTES, SMO_UNITS = 2 * BLOCK_BYTES;
 constexpr uint32_t SMO_DIAGS = SMO_UNITS + MAX_PAIR_UNITS * 16u;
@@ -372,7 +373,7 @@ __device__ __forceinline__ size_t shifted_site(int L, size_t X, size_t r) { // X
 // instead of one per use); thread et owns the spin components et + 64 m.
 template <bool TILE>
 __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q, bool accumulate,
-                                             const double2* __restrict__ scr, int et, char* s_epi) {
+                                             const double2* __restrict__ scr, int et, char* s_epi, double osign = 1.0) {
     Pair3Rec* pr = reinterpret_cast<Pair3Rec*>(s_epi);
     PairChanRec* pcs = reinterpret_cast<PairChanRec*>(s_epi + EPI_PAIR_BYTES);
     {
@@ -464,6 +465,8 @@ __device__ __forceinline__ void combine_item(const ProdArgs& a, int ip, size_t q
             if (c < nc) {
                 const int ch = TILE ? pcs[c].local : pcs[c].ch - a.ch_begin;
                 if (ch >= 0 && ch < nrows) {
+#pragma unroll
+                    for (int m = 0; m < NM; ++m) { acc[c][m].x *= osign; acc[c][m].y *= osign; } // +-1 (isospin limit: sign of a derived block)
                     if (accumulate) { // direct mode, X > 0: the same thread wrote this entry for the previous X
 #pragma unroll
                         for (int m = 0; m < NM; ++m) {

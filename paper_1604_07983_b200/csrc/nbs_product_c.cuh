@@ -1,0 +1,396 @@
+// Pipelined variant of the product kernel (eqs. 4.2-4.3) for the resident plan.
+//
+// Same arithmetic as k_product_t<false> (nbs_product.cuh): per diagram a complex GEMM over the shared index on
+// DMMA.8x8x4, effective-block entries gathered straight into MMA fragments.  What changes is how the blocks
+// reach shared memory and how the warps move from one sink pair to the next:
+//   * antisymmetric blocks (p, n, Sigma+-, Xi0-) are staged in their COMPACT form (55.5 KB instead of 111 KB),
+//     exactly as the block kernel and the forward FFT leave them in HBM: no expansion pass, no second buffer.
+//     The gather tables address the compact layout; a mirrored entry changes sides of its (+, -) pair, and the
+//     few entries that end up with two terms of one sign carry a flag (bit 31 of the table word) that flips the
+//     sign of the loaded value with one integer instruction.
+//   * shared memory holds four block slots (a full block takes two).  The host simulated the walk over a task
+//     (momentum pair q, -q: full chain, then half chain) and wrote a static program (nbs_tables.hpp, CItem /
+//     CLoad): every item knows where its blocks are, which of them it must wait for, and which bulk copies may be
+//     issued the moment it is complete.  The warp that completes an item (last to arrive at its counter) issues
+//     those copies; nobody waits at an item boundary unless the block it needs is still on its way.  Warps run up
+//     to two items ahead of the slowest one, so the tail of a small sink pair is filled with units of the next.
+#pragma once
+#include "nbs_product.cuh"
+
+namespace nbs {
+
+struct CProdArgs {
+    ProdArgs base;        // pairs, pair_chans, Ft, ch_begin, nch_out, L, scratch, max_pair_units, counter (epilogue and bookkeeping)
+    const double2* B;     // [V][R] momentum-space blocks, compact rows
+    size_t R;
+    const int* slot_off;  // [slots] complex offset inside the row of the block staged for a slot (isospin limit: the partner's)
+    const double* pair_sign; // [pairs] +-1: product of the signs of the two staged blocks (isospin limit), else +1
+    long long ntasks;     // momentum pairs
+    const int* qhalf;     // [ntasks] the momenta q <= -q
+    const CItem* prog;
+    int nitems;
+    const CLoad* loads;
+    const Unit3Rec* units;
+    const Diag3Rec* diags; // compact-table diagram records (Plan::diagsc)
+    const uint2* tab;      // Plan::tabc
+    uint32_t rec_stride, units_bytes; // record buffer: units at 0, diagram records at units_bytes
+};
+
+struct CCtrl {
+    unsigned long long bar_slot[C_NSLOT]; // a block has landed in slot s
+    unsigned long long bar_rec[C_NREC];   // unit and diagram records of an item have landed
+    unsigned long long full[PROD_NBUF];   // all compute warps have written their unit results of the item in ring buffer b
+    unsigned long long empty[PROD_NBUF];  // the epilogue warps are done with ring buffer b
+    int next_unit[8], done_cnt[8];        // per item in flight (sequence number modulo 8)
+    long long qtask[4];                   // task indices of this CTA (task number modulo 4)
+    int meta_q[PROD_NBUF], meta_pair[PROD_NBUF];
+};
+constexpr uint32_t SMC_REC = C_NSLOT * C_SLOT_BYTES; // 222 720
+inline size_t cprod_smem_bytes(uint32_t rec_stride) {
+    return (size_t)SMC_REC + (size_t)C_NREC * rec_stride + EPI_PAIR_BYTES + EPI_CG * sizeof(PairChanRec) + 16 + sizeof(CCtrl);
+}
+
+__device__ __forceinline__ void mbar_arrive(void* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// value with its sign flipped if bit 31 of the table word is set
+__device__ __forceinline__ double flipd(double v, uint32_t w) {
+    return __hiloint2double(__double2hiint(v) ^ (int)(w & 0x80000000u), __double2loint(v));
+}
+// b0 / b1: the block at planes a and a + 2 (b1 = b0 + plane stride of the block's kind)
+template <int NP>
+__device__ __forceinline__ void ldc(const char* b0, const char* b1, uint2 w, double2 (&u)[NP], double2 (&v)[NP]) {
+    const uint32_t ox = w.x & 0x7fffffffu, oy = w.y & 0x7fffffffu;
+    u[0] = *reinterpret_cast<const double2*>(b0 + ox);
+    v[0] = *reinterpret_cast<const double2*>(b0 + oy);
+    if (NP == 2) {
+        u[NP - 1] = *reinterpret_cast<const double2*>(b1 + ox);
+        v[NP - 1] = *reinterpret_cast<const double2*>(b1 + oy);
+    }
+}
+template <int NP, bool FIRST>
+__device__ __forceinline__ void subc(const double2 (&u)[NP], const double2 (&v)[NP], uint2 w, double2 (&out)[NP]) {
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const double dx = flipd(u[p].x, w.x) - flipd(v[p].x, w.y), dy = flipd(u[p].y, w.x) - flipd(v[p].y, w.y);
+        if (FIRST) out[p] = make_double2(dx, dy);
+        else { out[p].x += dx; out[p].y += dy; }
+    }
+}
+
+struct CSides { const char *a0, *a1, *b0, *b1; }; // side 1 (B~1) planes a / a + 2, side 2 (B~2) likewise
+
+__device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3Rec* diags, const uint2* __restrict__ tab,
+                                                  const CSides sd, double2* __restrict__ out, int lane) {
+    const int r = lane >> 2, kk = lane & 3;
+    constexpr int NT = 2;
+    AccSquare<NT> acc = {};
+    for (int d = u.diag_begin; d < u.diag_end; ++d) {
+        const Diag3Rec dr = load_diag(diags + d);
+        const int nsteps = dr.send - dr.sbeg;
+        if (dr.nwA == 1) {
+            // software pipeline: table words two k-steps ahead, shared-memory gathers one ahead
+            const uint2* tA = tab + dr.offA + (dr.sbeg * 4 + kk) * 8 + r;
+            const uint2* tB = tab + dr.offB + (dr.sbeg * 4 + kk) * 8 + r;
+            uint2 wa = __ldg(tA), wb = __ldg(tB);
+            uint2 na = __ldg(tA + 32), nb = __ldg(tB + 32);
+            double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
+            ldc<NT>(sd.a0, sd.a1, wa, ua, va);
+            ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
+            subc<NT, true>(ua, va, wa, A);
+            subc<NT, true>(ub, vb, wb, B);
+            for (int s = 0; s < nsteps; ++s) {
+                tA += 32; tB += 32;
+                wa = na; wb = nb;
+                ldc<NT>(sd.a0, sd.a1, wa, ua, va); // one step past the end reads a valid (unused) entry
+                ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
+                na = __ldg(tA + 32); nb = __ldg(tB + 32);
+                prefetch_l1(tA + 5 * 32); prefetch_l1(tB + 5 * 32);
+                mma_square(acc, A, B);
+                subc<NT, true>(ua, va, wa, A);
+                subc<NT, true>(ub, vb, wb, B);
+            }
+        } else {
+            const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry)
+            const uint2* tA = tab + dr.offA + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
+            const uint2* tB = tab + dr.offB + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
+            for (int s = 0; s < nsteps; ++s, tA += 32 * nw, tB += 32 * nw) {
+                double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
+                uint2 wa = __ldg(tA), wb = __ldg(tB);
+                ldc<NT>(sd.a0, sd.a1, wa, ua, va);
+                ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
+                subc<NT, true>(ua, va, wa, A);
+                subc<NT, true>(ub, vb, wb, B);
+                for (int j = 1; j < nw; ++j) {
+                    wa = __ldg(tA + j); wb = __ldg(tB + j);
+                    ldc<NT>(sd.a0, sd.a1, wa, ua, va);
+                    ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
+                    subc<NT, false>(ua, va, wa, A);
+                    subc<NT, false>(ub, vb, wb, B);
+                }
+                mma_square(acc, A, B);
+            }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < NT; ++i)
+#pragma unroll
+        for (int j = 0; j < NT; ++j)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int a1 = 2 * i + (r & 1), c1 = r >> 1;
+                const int cc = 2 * kk + e, a2 = 2 * j + (cc & 1), c2 = cc >> 1;
+                const int a3 = u.cls == 0 ? c1 : c2, a4 = u.cls == 0 ? c2 : c1;
+                out[((a1 * 4 + a2) * 4 + a3) * 4 + a4] =
+                    make_double2(acc.p1[i][j][e] - acc.p2[i][j][e], acc.p3[i][j][e] - acc.p1[i][j][e] - acc.p2[i][j][e]);
+            }
+}
+
+__device__ __forceinline__ void wide_loads_A_c(const char* a0, const char* a1, uint4 a01, uint4 a23, double2 (&ua)[4][2],
+                                               double2 (&va)[4][2]) {
+    ldc<2>(a0, a1, make_uint2(a01.x, a01.y), ua[0], va[0]);
+    ldc<2>(a0, a1, make_uint2(a01.z, a01.w), ua[1], va[1]);
+    ldc<2>(a0, a1, make_uint2(a23.x, a23.y), ua[2], va[2]);
+    ldc<2>(a0, a1, make_uint2(a23.z, a23.w), ua[3], va[3]);
+}
+__device__ __forceinline__ void wide_subs_A_c(const double2 (&ua)[4][2], const double2 (&va)[4][2], uint4 a01, uint4 a23,
+                                              double2 (&A)[4][2]) {
+    subc<2, true>(ua[0], va[0], make_uint2(a01.x, a01.y), A[0]);
+    subc<2, true>(ua[1], va[1], make_uint2(a01.z, a01.w), A[1]);
+    subc<2, true>(ua[2], va[2], make_uint2(a23.x, a23.y), A[2]);
+    subc<2, true>(ua[3], va[3], make_uint2(a23.z, a23.w), A[3]);
+}
+__device__ __forceinline__ void wide_loads_B_c(const char* sB, uint4 bw, double2 (&ub)[2][1], double2 (&vb)[2][1]) {
+    ldc<1>(sB, sB, make_uint2(bw.x, bw.y), ub[0], vb[0]);
+    ldc<1>(sB, sB, make_uint2(bw.z, bw.w), ub[1], vb[1]);
+}
+__device__ __forceinline__ void wide_fold_B_c(const double2 (&ub)[2][1], const double2 (&vb)[2][1], uint4 bw, double2 (&Bv)[1]) {
+    double2 part[1];
+    subc<1, true>(ub[0], vb[0], make_uint2(bw.x, bw.y), part);
+    subc<1, false>(ub[1], vb[1], make_uint2(bw.z, bw.w), part);
+    const double ox = __shfl_xor_sync(0xffffffffu, part[0].x, 16), oy = __shfl_xor_sync(0xffffffffu, part[0].y, 16);
+    Bv[0] = make_double2(part[0].x + ox, part[0].y + oy);
+}
+
+__device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec* diags, const uint2* __restrict__ tab,
+                                                const CSides sd, double2* __restrict__ out, int lane) {
+    const int r = lane >> 2, kk = lane & 3, aY = r & 3, hi = r >> 2;
+    const char* a0 = (u.cls == 2) ? sd.a0 : sd.b0; // operand A = the block that carries a3 and a4
+    const char* a1 = (u.cls == 2) ? sd.a1 : sd.b1;
+    const char* sB = (u.cls == 2) ? sd.b0 : sd.a0;
+    constexpr int NJ = 2;
+    double acc[NJ * 4][2] = {};
+    for (int d = u.diag_begin; d < u.diag_end; ++d) {
+        const Diag3Rec dr = load_diag(diags + d); // nwA == 1, nwB == 4
+        const int nsteps = dr.send - dr.sbeg;
+        const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA) + ((dr.sbeg * 4 + kk) * 8 + r) * 2;
+        const uint4* tB = reinterpret_cast<const uint4*>(tab + dr.offB) + ((dr.sbeg * 4 + kk) * 4 + aY) * 2;
+        double2 A[4][NJ], Bv[1], ua[4][NJ], va[4][NJ], ub[2][1], vb[2][1];
+        uint4 a01 = __ldg(tA), a23 = __ldg(tA + 1), bw = __ldg(tB + hi);
+        wide_loads_A_c(a0, a1, a01, a23, ua, va);
+        wide_loads_B_c(sB, bw, ub, vb);
+        uint4 na01 = __ldg(tA + 64), na23 = __ldg(tA + 65), nbw = __ldg(tB + 32 + hi);
+        wide_subs_A_c(ua, va, a01, a23, A);
+        for (int s = 0; s < nsteps; ++s) {
+            tA += 64; tB += 32;
+            wide_fold_B_c(ub, vb, bw, Bv);
+            a01 = na01; a23 = na23;
+            wide_loads_A_c(a0, a1, a01, a23, ua, va); // one step past the end reads valid (unused) entries
+            na01 = __ldg(tA + 64); na23 = __ldg(tA + 65);
+            prefetch_l1(tA + 3 * 64); prefetch_l1(tB + 3 * 32);
+            mma_wide<NJ>(acc, A, Bv[0], hi);
+            wide_subs_A_c(ua, va, a01, a23, A);
+            bw = nbw;
+            wide_loads_B_c(sB, bw, ub, vb);
+            nbw = __ldg(tB + 32 + hi);
+        }
+    }
+    double* o = reinterpret_cast<double*>(out);
+#pragma unroll
+    for (int j = 0; j < NJ; ++j)
+#pragma unroll
+        for (int g = 0; g < 4; ++g)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int aX = 2 * j + (r & 1), cX = 4 * g + (r >> 1);
+                const int cc = 2 * kk + e, part = cc >> 2, ay = cc & 3;
+                const int a1s = u.cls == 2 ? aX : ay, a2s = u.cls == 2 ? ay : aX;
+                o[2 * ((a1s * 4 + a2s) * 16 + cX) + part] = acc[j * 4 + g][e];
+            }
+}
+
+__global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a) {
+    extern __shared__ __align__(128) char prod_smem[];
+    char* smem = prod_smem;
+    char* s_rec = smem + SMC_REC;
+    char* s_epi = s_rec + C_NREC * a.rec_stride;
+    CCtrl* ctlp = reinterpret_cast<CCtrl*>(s_epi + ((EPI_PAIR_BYTES + EPI_CG * (uint32_t)sizeof(PairChanRec) + 15u) & ~15u));
+    volatile CCtrl* ctl = ctlp;
+    const int tid = threadIdx.x;
+    const size_t scr_stride = (size_t)a.base.max_pair_units * 256;
+    double2* scr0 = a.base.scratch + (size_t)blockIdx.x * PROD_NBUF * scr_stride;
+
+    // bulk copies of one release-list entry for the task at momentum q (mq = -q)
+    auto issue_load = [&](const CLoad ld, size_t q, size_t mq) {
+        const size_t mom = ((ld.src >> 8) & 1) ? mq : q;
+        const char* src = reinterpret_cast<const char*>(a.B + mom * a.R + __ldg(a.slot_off + (ld.src & 255)));
+        void* bar = &ctlp->bar_slot[ld.bar];
+        mbar_expect_tx(bar, ld.bytes);
+        const uint32_t part = ld.bytes >> 2; // four copies in flight (a multiple of 16 bytes for both block kinds)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) bulk_g2s(smem + ld.dst + p * part, src + (size_t)p * part, part, bar);
+    };
+    auto issue_records = [&](int pos, int rb) {
+        const int4 h0 = __ldg(reinterpret_cast<const int4*>(a.prog + pos));     // pair, nunits, unit_begin, ndiags
+        const int4 h1 = __ldg(reinterpret_cast<const int4*>(a.prog + pos) + 1); // diag_begin, ...
+        const uint32_t ubytes = (uint32_t)h0.y * (uint32_t)sizeof(Unit3Rec), dbytes = (uint32_t)h0.w * (uint32_t)sizeof(Diag3Rec);
+        void* bar = &ctlp->bar_rec[rb];
+        mbar_expect_tx(bar, ubytes + dbytes);
+        bulk_g2s(s_rec + rb * a.rec_stride, a.units + h0.z, ubytes, bar);
+        bulk_g2s(s_rec + rb * a.rec_stride + a.units_bytes, a.diags + h1.x, dbytes, bar);
+    };
+
+    if (tid == 0) {
+        for (int i = 0; i < C_NSLOT; ++i) mbar_init(&ctlp->bar_slot[i], 1);
+        for (int i = 0; i < C_NREC; ++i) mbar_init(&ctlp->bar_rec[i], 1);
+        for (int i = 0; i < PROD_NBUF; ++i) { mbar_init(&ctlp->full[i], PROD_CWARPS); mbar_init(&ctlp->empty[i], 1); }
+        for (int i = 0; i < 8; ++i) { ctl->next_unit[i] = 0; ctl->done_cnt[i] = 0; }
+        const long long t0 = (long long)atomicAdd(a.base.counter, 1ull);
+        ctl->qtask[0] = t0;
+        ctl->qtask[1] = (long long)atomicAdd(a.base.counter, 1ull);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (t0 < a.ntasks) {
+            // prologue: what the previous task would have issued for this one, and the first record buffers
+            const size_t q = (size_t)__ldg(a.qhalf + t0), mq = minus_q(a.base.L, q);
+            for (int i = 0; i < a.nitems; ++i) {
+                const int4 h2 = __ldg(reinterpret_cast<const int4*>(a.prog + i) + 2); // ps2, flags, rel_begin, rel_end
+                for (int j = h2.z; j < h2.w; ++j) {
+                    const int4 lv = __ldg(reinterpret_cast<const int4*>(a.loads + j));
+                    CLoad ld; ld.src = lv.x; ld.dst = (uint32_t)lv.y; ld.bytes = (uint32_t)lv.z; ld.bar = lv.w;
+                    if ((ld.src >> 9) & 1) issue_load(ld, q, mq);
+                }
+            }
+            for (int i = 0; i < C_NREC; ++i) issue_records(i, i);
+        }
+    }
+    __syncthreads();
+
+    if (tid >= PROD_CTHREADS) {
+        // ---------------- epilogue warps: combine item i while the compute warps run the following items
+        const int et = tid - PROD_CTHREADS;
+        for (unsigned it = 0;; ++it) {
+            const int b = it % PROD_NBUF;
+            mbar_wait(&ctlp->full[b], (it / PROD_NBUF) & 1u);
+            const int ip = ctl->meta_pair[b];
+            if (ip < 0) break;
+            const size_t q = (size_t)ctl->meta_q[b];
+            combine_item<false>(a.base, ip, q, false, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
+            if (et == 0) mbar_arrive(&ctlp->empty[b]); // combine_item ends with a barrier of the epilogue threads
+        }
+        return;
+    }
+
+    // ---------------- compute warps
+    const int lane = tid & 31;
+    uint32_t par = 0;       // phase parities of the slot barriers (every warp sees every item)
+    unsigned seq = 0;       // items started by this warp
+    unsigned ntask = 0;
+    long long qt = ctl->qtask[0];
+    while (qt < a.ntasks) {
+        const size_t q = (size_t)__ldg(a.qhalf + qt), mq = minus_q(a.base.L, q);
+        const long long qn = ctl->qtask[(ntask + 1) & 3];
+        const bool next_valid = qn < a.ntasks;
+        int4 h0 = __ldg(reinterpret_cast<const int4*>(a.prog));
+        int4 h1 = __ldg(reinterpret_cast<const int4*>(a.prog) + 1);
+        int4 h2 = __ldg(reinterpret_cast<const int4*>(a.prog) + 2);
+        for (int pos = 0; pos < a.nitems; ++pos, ++seq) {
+            const int4 c0 = h0, c1 = h1, c2 = h2; // this item; fetch the next one under it
+            if (pos + 1 < a.nitems) {
+                h0 = __ldg(reinterpret_cast<const int4*>(a.prog + pos + 1));
+                h1 = __ldg(reinterpret_cast<const int4*>(a.prog + pos + 1) + 1);
+                h2 = __ldg(reinterpret_cast<const int4*>(a.prog + pos + 1) + 2);
+            }
+            const int ip = c0.x, nunits = c0.y, flags = c2.y;
+            const int b = seq % PROD_NBUF, rb = seq % C_NREC, cs = seq & 7;
+            if (seq >= PROD_NBUF) mbar_wait(&ctlp->empty[b], ((seq / PROD_NBUF) - 1u) & 1u); // ring buffer b is free again
+            mbar_wait(&ctlp->bar_rec[rb], (seq / C_NREC) & 1u);
+            const int w1 = flags & 7, w2 = (flags >> 3) & 7;
+            if (w1) { mbar_wait(&ctlp->bar_slot[w1 - 1], (par >> (w1 - 1)) & 1u); par ^= 1u << (w1 - 1); }
+            if (w2) { mbar_wait(&ctlp->bar_slot[w2 - 1], (par >> (w2 - 1)) & 1u); par ^= 1u << (w2 - 1); }
+            if (lane == 0) { // every warp writes the same descriptor (the epilogue reads it after the last arrival)
+                ctl->meta_q[b] = (int)((flags & 64) ? mq : q);
+                ctl->meta_pair[b] = ip;
+            }
+            const Unit3Rec* s_units = reinterpret_cast<const Unit3Rec*>(s_rec + rb * a.rec_stride);
+            const Diag3Rec* s_diags = reinterpret_cast<const Diag3Rec*>(s_rec + rb * a.rec_stride + a.units_bytes);
+            CSides sd;
+            sd.a0 = smem + (uint32_t)c1.y; sd.a1 = sd.a0 + (uint32_t)c1.w;
+            sd.b0 = smem + (uint32_t)c1.z; sd.b1 = sd.b0 + (uint32_t)c2.x;
+            double2* scr = scr0 + b * scr_stride;
+            int* next_unit = const_cast<int*>(&ctl->next_unit[cs]);
+            auto grab = [&]() {
+                int i = 0;
+                if (lane == 0) i = atomicAdd(next_unit, 1);
+                return __shfl_sync(0xffffffffu, i, 0);
+            };
+            int i = grab();
+            while (i < nunits) {
+                const int4 uv = *reinterpret_cast<const int4*>(s_units + i);
+                Unit3Rec u;
+                u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
+                if (i + PROD_CWARPS < nunits) prefetch_unit(s_units + i + PROD_CWARPS, s_diags, a.tab, lane);
+                double2* out = scr + (size_t)u.slot * 256;
+                if (u.cls < 2) run_unit_square_c(u, s_diags, a.tab, sd, out, lane);
+                else run_unit_wide_c(u, s_diags, a.tab, sd, out, lane);
+                i = grab();
+            }
+            __syncwarp();
+            int old = 0;
+            if (lane == 0) {
+                __threadfence_block();
+                mbar_arrive(&ctlp->full[b]);
+                old = atomicAdd(const_cast<int*>(&ctl->done_cnt[cs]), 1);
+            }
+            old = __shfl_sync(0xffffffffu, old, 0);
+            if (old == PROD_CWARPS - 1) {
+                // this warp completed the item: its blocks and records are free.  Lanes issue the release list in
+                // parallel; lane 31 loads the records of the item C_NREC positions ahead into the buffer just vacated.
+                __threadfence_block();
+                if (lane == 0) { ctl->done_cnt[cs] = 0; ctl->next_unit[cs] = 0; }
+                if (lane == 30 && pos == 0) ctl->qtask[(ntask + 2) & 3] = (long long)atomicAdd(a.base.counter, 1ull);
+                __threadfence_block();
+                const int rel_begin = c2.z, nrel = c2.w - c2.z;
+                if (lane < nrel) {
+                    const int4 lv = __ldg(reinterpret_cast<const int4*>(a.loads + rel_begin + lane));
+                    CLoad ld; ld.src = lv.x; ld.dst = (uint32_t)lv.y; ld.bytes = (uint32_t)lv.z; ld.bar = lv.w;
+                    if (!((ld.src >> 9) & 1)) issue_load(ld, q, mq);
+                    else if (next_valid) {
+                        const size_t q2 = (size_t)__ldg(a.qhalf + qn);
+                        issue_load(ld, q2, minus_q(a.base.L, q2));
+                    }
+                }
+                if (lane == 31) {
+                    const int pr = pos + C_NREC;
+                    if (pr < a.nitems) issue_records(pr, rb);
+                    else if (next_valid) issue_records(pr - a.nitems, rb);
+                }
+                __threadfence_block();
+            }
+            __syncwarp();
+        }
+        ++ntask;
+        qt = qn;
+    }
+    // no work left: tell the epilogue warps (every warp arrives; lane 0 of each writes the same end marker)
+    {
+        const int b = seq % PROD_NBUF;
+        if (seq >= PROD_NBUF) mbar_wait(&ctlp->empty[b], ((seq / PROD_NBUF) - 1u) & 1u);
+        if (lane == 0) {
+            ctl->meta_pair[b] = -1;
+            __threadfence_block();
+            mbar_arrive(&ctlp->full[b]);
+        }
+    }
+}
+
+} // namespace nbs

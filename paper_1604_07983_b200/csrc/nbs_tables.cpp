@@ -479,6 +479,52 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         dedupe3[w] = off;
         return off;
     };
+    // The same tables for the pipelined kernel, in the layout of the block of kind `kind` on that side (raw index
+    // triples from make_side).  An antisymmetric block is gathered from its compact form: a term whose stored
+    // partner carries the opposite sign changes sides (u <-> v); when an entry then has more terms of one sign than
+    // it has places for, the surplus goes to the other side with bit 31 set (the kernel flips the sign of the value
+    // it loads); the vanishing diagonal is read from a zero pad.
+    std::map<std::vector<uint32_t>, uint32_t> dedupec;
+    auto intern3c = [&](const SideTable& t, int layout, int kind) -> uint32_t {
+        const int Kp = (t.K + 3) / 4 * 4, nw = t.n / 2;
+        const int rows = (layout == 2) ? 4 : 8, G = (layout == 1) ? 4 : 1;
+        const uint32_t pl = (uint32_t)plane_elems(kind);
+        std::vector<uint32_t> w((size_t)(Kp + 4) * rows * G * nw * 2, 0u);
+        for (int k = 0; k < t.K; ++k)
+            for (int r = 0; r < rows; ++r)
+                for (int g = 0; g < G; ++g) {
+                    const int c = (layout == 0) ? (r >> 1) : (layout == 1) ? 4 * g + (r >> 1) : 0;
+                    const int plane = (layout == 2) ? r : (r & 1);
+                    std::vector<uint32_t> plus, minus, zeros;
+                    for (int j = 0; j < t.n; ++j) {
+                        const uint16_t e = t.g[((size_t)c * t.K + k) * t.n + j];
+                        const int tri = e & 0x7fff, sg = (e & 0x8000) ? -1 : 1;
+                        const Located loc = locate(kind, tri / 144, (tri / 12) % 12, tri % 12);
+                        const uint32_t off = ((uint32_t)plane * pl + (uint32_t)loc.idx) * 16u;
+                        if (loc.sign == 0) zeros.push_back(off);
+                        else ((sg * loc.sign < 0) ? minus : plus).push_back(off);
+                    }
+                    std::vector<uint32_t> U, V;
+                    for (uint32_t o : plus) { if ((int)U.size() < nw) U.push_back(o); else V.push_back(o | 0x80000000u); }
+                    for (uint32_t o : minus) { if ((int)V.size() < nw) V.push_back(o); else U.push_back(o | 0x80000000u); }
+                    for (uint32_t o : zeros) { if ((int)U.size() < nw) U.push_back(o); else V.push_back(o); }
+                    if ((int)U.size() != nw || (int)V.size() != nw) { tab_err = "internal: compact gather does not fit"; return 0; }
+                    for (int j = 0; j < nw; ++j) {
+                        const size_t o = ((((size_t)k * rows + r) * G + g) * nw + j) * 2;
+                        w[o] = U[j]; w[o + 1] = V[j];
+                    }
+                }
+        w.push_back((uint32_t)layout);
+        auto it = dedupec.find(w);
+        if (it != dedupec.end()) return it->second;
+        w.pop_back();
+        const uint32_t off = (uint32_t)plan.tabc.size();
+        for (size_t i = 0; i < w.size(); i += 2) plan.tabc.push_back(uint2x{w[i], w[i + 1]});
+        while (plan.tabc.size() % 2) plan.tabc.push_back(uint2x{0, 0});
+        w.push_back((uint32_t)layout);
+        dedupec[w] = off;
+        return off;
+    };
     const int UNIT_SPLIT_STEPS = unit_split_steps, UNIT_COST_MAX = unit_cost_max; // cost: 2 per 16x16 step, 3 per 64x4 step
     for (size_t ip = 0; ip < pair_list.size(); ++ip) {
         const std::vector<Key>& order = pair_comp_order[ip];
@@ -518,8 +564,15 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
                     const SideTable &A = (c == 3) ? s2 : s1, &B = (c == 3) ? s1 : s2;
                     if (c < 2 ? !(A.n == B.n && (A.n == 2 || A.n == 8 || A.n == 24)) : !(A.n == 2 && B.n == 8))
                         return "internal: unexpected gather lengths";
-                    Diag3Rec r;
+                    Diag3Rec r, rc;
                     r.offA = intern3(A, c < 2 ? 0 : 1); r.offB = intern3(B, c < 2 ? 0 : 2);
+                    {
+                        const SideTable r1 = make_side(d.P, d.sign, false), r2 = make_side(d.P + 3, +1, false);
+                        const int k1 = block_kind(pair_list[ip].first), k2 = block_kind(pair_list[ip].second);
+                        const SideTable &Ar = (c == 3) ? r2 : r1, &Br = (c == 3) ? r1 : r2;
+                        rc.offA = intern3c(Ar, c < 2 ? 0 : 1, (c == 3) ? k2 : k1);
+                        rc.offB = intern3c(Br, c < 2 ? 0 : 2, (c == 3) ? k1 : k2);
+                    }
                     if (!tab_err.empty()) return tab_err;
                     r.K = (uint16_t)s1.K;
                     (pr.self_swap ? plan.sumK_exec_self : plan.sumK_exec) += s1.K;
@@ -534,6 +587,8 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
                         const int cost = (se - sb) * (c >= 2 ? 3 : 2) * (c < 2 ? (int)r.nwA : 1) + 2;
                         if (ucost > 0 && ucost + cost > UNIT_COST_MAX) flush();
                         plan.diags3.push_back(r);
+                        rc.K = r.K; rc.nwA = r.nwA; rc.nwB = r.nwB; rc.sbeg = r.sbeg; rc.send = r.send;
+                        plan.diagsc.push_back(rc);
                         ucost += cost;
                         plan.sumKp_exec += 4 * (se - sb);
                     }
@@ -546,6 +601,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         if (pr.nunits > MAX_PAIR_UNITS || pr.ndiags > MAX_PAIR_DIAGS) return "internal: too many units for one sink pair";
         for (int e = pr.nelem; e <= MAX_PAIR_ELEMS; ++e) pr.elem_unit_begin[e] = pr.nunits;
         plan.max_pair_units = std::max(plan.max_pair_units, pr.nunits);
+        plan.max_pair_diags = std::max(plan.max_pair_diags, pr.ndiags);
         // schedule: units by decreasing cost (warps take them in this order)
         std::vector<int> idx(pr.nunits);
         for (int i = 0; i < pr.nunits; ++i) idx[i] = i;
@@ -573,6 +629,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         plan.pairs3.push_back(pr);
     }
     plan.tab3.insert(plan.tab3.end(), 1024, uint2x{0, 0}); // the kernel prefetches a few k-steps past a table's end
+    plan.tabc.insert(plan.tabc.end(), 4096, uint2x{0, 0}); // the same; covers the self-check's layout-blind bound
 
     // ---- chains: order of the sink pairs inside one momentum task that reloads the fewest blocks.
     // Full chain (all pairs) for the momenta q <= -q (index order), half chain (without the pairs of
@@ -641,6 +698,127 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         plan.chain_single_begin = (int)plan.chain.size();
         for (int i = 0; i < (int)plan.pairs3.size(); ++i) make_chain(std::vector<int>{i});
     }
+    // isospin limit: the compact blocks of the derived slots are those of their partners up to a sign
+    //   n(x1 x2 x3) = -p(x2 x1 x3): the compact entry [xi_c = x1][pair (x2, x3)] of n is minus the compact entry
+    //   [xi_c = x1][pair (x2', x3)] of p with its antisymmetric pair (x1', x3) = (x2, x3): the same position.
+    for (size_t sl = 0; sl < plan.baryons.size(); ++sl) {
+        const int b = plan.baryons[sl], partner = iso_partner(b);
+        plan.slot_partner_iso.push_back(partner >= 0 ? slot_of[partner] : (int)sl);
+        plan.slot_sign_iso.push_back(partner >= 0 && b != NBS_SIGMA_M ? -1 : +1);
+    }
+
+    // ---- program of the pipelined kernel (nbs_tables.hpp): simulate the walk over one task, full chain at q then
+    // half chain at -q, with four block slots; repeat from the end state until the assignment is periodic.
+    {
+        struct Need { int id, nslots; }; // id = block slot * 2 + (1 if taken at -q)
+        const int n = plan.chain_full_n + plan.chain_half_n;
+        auto need_of = [&](int i, int side) {
+            const ChainRec& cr = plan.chain[i];
+            const Pair3Rec& pr = plan.pairs3[cr.pair];
+            const bool neg = i >= plan.chain_full_n; // half chain: the item's momentum is -q
+            const int slot = side ? pr.slot2 : pr.slot1;
+            const int at_minus = (side == 1) != neg;  // B~1 at the item's momentum, B~2 at minus that
+            return Need{slot * 2 + (at_minus ? 1 : 0), plan.slot_kind[slot] == BK_FULL ? 2 : 1};
+        };
+        struct SlotState { int id = -1, last = -(1 << 20); };
+        struct Sched { std::vector<CItem> items; std::vector<std::vector<CLoad>> rel; bool ok = true; };
+        auto simulate = [&](std::array<SlotState, C_NSLOT>& st, bool drain) {
+            Sched sc;
+            sc.items.resize(n);
+            sc.rel.assign(n, {});
+            for (auto& x : st) x.id = -1; // blocks of the previous task are never reused (another momentum)
+            if (drain) for (auto& x : st) x.last = -1; // every slot is free when the last item of the previous task is complete
+            for (int i = 0; i < n; ++i) {
+                const ChainRec& cr = plan.chain[i];
+                CItem& it = sc.items[i];
+                it.pair = cr.pair; it.nunits = cr.nunits; it.unit_begin = cr.unit_begin; it.ndiags = cr.ndiags;
+                it.diag_begin = cr.diag_begin;
+                it.flags = (i >= plan.chain_full_n) ? 64 : 0;
+                it.rel_begin = it.rel_end = 0;
+                int base[2] = {-1, -1};
+                bool fresh[2] = {false, false};
+                const Need nd[2] = {need_of(i, 0), need_of(i, 1)};
+                for (int side = 0; side < 2; ++side) // resident blocks first
+                    for (int s = 0; s < C_NSLOT; ++s)
+                        if (base[side] < 0 && st[s].id == nd[side].id && (s == 0 || st[s - 1].id != nd[side].id)) base[side] = s;
+                for (int side = 0; side < 2; ++side) {
+                    if (base[side] >= 0) continue;
+                    const int other = 1 - side;
+                    auto taken = [&](int s) { // slot s belongs to the other block of this item
+                        return base[other] >= 0 && s >= base[other] && s < base[other] + nd[other].nslots;
+                    };
+                    int best = -1, best_last = 1 << 30;
+                    for (int s = 0; s + nd[side].nslots <= C_NSLOT; s += nd[side].nslots) {
+                        bool free_ok = true;
+                        int last = -(1 << 20);
+                        for (int k = s; k < s + nd[side].nslots; ++k) { free_ok = free_ok && !taken(k); last = std::max(last, st[k].last); }
+                        // an antisymmetric block prefers a slot whose neighbour is busy as well (keeps pairs of slots free for full blocks)
+                        if (free_ok && last < best_last) { best = s; best_last = last; }
+                    }
+                    if (best < 0 || best_last >= i) { sc.ok = false; return sc; }
+                    base[side] = best; fresh[side] = true;
+                    CLoad ld;
+                    ld.src = (nd[side].id >> 1) | ((nd[side].id & 1) << 8);
+                    ld.dst = (uint32_t)best * C_SLOT_BYTES;
+                    ld.bytes = (uint32_t)block_elems(plan.slot_kind[nd[side].id >> 1]) * 16u;
+                    ld.bar = best;
+                    int dep = best_last; // the item whose completion frees the destination; < 0: an item of the previous task
+                    if (dep < -n) dep = -n; // free from the start: issue with the first item of the previous task
+                    if (dep < 0) { ld.src |= 1 << 9; sc.rel[dep + n].push_back(ld); }
+                    else sc.rel[dep].push_back(ld);
+                    for (int k = best; k < best + nd[side].nslots; ++k) st[k].id = -1; // whatever lived there is overwritten
+                    st[best].id = nd[side].id;
+                    if (nd[side].nslots == 2) st[best + 1].id = nd[side].id;
+                }
+                for (int side = 0; side < 2; ++side)
+                    for (int k = base[side]; k < base[side] + nd[side].nslots; ++k) st[k].last = i;
+                it.off1 = (uint32_t)base[0] * C_SLOT_BYTES; it.off2 = (uint32_t)base[1] * C_SLOT_BYTES;
+                it.ps1 = 2u * (uint32_t)plane_elems(plan.slot_kind[nd[0].id >> 1]) * 16u;
+                it.ps2 = 2u * (uint32_t)plane_elems(plan.slot_kind[nd[1].id >> 1]) * 16u;
+                if (fresh[0]) it.flags |= 1 + base[0];
+                if (fresh[1]) it.flags |= (1 + base[1]) << 3;
+            }
+            for (auto& x : st) x.last -= n; // relative to the next task
+            return sc;
+        };
+        auto same = [](const Sched& a, const Sched& b) {
+            if (a.items.size() != b.items.size()) return false;
+            for (size_t i = 0; i < a.items.size(); ++i) {
+                if (a.items[i].off1 != b.items[i].off1 || a.items[i].off2 != b.items[i].off2 || a.items[i].flags != b.items[i].flags) return false;
+                if (a.rel[i].size() != b.rel[i].size()) return false;
+                for (size_t j = 0; j < a.rel[i].size(); ++j)
+                    if (a.rel[i][j].src != b.rel[i][j].src || a.rel[i][j].dst != b.rel[i][j].dst) return false;
+            }
+            return true;
+        };
+        plan.cprog_ok = false;
+        if (n >= C_NREC) {
+            std::array<SlotState, C_NSLOT> st;
+            Sched prev, cur;
+            bool periodic = false;
+            for (int iter = 0; iter < 8 && !periodic; ++iter) {
+                cur = simulate(st, false);
+                if (!cur.ok) break;
+                periodic = iter > 0 && same(prev, cur);
+                prev = cur;
+            }
+            if (!periodic) {
+                std::array<SlotState, C_NSLOT> st2;
+                cur = simulate(st2, true);
+                plan.cprog_drain = 1;
+            }
+            if (cur.ok) {
+                for (int i = 0; i < n; ++i) {
+                    cur.items[i].rel_begin = (int)plan.cloads.size();
+                    for (auto& ld : cur.rel[i]) plan.cloads.push_back(ld);
+                    cur.items[i].rel_end = (int)plan.cloads.size();
+                }
+                plan.cprog = cur.items;
+                plan.cprog_ok = true;
+            }
+        }
+    }
+
     // tile-wise plan: expansion map of a two-plane chunk of an antisymmetric block
     for (int kind = BK_ASYM13; kind <= BK_ASYM23; ++kind) {
         std::vector<int>& g = plan.gather_pp[kind - 1];

@@ -31,31 +31,41 @@ NBS_HD constexpr int sm_index(int xi1, int xi2, int xi3) { return xi1 * SM_STRID
 
 // Blocks of baryons with two quarks of one flavour are antisymmetric under the exchange of those
 // two source slots (the Wick sign of exchanging the two identical quark fields): p, Sigma+, Sigma-
-// in slots (1,3), n, Xi0, Xi- in slots (2,3).  Only the entries with xi_a < xi_b are built and
-// Fourier transformed (66 of 144 index pairs; 46 % of the data), in the "compact" layout
-//   antisymmetric plane: [rank(xi_c) (free slot): 12][pair (xi_a < xi_b): 66, then one pad]  (row 67),
-//   rank(xi) = 6 (xi & 1) + (xi >> 1): the lanes of the block kernel (tile origins xi_c = 2 i_c fastest, then
-//   xi_b = 2 i_b) store to rows 67 apart and pairs 2 apart, 3 n + const modulo the 8 bank groups;
-// after the transform they are expanded (mirror entries with the sign flipped, diagonal zero) into
-// the full staged layout the product kernel gathers from.
+// in slots (1,3), n, Xi0, Xi- in slots (2,3).  Only the entries with xi_a < xi_b are built, Fourier
+// transformed and staged by the product kernel (66 of 144 index pairs), in the "compact" layout
+//   antisymmetric plane: [xi_c (free slot): 12][72 positions] + 4 pads = 868 entries,
+//   the pair (xi_a < xi_b) of row xi_c at position (as_pair_pos(xi_a, xi_b) + xi_c) mod 72,
+// where as_pair_pos = 4 m + (xi_a + xi_b) mod 4 with m a running number inside the residue class.  The position
+// is therefore congruent to xi_a + xi_b + xi_c modulo 4 -- the same rule as sm_index -- and the plane stride
+// 868 = 4 (mod 8): every gather pattern that is free of bank conflicts on a full staged block is free of them on
+// the compact block too, mirrored entries included (the sum is symmetric in xi_a, xi_b).  The six unused
+// positions of a row (52, 54, 60, 62, 68, 70 before the rotation) and the plane pads are zero; the identically
+// vanishing diagonal xi_a == xi_b is read from the unused position of the matching residue.
 enum { BK_FULL = 0, BK_ASYM13 = 1, BK_ASYM23 = 2 };
-constexpr int AS_ROW = 67;
-constexpr int AS_PLANE = 12 * AS_ROW;  // 804
-constexpr int AS_BLOCK = 4 * AS_PLANE; // 3216 complex per compact antisymmetric block
-NBS_HD constexpr int as_pair_index(int a, int b) { return a * (23 - a) / 2 + (b - a - 1); } // a < b
-NBS_HD constexpr int as_row_rank(int c) { return (c & 1) * 6 + (c >> 1); }
+constexpr int AS_ROW = 72;
+constexpr int AS_PLANE = 12 * AS_ROW + 4; // 868
+constexpr int AS_BLOCK = 4 * AS_PLANE;    // 3472 complex per compact antisymmetric block
+constexpr int AS_ROW_PADS = 6;
+NBS_HD constexpr int as_pad_pos(int i) { return 52 + 8 * (i >> 1) + 2 * (i & 1); } // 52, 54, 60, 62, 68, 70
+NBS_HD constexpr int as_pair_pos(int a, int b) { // a < b
+    const int a0 = a & 3, a1 = a >> 2, b1 = b >> 2, rho = (a + b) & 3;
+    const int m = (a1 < b1) ? a0 + 4 * (a1 + b1 - 1) : 12 + 2 * a1 + ((a0 >> 1) | (a0 & (rho >> 1)));
+    return 4 * m + rho;
+}
+NBS_HD constexpr int as_index(int a, int b, int c) { return c * AS_ROW + (as_pair_pos(a, b) + c) % AS_ROW; } // a < b
+NBS_HD constexpr int as_zero_index(int a, int c) { return c * AS_ROW + (52 + ((2 * a) & 3) + c) % AS_ROW; } // a == b
 NBS_HD constexpr int plane_elems(int kind) { return kind == BK_FULL ? SM_PLANE : AS_PLANE; }
 NBS_HD constexpr int block_elems(int kind) { return 4 * plane_elems(kind); }
 struct Located {
     int idx;  // position inside the sink-spin plane of the compact layout
-    int sign; // +1, or -1 if the stored partner carries the opposite sign
+    int sign; // +1, or -1 if the stored partner carries the opposite sign; 0: identically zero (idx = a zero pad)
 };
 NBS_HD constexpr Located locate(int kind, int xi1, int xi2, int xi3) {
     if (kind == BK_FULL) return Located{sm_index(xi1, xi2, xi3), 1};
     const int a = (kind == BK_ASYM13) ? xi1 : xi2, b = xi3, c = (kind == BK_ASYM13) ? xi2 : xi1;
-    if (a == b) return Located{as_row_rank(c) * AS_ROW + 66, 1}; // identically zero (the pad)
-    if (a < b) return Located{as_row_rank(c) * AS_ROW + as_pair_index(a, b), 1};
-    return Located{as_row_rank(c) * AS_ROW + as_pair_index(b, a), -1};
+    if (a == b) return Located{as_zero_index(a, c), 0};
+    if (a < b) return Located{as_index(a, b, c), 1};
+    return Located{as_index(b, a, c), -1};
 }
 int block_kind(int baryon); // from the slot flavours of eqs. 2.2-2.3
 
@@ -135,6 +145,33 @@ struct ChainRec { // order in which one CTA walks the sink pairs of one momentum
     int buf1, off1, buf2, off2; // Plan::slot_src of the two blocks
 };
 
+// ---- pipelined product kernel (k_product_c): compact antisymmetric blocks staged as they are -------------
+// Shared memory holds four block slots of C_SLOT_BYTES: a compact antisymmetric block takes one, a full staged
+// block two adjacent ones (0-1 or 2-3).  One task = one momentum pair (q, -q): the full chain at q followed by
+// the half chain at -q.  The host simulates the walk once (build_plan) and writes a static program: for every
+// item the slots of its two blocks, which of them are fresh loads (the item waits for the slot's barrier), and
+// a release list -- the bulk copies that may be issued as soon as the item is complete, because they overwrite
+// blocks that nobody needs any more.  The program is cyclic: release lists near its end carry the first loads of
+// the next task.
+constexpr uint32_t C_SLOT_BYTES = 2u * SM_PLANE * 16u; // 55 680 >= AS_BLOCK * 16 = 55 552
+constexpr int C_NSLOT = 4;
+constexpr int C_NREC = 3; // unit / diagram record buffers: a warp may run two items ahead of the slowest one
+struct CItem { // 48 bytes, read as three int4
+    int pair, nunits, unit_begin, ndiags;
+    int diag_begin;
+    uint32_t off1, off2;     // shared-memory byte offsets of B~1 and B~2 of this item
+    uint32_t ps1, ps2;       // byte stride between the sink-spin planes a and a + 2 of the two blocks
+    int flags;               // bits 0-2: 1 + slot to wait for on side 1 (0: resident); bits 3-5: same for side 2;
+                             // bit 6: the item belongs to momentum -q of the task (half chain)
+    int rel_begin, rel_end;  // release list (Plan::cloads) of this item
+};
+struct CLoad { // 16 bytes
+    int src;        // bits 0-7: block slot (Plan::baryons index); bit 8: at -q; bit 9: of the next task
+    uint32_t dst;   // shared-memory byte offset
+    uint32_t bytes;
+    int bar;        // slot barrier that completes
+};
+
 struct uint2x { uint32_t x, y; }; // host mirror of CUDA uint2
 struct int2x { int x, y; };
 
@@ -182,7 +219,19 @@ struct Plan {
     // gather_pp[j] & 0x3fffffff of the same site's compact plane pair [2][AS_PLANE], negated if bit 30 is set; -1 = zero.
     std::vector<int> gather_pp[2];
     int max_pair_units = 0;
+    int max_pair_diags = 0;
     double sumKp_exec = 0; // executed k-steps x 4 (padding included)
+    // pipelined kernel: gather tables in the layout of the block kind of each side (compact for antisymmetric
+    // blocks; bit 31 of a word = the term enters with the opposite sign), one diagram record per entry of diags3
+    std::vector<uint2x> tabc;
+    std::vector<Diag3Rec> diagsc;
+    std::vector<CItem> cprog;   // one task: full chain at q, half chain at -q
+    std::vector<CLoad> cloads;
+    bool cprog_ok = false;      // false: the plan is too small / too large for the pipelined kernel
+    int cprog_drain = 0;        // 1: no periodic slot assignment was found, every task starts from empty slots
+    // isospin limit (d == u): derived slots are read from their partner's compact block with a sign
+    std::vector<int> slot_partner_iso;  // [slot] slot to read (itself if not derived)
+    std::vector<int> slot_sign_iso;     // [slot] +1 / -1
 };
 
 // Returns "" on success, else an error message (invalid id, flavour violation).

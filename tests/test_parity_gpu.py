@@ -687,8 +687,8 @@ def test_tilewise_plan_equals_resident_plan_and_oracle(torch_cuda, nbs, oracle, 
     B = oracle.all_blocks(S, oracle.sink_names(chans))
     Fo = oracle.correlator_fft(L, B, chans)
     assert_parity(F_res, Fo, chans)
-    # resident: B [V][33216] + Be [V][6 * 6960] + Ft [V][52][256]; tile-wise: n chunks [V][3480] + Ft [V][6][256]
-    base = ws_res - V * (33216 + 6 * 6960 + 52 * 256) * 16
+    # resident: B [V][34752] (compact rows; no expanded copy with the pipelined kernel) + Ft [V][52][256]; tile-wise: n chunks [V][3480] + Ft [V][6][256]
+    base = ws_res - V * (34752 + 52 * 256) * 16
     for nchunks in (2, 3):
         budget = base + V * (nchunks * 3480 + 6 * 256) * 16 + V * 3480 * 8  # half a chunk of slack
         with nbs.Nbs(L, 1, workspace_budget_bytes=budget) as ctx:
@@ -757,7 +757,7 @@ def test_repeated_runs_are_bitwise_identical(torch_cuda, nbs):
     with nbs.Nbs(L, 1) as ctx:
         ws1 = ctx.workspace_bytes()
     V = L ** 3
-    base = ws1 - V * (33216 + 6 * 6960 + 52 * 256) * 16
+    base = ws1 - V * (34752 + 52 * 256) * 16
     with nbs.Nbs(L, 1, workspace_budget_bytes=base + V * (2 * 3480 + 6 * 256) * 16 + V * 3480 * 8) as ctx:
         assert ctx.tiled_info()["tiled"]
         first = None
