@@ -43,6 +43,7 @@ def stale() -> bool:
 
 def build(verbose: bool = False) -> str:
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
+    flags += os.environ.get("NBS_NVCC_FLAGS", "").split()  # e.g. -DNBS_PROF: cycle counters of the product kernel
     cmd = [_nvcc(), *flags, "-I", INCLUDE, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")

@@ -61,7 +61,7 @@ struct nbs_ctx {
     int prod_grid = 0;
     // pipelined product kernel (nbs_product_c.cuh): compact antisymmetric blocks staged as they are, no expansion
     bool use_c = false;
-    uint2x* d_tabc = nullptr;
+    uint32_t* d_tabc = nullptr;
     Diag3Rec* d_diagsc = nullptr;
     CItem* d_cprog = nullptr;
     CLoad* d_cloads = nullptr;
@@ -444,18 +444,35 @@ int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
     if (P.diagsc.size() != P.diags3.size()) return -130;
     {   // 5: compact gather tables and the program of the pipelined kernel
         const size_t ntabc = P.tabc.size();
-        for (auto& w : P.tabc) {
-            const uint32_t x = w.x & 0x7fffffffu, y = w.y & 0x7fffffffu;
-            if (x % 16 || y % 16 || x >= BLOCK_BYTES || y >= BLOCK_BYTES) return -131;
-        }
+        for (uint32_t w : P.tabc) // offsets inside one plane, 16-byte aligned (the kind of the block is checked per unit below)
+            if ((w & 0xfu) || ((w >> 16) & 0xfu) || (w & 0x7ff0u) >= PLANE_BYTES || ((w >> 16) & 0x7ff0u) >= PLANE_BYTES) return -131;
         for (size_t i = 0; i < P.diagsc.size(); ++i) {
             const Diag3Rec &d = P.diagsc[i], &o = P.diags3[i];
             if (d.sbeg != o.sbeg || d.send != o.send || d.nwA != o.nwA || d.nwB != o.nwB || d.K != o.K) return -132;
-            const size_t stepA = 4 * 8 * (size_t)d.nwA, stepB4 = 4 * 4 * (size_t)d.nwB, stepB8 = 4 * 8 * (size_t)d.nwB;
-            if (d.offA + (size_t)(d.send + 1) * std::max<size_t>(stepA, 4 * 8 * 4) > ntabc) return -133;
-            if (d.offB + (size_t)(d.send + 1) * std::max(stepB4, stepB8) > ntabc) return -134;
-            if (d.offA % 2 || d.offB % 2) return -135;
+            if (d.offA % 4 || d.offB % 4) return -135;
         }
+        for (auto& pr : P.pairs3) // table extents with the register pipeline's look-ahead, by class of the unit
+            for (int u = 0; u < pr.nunits; ++u) {
+                const Unit3Rec& ur = P.units3[pr.unit_begin + u];
+                const int k1 = P.slot_kind[pr.slot1], k2 = P.slot_kind[pr.slot2];
+                for (int di = ur.diag_begin; di < ur.diag_end; ++di) {
+                    const Diag3Rec& d = P.diagsc[pr.diag_begin + di];
+                    const size_t steps = (size_t)d.send + C_TAB_LOOKAHEAD;
+                    const size_t wordsA = ur.cls < 2 ? 16 * (size_t)d.nwA : 64, wordsB = ur.cls < 2 ? 16 * (size_t)d.nwB : 16;
+                    if (d.offA + steps * wordsA > ntabc) return -133;
+                    if (d.offB + steps * wordsB > ntabc) return -134;
+                    // the words really used stay inside a plane of the block they address
+                    const int kA = ur.cls == 3 ? k2 : k1, kB = ur.cls == 3 ? k1 : k2;
+                    for (size_t x = (size_t)d.sbeg * wordsA; x < (size_t)d.send * wordsA; ++x) {
+                        const uint32_t w = P.tabc[d.offA + x];
+                        if ((w & 0x7ff0u) >= (uint32_t)plane_elems(kA) * 16u || ((w >> 16) & 0x7ff0u) >= (uint32_t)plane_elems(kA) * 16u) return -148;
+                    }
+                    for (size_t x = (size_t)d.sbeg * wordsB; x < (size_t)d.send * wordsB; ++x) {
+                        const uint32_t w = P.tabc[d.offB + x];
+                        if ((w & 0x7ff0u) >= (uint32_t)plane_elems(kB) * 16u || ((w >> 16) & 0x7ff0u) >= (uint32_t)plane_elems(kB) * 16u) return -149;
+                    }
+                }
+            }
         if (P.cprog_ok) {
             if ((int)P.cprog.size() != P.chain_full_n + P.chain_half_n || (int)P.cprog.size() < C_NREC) return -136;
             std::vector<int> fresh(C_NSLOT, 0), loaded(C_NSLOT, 0);
@@ -909,7 +926,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
             ca.pair_sign = iso ? c->d_pair_sign_iso : c->d_pair_sign;
             ca.ntasks = c->ntasks_half; ca.qhalf = c->d_qorder_half;
             ca.prog = c->d_cprog; ca.nitems = (int)c->plan.cprog.size(); ca.loads = c->d_cloads;
-            ca.units = c->d_units3; ca.diags = c->d_diagsc; ca.tab = reinterpret_cast<const uint2*>(c->d_tabc);
+            ca.units = c->d_units3; ca.diags = c->d_diagsc; ca.tab = c->d_tabc;
             ca.rec_stride = c->c_rec_stride; ca.units_bytes = c->c_units_bytes;
             grid = (unsigned)std::min<long long>(c->prod_grid, ca.ntasks);
             k_product_c<<<grid, PROD_THREADS, c->c_smem, st>>>(ca);
@@ -970,6 +987,19 @@ int nbs_stage_times(nbs_ctx* c, double* ms, long long* calls, int reset) {
         c->event_pool.push_back(p.b);
     }
     c->pending.clear();
+#ifdef NBS_PROF
+    {
+        unsigned long long pf[PF_N] = {}, zero[PF_N] = {};
+        cudaMemcpyFromSymbol(pf, g_cprof, sizeof(pf));
+        cudaMemcpyToSymbol(g_cprof, zero, sizeof(zero));
+        static const char* names[PF_N] = {"total", "units", "wait_empty", "wait_rec", "wait_slot", "release", "flush"};
+        if (pf[PF_TOTAL]) {
+            fprintf(stderr, "[NBS_PROF] compute-warp cycles:");
+            for (int i = 0; i < PF_N; ++i) fprintf(stderr, " %s %.2f%%", names[i], 100.0 * (double)pf[i] / (double)pf[PF_TOTAL]);
+            fprintf(stderr, "\n");
+        }
+    }
+#endif
     for (int i = 0; i < NBS_NUM_STAGES; ++i) {
         if (ms) ms[i] = c->stage_ms[i];
         if (calls) calls[i] = c->stage_calls[i];

@@ -32,7 +32,7 @@ struct CProdArgs {
     const CLoad* loads;
     const Unit3Rec* units;
     const Diag3Rec* diags; // compact-table diagram records (Plan::diagsc)
-    const uint2* tab;      // Plan::tabc
+    const uint32_t* tab;   // Plan::tabc, packed words
     uint32_t rec_stride, units_bytes; // record buffer: units at 0, diagram records at units_bytes
 };
 
@@ -53,80 +53,109 @@ inline size_t cprod_smem_bytes(uint32_t rec_stride) {
 __device__ __forceinline__ void mbar_arrive(void* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// value with its sign flipped if bit 31 of the table word is set
+// value with its sign flipped if bit 31 of w is set
 __device__ __forceinline__ double flipd(double v, uint32_t w) {
     return __hiloint2double(__double2hiint(v) ^ (int)(w & 0x80000000u), __double2loint(v));
 }
-// b0 / b1: the block at planes a and a + 2 (b1 = b0 + plane stride of the block's kind)
+// One packed table word (nbs_tables.hpp) = one (+, -) pair of gather terms.  p0 / p1: the lane's sink-spin plane a
+// and plane a + 2 of the staged block.
 template <int NP>
-__device__ __forceinline__ void ldc(const char* b0, const char* b1, uint2 w, double2 (&u)[NP], double2 (&v)[NP]) {
-    const uint32_t ox = w.x & 0x7fffffffu, oy = w.y & 0x7fffffffu;
-    u[0] = *reinterpret_cast<const double2*>(b0 + ox);
-    v[0] = *reinterpret_cast<const double2*>(b0 + oy);
+__device__ __forceinline__ void ldc(const char* p0, const char* p1, uint32_t w, double2 (&u)[NP], double2 (&v)[NP]) {
+    const uint32_t ox = w & 0x7ff0u, oy = (w >> 16) & 0x7ff0u;
+    u[0] = *reinterpret_cast<const double2*>(p0 + ox);
+    v[0] = *reinterpret_cast<const double2*>(p0 + oy);
     if (NP == 2) {
-        u[NP - 1] = *reinterpret_cast<const double2*>(b1 + ox);
-        v[NP - 1] = *reinterpret_cast<const double2*>(b1 + oy);
+        u[NP - 1] = *reinterpret_cast<const double2*>(p1 + ox);
+        v[NP - 1] = *reinterpret_cast<const double2*>(p1 + oy);
     }
 }
 template <int NP, bool FIRST>
-__device__ __forceinline__ void subc(const double2 (&u)[NP], const double2 (&v)[NP], uint2 w, double2 (&out)[NP]) {
+__device__ __forceinline__ void subc(const double2 (&u)[NP], const double2 (&v)[NP], uint32_t w, double2 (&out)[NP]) {
+    const uint32_t fu = w << 16; // flip flag of the + term to bit 31
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
-        const double dx = flipd(u[p].x, w.x) - flipd(v[p].x, w.y), dy = flipd(u[p].y, w.x) - flipd(v[p].y, w.y);
+        const double dx = flipd(u[p].x, fu) - flipd(v[p].x, w), dy = flipd(u[p].y, fu) - flipd(v[p].y, w);
         if (FIRST) out[p] = make_double2(dx, dy);
         else { out[p].x += dx; out[p].y += dy; }
     }
 }
+__device__ __forceinline__ uint32_t ldw(const uint32_t* p) { return __ldg(p); }
 
-struct CSides { const char *a0, *a1, *b0, *b1; }; // side 1 (B~1) planes a / a + 2, side 2 (B~2) likewise
+// -DNBS_PROF: cycle counters of the compute warps, summed over the launch (read by nbs_stage_times, printed to stderr)
+#ifdef NBS_PROF
+enum { PF_TOTAL, PF_UNITS, PF_EMPTY, PF_REC, PF_SLOT, PF_RELEASE, PF_FLUSH, PF_N };
+__device__ unsigned long long g_cprof[PF_N];
+#define PF_T(var) const long long var = clock64()
+#define PF_ADD(idx, t0) pf[idx] += clock64() - (t0)
+#else
+#define PF_T(var)
+#define PF_ADD(idx, t0)
+#endif
 
-__device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3Rec* diags, const uint2* __restrict__ tab,
+// Per-lane views of the two staged blocks of an item: a0 / a1 = B~1 at the lane's plane (r & 1) and two planes
+// further, b0 / b1 the same for B~2; w1 / w2 = plane (r & 3) of B~1 / B~2 (operand B of the 64 x 4 classes).
+struct CSides { const char *a0, *a1, *b0, *b1, *w1, *w2; };
+
+// L1 prefetch of the head of the two gather tables of a diagram record (dp: shared memory)
+__device__ __forceinline__ void prefetch_diag_c(const Diag3Rec* dp, bool wide, const uint32_t* __restrict__ tab, int lane) {
+    if (lane < 12) {
+        const int4 dv = *reinterpret_cast<const int4*>(dp);
+        const uint32_t sbeg = (uint32_t)dv.z & 0xffffu, nwA = (uint32_t)dv.w & 0xffu, nwB = ((uint32_t)dv.w >> 8) & 0xffu;
+        const uint32_t off = (lane < 8) ? (uint32_t)dv.x + sbeg * (wide ? 64u : 16u * nwA) : (uint32_t)dv.y + sbeg * (wide ? 16u : 16u * nwB);
+        prefetch_l1(reinterpret_cast<const char*>(tab + off) + (lane & 7) * 128);
+    }
+}
+
+__device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3Rec* diags, const uint32_t* __restrict__ tab,
                                                   const CSides sd, double2* __restrict__ out, int lane) {
-    const int r = lane >> 2, kk = lane & 3;
+    const int r = lane >> 2, kk = lane & 3, c = r >> 1;
     constexpr int NT = 2;
     AccSquare<NT> acc = {};
     for (int d = u.diag_begin; d < u.diag_end; ++d) {
         const Diag3Rec dr = load_diag(diags + d);
+        if (d + 1 < u.diag_end) prefetch_diag_c(diags + d + 1, false, tab, lane);
         const int nsteps = dr.send - dr.sbeg;
         if (dr.nwA == 1) {
-            // software pipeline: table words two k-steps ahead, shared-memory gathers one ahead
-            const uint2* tA = tab + dr.offA + (dr.sbeg * 4 + kk) * 8 + r;
-            const uint2* tB = tab + dr.offB + (dr.sbeg * 4 + kk) * 8 + r;
-            uint2 wa = __ldg(tA), wb = __ldg(tB);
-            uint2 na = __ldg(tA + 32), nb = __ldg(tB + 32);
+            // software pipeline: table words four k-steps ahead in registers, shared-memory gathers one ahead
+            const uint32_t* tA = tab + dr.offA + dr.sbeg * 16 + kk * 4 + c;
+            const uint32_t* tB = tab + dr.offB + dr.sbeg * 16 + kk * 4 + c;
+            const uint32_t wa0 = ldw(tA), wb0 = ldw(tB);
+            uint32_t wa1 = ldw(tA + 16), wb1 = ldw(tB + 16), wa2 = ldw(tA + 32), wb2 = ldw(tB + 32);
+            uint32_t wa3 = ldw(tA + 48), wb3 = ldw(tB + 48), wa4 = ldw(tA + 64), wb4 = ldw(tB + 64);
             double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
-            ldc<NT>(sd.a0, sd.a1, wa, ua, va);
-            ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
-            subc<NT, true>(ua, va, wa, A);
-            subc<NT, true>(ub, vb, wb, B);
+            ldc<NT>(sd.a0, sd.a1, wa0, ua, va);
+            ldc<NT>(sd.b0, sd.b1, wb0, ub, vb);
+            subc<NT, true>(ua, va, wa0, A);
+            subc<NT, true>(ub, vb, wb0, B);
             for (int s = 0; s < nsteps; ++s) {
-                tA += 32; tB += 32;
-                wa = na; wb = nb;
-                ldc<NT>(sd.a0, sd.a1, wa, ua, va); // one step past the end reads a valid (unused) entry
-                ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
-                na = __ldg(tA + 32); nb = __ldg(tB + 32);
-                prefetch_l1(tA + 5 * 32); prefetch_l1(tB + 5 * 32);
+                tA += 16; tB += 16;
+                ldc<NT>(sd.a0, sd.a1, wa1, ua, va); // k-step s + 1 (one step past the end: a valid, unused entry)
+                ldc<NT>(sd.b0, sd.b1, wb1, ub, vb);
+                const uint32_t na = ldw(tA + 64), nb = ldw(tB + 64); // k-step s + 5
                 mma_square(acc, A, B);
-                subc<NT, true>(ua, va, wa, A);
-                subc<NT, true>(ub, vb, wb, B);
+                subc<NT, true>(ua, va, wa1, A);
+                subc<NT, true>(ub, vb, wb1, B);
+                wa1 = wa2; wa2 = wa3; wa3 = wa4; wa4 = na;
+                wb1 = wb2; wb2 = wb3; wb3 = wb4; wb4 = nb;
             }
         } else {
-            const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry)
-            const uint2* tA = tab + dr.offA + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
-            const uint2* tB = tab + dr.offB + ((dr.sbeg * 4 + kk) * 8 + r) * nw;
-            for (int s = 0; s < nsteps; ++s, tA += 32 * nw, tB += 32 * nw) {
+            const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry): 16-byte groups of four words
+            const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA + ((dr.sbeg * 4 + kk) * 4 + c) * nw);
+            const uint4* tB = reinterpret_cast<const uint4*>(tab + dr.offB + ((dr.sbeg * 4 + kk) * 4 + c) * nw);
+            for (int s = 0; s < nsteps; ++s, tA += 4 * nw, tB += 4 * nw) {
                 double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
-                uint2 wa = __ldg(tA), wb = __ldg(tB);
-                ldc<NT>(sd.a0, sd.a1, wa, ua, va);
-                ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
-                subc<NT, true>(ua, va, wa, A);
-                subc<NT, true>(ub, vb, wb, B);
-                for (int j = 1; j < nw; ++j) {
-                    wa = __ldg(tA + j); wb = __ldg(tB + j);
-                    ldc<NT>(sd.a0, sd.a1, wa, ua, va);
-                    ldc<NT>(sd.b0, sd.b1, wb, ub, vb);
-                    subc<NT, false>(ua, va, wa, A);
-                    subc<NT, false>(ub, vb, wb, B);
+#pragma unroll
+                for (int p = 0; p < NT; ++p) A[p] = B[p] = make_double2(0.0, 0.0);
+                for (int j = 0; j < nw / 4; ++j) {
+                    const uint4 qa = __ldg(tA + j), qb = __ldg(tB + j);
+                    const uint32_t xa[4] = {qa.x, qa.y, qa.z, qa.w}, xb[4] = {qb.x, qb.y, qb.z, qb.w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        ldc<NT>(sd.a0, sd.a1, xa[e], ua, va);
+                        ldc<NT>(sd.b0, sd.b1, xb[e], ub, vb);
+                        subc<NT, false>(ua, va, xa[e], A);
+                        subc<NT, false>(ub, vb, xb[e], B);
+                    }
                 }
                 mma_square(acc, A, B);
             }
@@ -146,63 +175,66 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
             }
 }
 
-__device__ __forceinline__ void wide_loads_A_c(const char* a0, const char* a1, uint4 a01, uint4 a23, double2 (&ua)[4][2],
-                                               double2 (&va)[4][2]) {
-    ldc<2>(a0, a1, make_uint2(a01.x, a01.y), ua[0], va[0]);
-    ldc<2>(a0, a1, make_uint2(a01.z, a01.w), ua[1], va[1]);
-    ldc<2>(a0, a1, make_uint2(a23.x, a23.y), ua[2], va[2]);
-    ldc<2>(a0, a1, make_uint2(a23.z, a23.w), ua[3], va[3]);
+__device__ __forceinline__ void wide_loads_A_c(const char* a0, const char* a1, uint4 w, double2 (&ua)[4][2], double2 (&va)[4][2]) {
+    ldc<2>(a0, a1, w.x, ua[0], va[0]);
+    ldc<2>(a0, a1, w.y, ua[1], va[1]);
+    ldc<2>(a0, a1, w.z, ua[2], va[2]);
+    ldc<2>(a0, a1, w.w, ua[3], va[3]);
 }
-__device__ __forceinline__ void wide_subs_A_c(const double2 (&ua)[4][2], const double2 (&va)[4][2], uint4 a01, uint4 a23,
-                                              double2 (&A)[4][2]) {
-    subc<2, true>(ua[0], va[0], make_uint2(a01.x, a01.y), A[0]);
-    subc<2, true>(ua[1], va[1], make_uint2(a01.z, a01.w), A[1]);
-    subc<2, true>(ua[2], va[2], make_uint2(a23.x, a23.y), A[2]);
-    subc<2, true>(ua[3], va[3], make_uint2(a23.z, a23.w), A[3]);
+__device__ __forceinline__ void wide_subs_A_c(const double2 (&ua)[4][2], const double2 (&va)[4][2], uint4 w, double2 (&A)[4][2]) {
+    subc<2, true>(ua[0], va[0], w.x, A[0]);
+    subc<2, true>(ua[1], va[1], w.y, A[1]);
+    subc<2, true>(ua[2], va[2], w.z, A[2]);
+    subc<2, true>(ua[3], va[3], w.w, A[3]);
 }
-__device__ __forceinline__ void wide_loads_B_c(const char* sB, uint4 bw, double2 (&ub)[2][1], double2 (&vb)[2][1]) {
-    ldc<1>(sB, sB, make_uint2(bw.x, bw.y), ub[0], vb[0]);
-    ldc<1>(sB, sB, make_uint2(bw.z, bw.w), ub[1], vb[1]);
+// B entry (8 gather terms = 4 pairs): the lanes hi = 0 and hi = 1 of one (aY, k) need the same entry, so each gathers
+// two of the four pairs and the halves are exchanged with a shuffle (lane ^ 16 flips hi)
+__device__ __forceinline__ void wide_loads_B_c(const char* sB, uint2 bw, double2 (&ub)[2][1], double2 (&vb)[2][1]) {
+    ldc<1>(sB, sB, bw.x, ub[0], vb[0]);
+    ldc<1>(sB, sB, bw.y, ub[1], vb[1]);
 }
-__device__ __forceinline__ void wide_fold_B_c(const double2 (&ub)[2][1], const double2 (&vb)[2][1], uint4 bw, double2 (&Bv)[1]) {
+__device__ __forceinline__ void wide_fold_B_c(const double2 (&ub)[2][1], const double2 (&vb)[2][1], uint2 bw, double2 (&Bv)[1]) {
     double2 part[1];
-    subc<1, true>(ub[0], vb[0], make_uint2(bw.x, bw.y), part);
-    subc<1, false>(ub[1], vb[1], make_uint2(bw.z, bw.w), part);
+    subc<1, true>(ub[0], vb[0], bw.x, part);
+    subc<1, false>(ub[1], vb[1], bw.y, part);
     const double ox = __shfl_xor_sync(0xffffffffu, part[0].x, 16), oy = __shfl_xor_sync(0xffffffffu, part[0].y, 16);
     Bv[0] = make_double2(part[0].x + ox, part[0].y + oy);
 }
 
-__device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec* diags, const uint2* __restrict__ tab,
+__device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec* diags, const uint32_t* __restrict__ tab,
                                                 const CSides sd, double2* __restrict__ out, int lane) {
-    const int r = lane >> 2, kk = lane & 3, aY = r & 3, hi = r >> 2;
+    const int r = lane >> 2, kk = lane & 3, hi = r >> 2;
     const char* a0 = (u.cls == 2) ? sd.a0 : sd.b0; // operand A = the block that carries a3 and a4
     const char* a1 = (u.cls == 2) ? sd.a1 : sd.b1;
-    const char* sB = (u.cls == 2) ? sd.b0 : sd.a0;
+    const char* sB = (u.cls == 2) ? sd.w2 : sd.w1; // operand B at the lane's plane aY = r & 3
     constexpr int NJ = 2;
     double acc[NJ * 4][2] = {};
     for (int d = u.diag_begin; d < u.diag_end; ++d) {
         const Diag3Rec dr = load_diag(diags + d); // nwA == 1, nwB == 4
+        if (d + 1 < u.diag_end) prefetch_diag_c(diags + d + 1, true, tab, lane);
         const int nsteps = dr.send - dr.sbeg;
-        const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA) + ((dr.sbeg * 4 + kk) * 8 + r) * 2;
-        const uint4* tB = reinterpret_cast<const uint4*>(tab + dr.offB) + ((dr.sbeg * 4 + kk) * 4 + aY) * 2;
+        // A table [k][cX & 3][g] (one uint4 per lane and k-step), B table [k][4 pairs] (one uint2 per lane: pairs 2 hi, 2 hi + 1)
+        const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA) + (dr.sbeg * 4 + kk) * 4 + (r >> 1);
+        const uint2* tB = reinterpret_cast<const uint2*>(tab + dr.offB) + (dr.sbeg * 4 + kk) * 2 + hi;
+        // software pipeline: table words three k-steps ahead in registers; the A gathers of step s + 1 fly under the
+        // MMAs of step s, the (8-term) B gather of step s + 1 is issued after them and folded at the top of step s + 1
         double2 A[4][NJ], Bv[1], ua[4][NJ], va[4][NJ], ub[2][1], vb[2][1];
-        uint4 a01 = __ldg(tA), a23 = __ldg(tA + 1), bw = __ldg(tB + hi);
-        wide_loads_A_c(a0, a1, a01, a23, ua, va);
-        wide_loads_B_c(sB, bw, ub, vb);
-        uint4 na01 = __ldg(tA + 64), na23 = __ldg(tA + 65), nbw = __ldg(tB + 32 + hi);
-        wide_subs_A_c(ua, va, a01, a23, A);
+        uint4 a_c = __ldg(tA), a_1 = __ldg(tA + 16), a_2 = __ldg(tA + 32), a_3 = __ldg(tA + 48);
+        uint2 b_c = __ldg(tB), b_1 = __ldg(tB + 8), b_2 = __ldg(tB + 16), b_3 = __ldg(tB + 24);
+        wide_loads_A_c(a0, a1, a_c, ua, va);
+        wide_loads_B_c(sB, b_c, ub, vb);
+        wide_subs_A_c(ua, va, a_c, A);
         for (int s = 0; s < nsteps; ++s) {
-            tA += 64; tB += 32;
-            wide_fold_B_c(ub, vb, bw, Bv);
-            a01 = na01; a23 = na23;
-            wide_loads_A_c(a0, a1, a01, a23, ua, va); // one step past the end reads valid (unused) entries
-            na01 = __ldg(tA + 64); na23 = __ldg(tA + 65);
-            prefetch_l1(tA + 3 * 64); prefetch_l1(tB + 3 * 32);
+            tA += 16; tB += 8;
+            wide_fold_B_c(ub, vb, b_c, Bv);
+            wide_loads_A_c(a0, a1, a_1, ua, va); // k-step s + 1 (one step past the end: valid, unused entries)
+            const uint4 na = __ldg(tA + 48);     // k-step s + 4
+            const uint2 nb = __ldg(tB + 24);
             mma_wide<NJ>(acc, A, Bv[0], hi);
-            wide_subs_A_c(ua, va, a01, a23, A);
-            bw = nbw;
-            wide_loads_B_c(sB, bw, ub, vb);
-            nbw = __ldg(tB + 32 + hi);
+            wide_subs_A_c(ua, va, a_1, A);
+            wide_loads_B_c(sB, b_1, ub, vb);
+            a_c = a_1; a_1 = a_2; a_2 = a_3; a_3 = na;
+            b_c = b_1; b_1 = b_2; b_2 = b_3; b_3 = nb;
         }
     }
     double* o = reinterpret_cast<double*>(out);
@@ -217,6 +249,12 @@ __device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec
                 const int a1s = u.cls == 2 ? aX : ay, a2s = u.cls == 2 ? ay : aX;
                 o[2 * ((a1s * 4 + a2s) * 16 + cX) + part] = acc[j * 4 + g][e];
             }
+}
+
+// L1 prefetch of the table heads of the first diagram of a unit (urec, drecs: shared memory)
+__device__ __forceinline__ void prefetch_unit_c(const Unit3Rec* urec, const Diag3Rec* drecs, const uint32_t* __restrict__ tab, int lane) {
+    const int4 uv = *reinterpret_cast<const int4*>(urec);
+    prefetch_diag_c(drecs + uv.x, uv.z >= 2, tab, lane);
 }
 
 __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a) {
@@ -292,6 +330,10 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
 
     // ---------------- compute warps
     const int lane = tid & 31;
+#ifdef NBS_PROF
+    long long pf[PF_N] = {};
+    const long long pf_start = clock64();
+#endif
     uint32_t par = 0;       // phase parities of the slot barriers (every warp sees every item)
     unsigned seq = 0;       // items started by this warp
     unsigned ntask = 0;
@@ -312,20 +354,31 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
             }
             const int ip = c0.x, nunits = c0.y, flags = c2.y;
             const int b = seq % PROD_NBUF, rb = seq % C_NREC, cs = seq & 7;
+            PF_T(t_e);
             if (seq >= PROD_NBUF) mbar_wait(&ctlp->empty[b], ((seq / PROD_NBUF) - 1u) & 1u); // ring buffer b is free again
+            PF_ADD(PF_EMPTY, t_e);
+            PF_T(t_r);
             mbar_wait(&ctlp->bar_rec[rb], (seq / C_NREC) & 1u);
+            PF_ADD(PF_REC, t_r);
+            PF_T(t_s);
             const int w1 = flags & 7, w2 = (flags >> 3) & 7;
             if (w1) { mbar_wait(&ctlp->bar_slot[w1 - 1], (par >> (w1 - 1)) & 1u); par ^= 1u << (w1 - 1); }
             if (w2) { mbar_wait(&ctlp->bar_slot[w2 - 1], (par >> (w2 - 1)) & 1u); par ^= 1u << (w2 - 1); }
+            PF_ADD(PF_SLOT, t_s);
             if (lane == 0) { // every warp writes the same descriptor (the epilogue reads it after the last arrival)
                 ctl->meta_q[b] = (int)((flags & 64) ? mq : q);
                 ctl->meta_pair[b] = ip;
             }
             const Unit3Rec* s_units = reinterpret_cast<const Unit3Rec*>(s_rec + rb * a.rec_stride);
             const Diag3Rec* s_diags = reinterpret_cast<const Diag3Rec*>(s_rec + rb * a.rec_stride + a.units_bytes);
-            CSides sd;
-            sd.a0 = smem + (uint32_t)c1.y; sd.a1 = sd.a0 + (uint32_t)c1.w;
-            sd.b0 = smem + (uint32_t)c1.z; sd.b1 = sd.b0 + (uint32_t)c2.x;
+            CSides sd; // c1.w / c2.x: byte stride of two planes of B~1 / B~2
+            {
+                const uint32_t ps1 = (uint32_t)c1.w, ps2 = (uint32_t)c2.x, r = (uint32_t)lane >> 2;
+                sd.a0 = smem + (uint32_t)c1.y + (r & 1u) * (ps1 >> 1); sd.a1 = sd.a0 + ps1;
+                sd.b0 = smem + (uint32_t)c1.z + (r & 1u) * (ps2 >> 1); sd.b1 = sd.b0 + ps2;
+                sd.w1 = smem + (uint32_t)c1.y + (r & 3u) * (ps1 >> 1);
+                sd.w2 = smem + (uint32_t)c1.z + (r & 3u) * (ps2 >> 1);
+            }
             double2* scr = scr0 + b * scr_stride;
             int* next_unit = const_cast<int*>(&ctl->next_unit[cs]);
             auto grab = [&]() {
@@ -338,10 +391,12 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
                 const int4 uv = *reinterpret_cast<const int4*>(s_units + i);
                 Unit3Rec u;
                 u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
-                if (i + PROD_CWARPS < nunits) prefetch_unit(s_units + i + PROD_CWARPS, s_diags, a.tab, lane);
+                if (i + PROD_CWARPS < nunits) prefetch_unit_c(s_units + i + PROD_CWARPS, s_diags, a.tab, lane);
                 double2* out = scr + (size_t)u.slot * 256;
+                PF_T(t_u);
                 if (u.cls < 2) run_unit_square_c(u, s_diags, a.tab, sd, out, lane);
                 else run_unit_wide_c(u, s_diags, a.tab, sd, out, lane);
+                PF_ADD(PF_UNITS, t_u);
                 i = grab();
             }
             __syncwarp();
@@ -352,6 +407,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
                 old = atomicAdd(const_cast<int*>(&ctl->done_cnt[cs]), 1);
             }
             old = __shfl_sync(0xffffffffu, old, 0);
+            PF_T(t_l);
             if (old == PROD_CWARPS - 1) {
                 // this warp completed the item: its blocks and records are free.  Lanes issue the release list in
                 // parallel; lane 31 loads the records of the item C_NREC positions ahead into the buffer just vacated.
@@ -377,10 +433,16 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
                 __threadfence_block();
             }
             __syncwarp();
+            PF_ADD(PF_RELEASE, t_l);
         }
         ++ntask;
         qt = qn;
     }
+#ifdef NBS_PROF
+    pf[PF_TOTAL] = clock64() - pf_start;
+    if (lane == 0)
+        for (int i = 0; i < PF_N; ++i) atomicAdd(&g_cprof[i], (unsigned long long)pf[i]);
+#endif
     // no work left: tell the epilogue warps (every warp arrives; lane 0 of each writes the same end marker)
     {
         const int b = seq % PROD_NBUF;

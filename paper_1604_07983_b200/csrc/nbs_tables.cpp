@@ -479,39 +479,40 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         dedupe3[w] = off;
         return off;
     };
-    // The same tables for the pipelined kernel, in the layout of the block of kind `kind` on that side (raw index
-    // triples from make_side).  An antisymmetric block is gathered from its compact form: a term whose stored
-    // partner carries the opposite sign changes sides (u <-> v); when an entry then has more terms of one sign than
-    // it has places for, the surplus goes to the other side with bit 31 set (the kernel flips the sign of the value
-    // it loads); the vanishing diagonal is read from a zero pad.
+    // Tables of the pipelined kernel (nbs_tables.hpp, "packed gather tables"): one 32-bit word per term pair,
+    // offsets inside ONE sink-spin plane of a block of kind `kind` (raw index triples from make_side).  An
+    // antisymmetric block is gathered from its compact form: a term whose stored partner carries the opposite sign
+    // changes sides (u <-> v); when an entry then has more terms of one sign than it has places for, the surplus
+    // goes to the other side with its flip bit set; the vanishing diagonal is read from a zero pad.
     std::map<std::vector<uint32_t>, uint32_t> dedupec;
     auto intern3c = [&](const SideTable& t, int layout, int kind) -> uint32_t {
         const int Kp = (t.K + 3) / 4 * 4, nw = t.n / 2;
-        const int rows = (layout == 2) ? 4 : 8, G = (layout == 1) ? 4 : 1;
-        const uint32_t pl = (uint32_t)plane_elems(kind);
-        std::vector<uint32_t> w((size_t)(Kp + 4) * rows * G * nw * 2, 0u);
+        const int G = (layout == 1) ? 4 : 1, CC = (layout == 2) ? 1 : 4;
+        // C_TAB_LOOKAHEAD all-zero k-steps close every table: the kernel's software pipeline reads that far past
+        // the end of a unit's range, and a zero word gathers u = v = entry 0 of the plane (difference 0)
+        std::vector<uint32_t> w((size_t)(Kp + 4 * C_TAB_LOOKAHEAD) * CC * G * nw, 0u);
         for (int k = 0; k < t.K; ++k)
-            for (int r = 0; r < rows; ++r)
+            for (int cc = 0; cc < CC; ++cc)
                 for (int g = 0; g < G; ++g) {
-                    const int c = (layout == 0) ? (r >> 1) : (layout == 1) ? 4 * g + (r >> 1) : 0;
-                    const int plane = (layout == 2) ? r : (r & 1);
+                    const int c = (layout == 0) ? cc : (layout == 1) ? 4 * g + cc : 0; // carried source spin(s)
                     std::vector<uint32_t> plus, minus, zeros;
                     for (int j = 0; j < t.n; ++j) {
                         const uint16_t e = t.g[((size_t)c * t.K + k) * t.n + j];
                         const int tri = e & 0x7fff, sg = (e & 0x8000) ? -1 : 1;
                         const Located loc = locate(kind, tri / 144, (tri / 12) % 12, tri % 12);
-                        const uint32_t off = ((uint32_t)plane * pl + (uint32_t)loc.idx) * 16u;
+                        const uint32_t off = (uint32_t)loc.idx * 16u; // < 2^15
                         if (loc.sign == 0) zeros.push_back(off);
                         else ((sg * loc.sign < 0) ? minus : plus).push_back(off);
                     }
-                    std::vector<uint32_t> U, V;
-                    for (uint32_t o : plus) { if ((int)U.size() < nw) U.push_back(o); else V.push_back(o | 0x80000000u); }
-                    for (uint32_t o : minus) { if ((int)V.size() < nw) V.push_back(o); else U.push_back(o | 0x80000000u); }
+                    std::vector<uint32_t> U, V; // 16-bit halves: byte offset | flip << 15
+                    for (uint32_t o : plus) { if ((int)U.size() < nw) U.push_back(o); else V.push_back(o | 0x8000u); }
+                    for (uint32_t o : minus) { if ((int)V.size() < nw) V.push_back(o); else U.push_back(o | 0x8000u); }
                     for (uint32_t o : zeros) { if ((int)U.size() < nw) U.push_back(o); else V.push_back(o); }
                     if ((int)U.size() != nw || (int)V.size() != nw) { tab_err = "internal: compact gather does not fit"; return 0; }
                     for (int j = 0; j < nw; ++j) {
-                        const size_t o = ((((size_t)k * rows + r) * G + g) * nw + j) * 2;
-                        w[o] = U[j]; w[o + 1] = V[j];
+                        // layout 0: [k][c][nw]; layout 1: [k][cX & 3][g]; layout 2: [k][nw]
+                        const size_t o = (layout == 1) ? ((size_t)k * 4 + cc) * 4 + g : ((size_t)k * CC + cc) * nw + j;
+                        w[o] = U[j] | (V[j] << 16);
                     }
                 }
         w.push_back((uint32_t)layout);
@@ -519,8 +520,8 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         if (it != dedupec.end()) return it->second;
         w.pop_back();
         const uint32_t off = (uint32_t)plan.tabc.size();
-        for (size_t i = 0; i < w.size(); i += 2) plan.tabc.push_back(uint2x{w[i], w[i + 1]});
-        while (plan.tabc.size() % 2) plan.tabc.push_back(uint2x{0, 0});
+        plan.tabc.insert(plan.tabc.end(), w.begin(), w.end());
+        while (plan.tabc.size() % 4) plan.tabc.push_back(0u); // 16-byte aligned tables
         w.push_back((uint32_t)layout);
         dedupec[w] = off;
         return off;
@@ -629,7 +630,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         plan.pairs3.push_back(pr);
     }
     plan.tab3.insert(plan.tab3.end(), 1024, uint2x{0, 0}); // the kernel prefetches a few k-steps past a table's end
-    plan.tabc.insert(plan.tabc.end(), 4096, uint2x{0, 0}); // the same; covers the self-check's layout-blind bound
+    plan.tabc.insert(plan.tabc.end(), 256, 0u); // L1 prefetches run a little past a table's end
 
     // ---- chains: order of the sink pairs inside one momentum task that reloads the fewest blocks.
     // Full chain (all pairs) for the momenta q <= -q (index order), half chain (without the pairs of

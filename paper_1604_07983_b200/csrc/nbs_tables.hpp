@@ -153,6 +153,12 @@ struct ChainRec { // order in which one CTA walks the sink pairs of one momentum
 // a release list -- the bulk copies that may be issued as soon as the item is complete, because they overwrite
 // blocks that nobody needs any more.  The program is cyclic: release lists near its end carry the first loads of
 // the next task.
+// Packed gather tables (Plan::tabc): one 32-bit word per (+, -) pair of gather terms, byte offsets inside ONE sink-spin
+// plane of the block (the plane of the reading lane is part of its base pointer, so a table serves all planes):
+//   bits 4-14 offset of the + term, bit 15 its flip flag, bits 20-30 offset of the - term, bit 31 its flip flag
+//   (a set flip flag: the loaded value enters with the opposite sign -- compact blocks only, see build_plan).
+//   16x16 sides  [k][c (carried spin)][nw]          64x4 A side  [k][cX & 3][g = cX >> 2]          64x4 B side  [k][nw = 4]
+constexpr int C_TAB_LOOKAHEAD = 5; // k-steps the kernel's register pipeline may read past the end of a range (tables are padded by as many)
 constexpr uint32_t C_SLOT_BYTES = 2u * SM_PLANE * 16u; // 55 680 >= AS_BLOCK * 16 = 55 552
 constexpr int C_NSLOT = 4;
 constexpr int C_NREC = 3; // unit / diagram record buffers: a warp may run two items ahead of the slowest one
@@ -221,10 +227,10 @@ struct Plan {
     int max_pair_units = 0;
     int max_pair_diags = 0;
     double sumKp_exec = 0; // executed k-steps x 4 (padding included)
-    // pipelined kernel: gather tables in the layout of the block kind of each side (compact for antisymmetric
-    // blocks; bit 31 of a word = the term enters with the opposite sign), one diagram record per entry of diags3
-    std::vector<uint2x> tabc;
-    std::vector<Diag3Rec> diagsc;
+    // pipelined kernel: packed gather tables in the layout of the block kind of each side (compact for
+    // antisymmetric blocks), one diagram record per entry of diags3
+    std::vector<uint32_t> tabc;
+    std::vector<Diag3Rec> diagsc; // offA / offB in 32-bit words of tabc
     std::vector<CItem> cprog;   // one task: full chain at q, half chain at -q
     std::vector<CLoad> cloads;
     bool cprog_ok = false;      // false: the plan is too small / too large for the pipelined kernel
