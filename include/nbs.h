@@ -234,6 +234,9 @@ int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);
  *   mode 0: 16 DMMA.8x8x4      mode 1: 16 DFMA      mode 2: 16 DADD
  *   mode 3: 12 DMMA + 12 DADD  (one k-step of the 16x16 accumulator class of the product kernel)
  *   mode 4: 16 DMMA + 24 DADD  (one k-step of the 64x4 class)
+ *   mode 5: 12 DADD then 12 DMMA, instruction order pinned      mode 6: DADD and DMMA strictly alternating, order pinned
+ *   mode 7 / 8: mode 6 with 8 / 4 independent integer instructions between the FP64 instructions of a pair
+ *   (modes 5-8 answer scheduling questions: does interleaving, or integer work in between, cost FP64 throughput)
  * per warp on 16 warps per SM, all SMs.  *tflops = executed FP64 flops per second / 1e12 (a DMMA counts
  * 8*8*4*2 = 512, a DFMA 64, a DADD 32 per warp instruction); *ms = duration of the timed launch.  Either may be NULL.
  */

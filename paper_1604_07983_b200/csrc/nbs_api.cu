@@ -661,7 +661,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         c->prod_grid = prop.multiProcessorCount;
         // pipelined kernel: needs a program (Plan::cprog_ok) and room for three record buffers
         c->c_units_bytes = (uint32_t)c->plan.max_pair_units * (uint32_t)sizeof(Unit3Rec);
-        c->c_rec_stride = c->c_units_bytes + (uint32_t)c->plan.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
+        c->c_rec_stride = C_ITEM_BYTES + c->c_units_bytes + (uint32_t)c->plan.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
         c->c_smem = cprod_smem_bytes(c->c_rec_stride);
         c->use_c = c->plan.cprog_ok && c->c_smem <= (size_t)prop.sharedMemPerBlockOptin && c->plan.baryons.size() < 256;
 #ifdef NBS_NO_PIPELINE
@@ -929,7 +929,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
             ca.units = c->d_units3; ca.diags = c->d_diagsc; ca.tab = c->d_tabc;
             ca.rec_stride = c->c_rec_stride; ca.units_bytes = c->c_units_bytes;
             grid = (unsigned)std::min<long long>(c->prod_grid, ca.ntasks);
-            k_product_c<<<grid, PROD_THREADS, c->c_smem, st>>>(ca);
+            k_product_c<<<grid, C_THREADS, c->c_smem, st>>>(ca);
         } else
         k_product_t<false><<<grid, PROD_THREADS, PROD_SMEM, st>>>(pa);
         CU(c, cudaGetLastError());
@@ -992,11 +992,11 @@ int nbs_stage_times(nbs_ctx* c, double* ms, long long* calls, int reset) {
         unsigned long long pf[PF_N] = {}, zero[PF_N] = {};
         cudaMemcpyFromSymbol(pf, g_cprof, sizeof(pf));
         cudaMemcpyToSymbol(g_cprof, zero, sizeof(zero));
-        static const char* names[PF_N] = {"total", "units", "wait_empty", "wait_rec", "wait_slot", "release", "flush"};
+        static const char* names[PF_N] = {"total", "units", "wait_empty", "wait_rec", "wait_slot", "release", "flush", "epi_total", "epi_busy"};
         if (pf[PF_TOTAL]) {
             fprintf(stderr, "[NBS_PROF] compute-warp cycles:");
-            for (int i = 0; i < PF_N; ++i) fprintf(stderr, " %s %.2f%%", names[i], 100.0 * (double)pf[i] / (double)pf[PF_TOTAL]);
-            fprintf(stderr, "\n");
+            for (int i = 0; i < PF_EPI_TOTAL; ++i) fprintf(stderr, " %s %.2f%%", names[i], 100.0 * (double)pf[i] / (double)pf[PF_TOTAL]);
+            fprintf(stderr, "; epilogue warps busy %.1f%%\n", 100.0 * (double)pf[PF_EPI_BUSY] / (double)pf[PF_EPI_TOTAL]);
         }
     }
 #endif
@@ -1093,7 +1093,7 @@ int nbs_tiled_info(const nbs_ctx* c, int* chunk_slots, long long* chunk_builds) 
 int nbs_probe_fp64(nbs_ctx* c, int mode, int iters, double* tflops, double* ms_out) {
     if (!c) return NBS_EINVAL;
     if (c->cuda_failed) return NBS_ECUDA;
-    if (mode < 0 || mode > 4 || iters < 1) return fail(c, NBS_EINVAL, "nbs_probe_fp64: mode in [0, 4], iters >= 1");
+    if (mode < 0 || mode > 8 || iters < 1) return fail(c, NBS_EINVAL, "nbs_probe_fp64: mode in [0, 8], iters >= 1");
     CU(c, cudaSetDevice(c->device));
     cudaEvent_t a = nullptr, b = nullptr;
     CU(c, cudaEventCreate(&a));
@@ -1106,7 +1106,11 @@ int nbs_probe_fp64(nbs_ctx* c, int mode, int iters, double* tflops, double* ms_o
         case 1: k_probe_fp64<1><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
         case 2: k_probe_fp64<2><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
         case 3: k_probe_fp64<3><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
-        default: k_probe_fp64<4><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        case 4: k_probe_fp64<4><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        case 5: k_probe_fp64<5><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        case 6: k_probe_fp64<6><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        case 7: k_probe_fp64<7><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
+        default: k_probe_fp64<8><<<grid, PROBE_THREADS>>>(n, 1e-9, sink); break;
         }
     };
     launch(iters / 8 + 1); // warm-up

@@ -13,9 +13,18 @@
 namespace nbs {
 
 constexpr int PROBE_THREADS = 512; // 16 warps per CTA, one CTA per SM: 4 warps per SM sub-partition
-__host__ __device__ constexpr int probe_dmma(int mode) { return mode == 0 ? 16 : mode == 3 ? 12 : mode == 4 ? 16 : 0; }
+//   mode 5: 12 DADD, then 12 DMMA, order pinned (volatile asm)    mode 6: DADD and DMMA strictly alternating, order pinned
+//   mode 7 / 8: mode 6 with 8 / 4 independent integer instructions per DADD + DMMA pair
+__host__ __device__ constexpr int probe_dmma(int mode) { return mode == 0 ? 16 : mode == 3 ? 12 : mode == 4 ? 16 : mode >= 5 ? 12 : 0; }
 __host__ __device__ constexpr int probe_dfma(int mode) { return mode == 1 ? 16 : 0; }
-__host__ __device__ constexpr int probe_dadd(int mode) { return mode == 2 ? 16 : mode == 3 ? 12 : mode == 4 ? 24 : 0; }
+__host__ __device__ constexpr int probe_dadd(int mode) { return mode == 2 ? 16 : mode == 3 ? 12 : mode == 4 ? 24 : mode >= 5 ? 12 : 0; }
+__device__ __forceinline__ void dmma884_v(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void dadd_v(double& d, double a, double b) {
+    asm volatile("add.f64 %0, %1, %2;" : "=d"(d) : "d"(a), "d"(b));
+}
 
 template <int MODE>
 __global__ void __launch_bounds__(PROBE_THREADS, 1) k_probe_fp64(int iters, double delta, double* __restrict__ sink) {
@@ -29,6 +38,9 @@ __global__ void __launch_bounds__(PROBE_THREADS, 1) k_probe_fp64(int iters, doub
     double w[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) w[i] = 0.5 + 1e-3 * (lane - i);
+    unsigned iw[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) iw[i] = lane + i;
     for (int it = 0; it < iters; ++it) {
         if (MODE == 0) {
 #pragma unroll
@@ -54,6 +66,28 @@ __global__ void __launch_bounds__(PROBE_THREADS, 1) k_probe_fp64(int iters, doub
                     dmma884(acc[(i * 2 + j) * 3 + 1][0], acc[(i * 2 + j) * 3 + 1][1], Ai[i], Bi[j]);
                     dmma884(acc[(i * 2 + j) * 3 + 2][0], acc[(i * 2 + j) * 3 + 2][1], sA[i], sB[j]);
                 }
+        } else if (MODE == 5) {
+#pragma unroll
+            for (int i = 0; i < 12; ++i) dadd_v(v[i], v[i], delta);
+#pragma unroll
+            for (int i = 0; i < 12; ++i) dmma884_v(acc[i][0], acc[i][1], v[i], v[(i + 1) % 12]);
+        } else if (MODE == 7 || MODE == 8) {
+            // mode 5 plus integer work between the FP64 instructions (order pinned): 4 (mode 7) or 2 (mode 8) per FP64 op
+#pragma unroll
+            for (int i = 0; i < 12; ++i) {
+                dadd_v(v[i], v[i], delta);
+#pragma unroll
+                for (int k = 0; k < (MODE == 7 ? 4 : 2); ++k) asm volatile("xor.b32 %0, %0, %1;" : "+r"(iw[(i + k) & 7]) : "r"(it));
+                dmma884_v(acc[i][0], acc[i][1], v[(i + 4) % 12], v[(i + 5) % 12]);
+#pragma unroll
+                for (int k = 0; k < (MODE == 7 ? 4 : 2); ++k) asm volatile("xor.b32 %0, %0, %1;" : "+r"(iw[(i + k + 4) & 7]) : "r"(it));
+            }
+        } else if (MODE == 6) {
+#pragma unroll
+            for (int i = 0; i < 12; ++i) {
+                dadd_v(v[i], v[i], delta);
+                dmma884_v(acc[i][0], acc[i][1], v[(i + 4) % 12], v[(i + 5) % 12]);
+            }
         } else {
             // A[4][2] complex (16 subtractions), B entry (8 adds), 16 MMAs (mma_wide)
 #pragma unroll
@@ -72,6 +106,8 @@ __global__ void __launch_bounds__(PROBE_THREADS, 1) k_probe_fp64(int iters, doub
     for (int i = 0; i < 16; ++i) s += acc[i][0] + acc[i][1];
 #pragma unroll
     for (int i = 0; i < 16; ++i) s += v[i];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += (double)iw[i];
     if (s == 1.2345e-300) sink[blockIdx.x * PROBE_THREADS + threadIdx.x] = s; // keeps the arithmetic alive
 }
 

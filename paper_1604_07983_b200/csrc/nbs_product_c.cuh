@@ -19,6 +19,13 @@
 
 namespace nbs {
 
+// Warp split: 10 compute + 2 epilogue warps, as in k_product_t.  Measured alternatives (profiles/r2_summary.md):
+// 8 compute warps run within 2 % of 10 (the arithmetic nearly saturates at two warps per SM sub-partition); four
+// epilogue warps with a pipelined row reader remove the epilogue's own floor (49 ms per launch, latency-bound) but
+// take issue slots and shared-memory bandwidth from the compute warps of every sub-partition (67 against 63.6 ms).
+constexpr int C_CWARPS = PROD_CWARPS, C_EWARPS = PROD_EWARPS;
+constexpr int C_CTHREADS = C_CWARPS * 32, C_ETHREADS = C_EWARPS * 32, C_THREADS = C_CTHREADS + C_ETHREADS;
+
 struct CProdArgs {
     ProdArgs base;        // pairs, pair_chans, Ft, ch_begin, nch_out, L, scratch, max_pair_units, counter (epilogue and bookkeeping)
     const double2* B;     // [V][R] momentum-space blocks, compact rows
@@ -33,7 +40,7 @@ struct CProdArgs {
     const Unit3Rec* units;
     const Diag3Rec* diags; // compact-table diagram records (Plan::diagsc)
     const uint32_t* tab;   // Plan::tabc, packed words
-    uint32_t rec_stride, units_bytes; // record buffer: units at 0, diagram records at units_bytes
+    uint32_t rec_stride, units_bytes; // record buffer: the item (CItem), unit records at C_ITEM_BYTES, diagram records units_bytes further
 };
 
 struct CCtrl {
@@ -46,6 +53,8 @@ struct CCtrl {
     int meta_q[PROD_NBUF], meta_pair[PROD_NBUF];
 };
 constexpr uint32_t SMC_REC = C_NSLOT * C_SLOT_BYTES; // 222 720
+constexpr uint32_t C_ITEM_BYTES = 48;
+static_assert(sizeof(CItem) == C_ITEM_BYTES, "CItem is read as three int4");
 inline size_t cprod_smem_bytes(uint32_t rec_stride) {
     return (size_t)SMC_REC + (size_t)C_NREC * rec_stride + EPI_PAIR_BYTES + EPI_CG * sizeof(PairChanRec) + 16 + sizeof(CCtrl);
 }
@@ -83,7 +92,7 @@ __device__ __forceinline__ uint32_t ldw(const uint32_t* p) { return __ldg(p); }
 
 // -DNBS_PROF: cycle counters of the compute warps, summed over the launch (read by nbs_stage_times, printed to stderr)
 #ifdef NBS_PROF
-enum { PF_TOTAL, PF_UNITS, PF_EMPTY, PF_REC, PF_SLOT, PF_RELEASE, PF_FLUSH, PF_N };
+enum { PF_TOTAL, PF_UNITS, PF_EMPTY, PF_REC, PF_SLOT, PF_RELEASE, PF_FLUSH, PF_EPI_TOTAL, PF_EPI_BUSY, PF_N };
 __device__ unsigned long long g_cprof[PF_N];
 #define PF_T(var) const long long var = clock64()
 #define PF_ADD(idx, t0) pf[idx] += clock64() - (t0)
@@ -95,6 +104,17 @@ __device__ unsigned long long g_cprof[PF_N];
 // Per-lane views of the two staged blocks of an item: a0 / a1 = B~1 at the lane's plane (r & 1) and two planes
 // further, b0 / b1 the same for B~2; w1 / w2 = plane (r & 3) of B~1 / B~2 (operand B of the 64 x 4 classes).
 struct CSides { const char *a0, *a1, *b0, *b1, *w1, *w2; };
+// item: the staged CItem (shared memory); words 5-8 = off1, off2, ps1, ps2
+__device__ __forceinline__ CSides make_sides(const char* smem, const int* item, int lane) {
+    const uint32_t off1 = (uint32_t)item[5], off2 = (uint32_t)item[6], ps1 = (uint32_t)item[7], ps2 = (uint32_t)item[8];
+    const uint32_t r = (uint32_t)lane >> 2;
+    CSides sd;
+    sd.a0 = smem + off1 + (r & 1u) * (ps1 >> 1); sd.a1 = sd.a0 + ps1;
+    sd.b0 = smem + off2 + (r & 1u) * (ps2 >> 1); sd.b1 = sd.b0 + ps2;
+    sd.w1 = smem + off1 + (r & 3u) * (ps1 >> 1);
+    sd.w2 = smem + off2 + (r & 3u) * (ps2 >> 1);
+    return sd;
+}
 
 // L1 prefetch of the head of the two gather tables of a diagram record (dp: shared memory)
 __device__ __forceinline__ void prefetch_diag_c(const Diag3Rec* dp, bool wide, const uint32_t* __restrict__ tab, int lane) {
@@ -106,8 +126,35 @@ __device__ __forceinline__ void prefetch_diag_c(const Diag3Rec* dp, bool wide, c
     }
 }
 
+__device__ __forceinline__ void wide_loads_A_c(const char* a0, const char* a1, uint4 w, double2 (&ua)[4][2], double2 (&va)[4][2]) {
+    ldc<2>(a0, a1, w.x, ua[0], va[0]);
+    ldc<2>(a0, a1, w.y, ua[1], va[1]);
+    ldc<2>(a0, a1, w.z, ua[2], va[2]);
+    ldc<2>(a0, a1, w.w, ua[3], va[3]);
+}
+__device__ __forceinline__ void wide_subs_A_c(const double2 (&ua)[4][2], const double2 (&va)[4][2], uint4 w, double2 (&A)[4][2]) {
+    subc<2, true>(ua[0], va[0], w.x, A[0]);
+    subc<2, true>(ua[1], va[1], w.y, A[1]);
+    subc<2, true>(ua[2], va[2], w.z, A[2]);
+    subc<2, true>(ua[3], va[3], w.w, A[3]);
+}
+// B entry (8 gather terms = 4 pairs): the lanes hi = 0 and hi = 1 of one (aY, k) need the same entry, so each gathers
+// two of the four pairs and the halves are exchanged with a shuffle (lane ^ 16 flips hi)
+__device__ __forceinline__ void wide_loads_B_c(const char* sB, uint2 bw, double2 (&ub)[2][1], double2 (&vb)[2][1]) {
+    ldc<1>(sB, sB, bw.x, ub[0], vb[0]);
+    ldc<1>(sB, sB, bw.y, ub[1], vb[1]);
+}
+__device__ __forceinline__ void wide_fold_B_c(const double2 (&ub)[2][1], const double2 (&vb)[2][1], uint2 bw, double2 (&Bv)[1]) {
+    double2 part[1];
+    subc<1, true>(ub[0], vb[0], bw.x, part);
+    subc<1, false>(ub[1], vb[1], bw.y, part);
+    const double ox = __shfl_xor_sync(0xffffffffu, part[0].x, 16), oy = __shfl_xor_sync(0xffffffffu, part[0].y, 16);
+    Bv[0] = make_double2(part[0].x + ox, part[0].y + oy);
+}
+
 __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3Rec* diags, const uint32_t* __restrict__ tab,
-                                                  const CSides sd, double2* __restrict__ out, int lane) {
+                                                  const char* smem, const int* item, double2* __restrict__ out, int lane) {
+    const CSides sd = make_sides(smem, item, lane);
     const int r = lane >> 2, kk = lane & 3, c = r >> 1;
     constexpr int NT = 2;
     AccSquare<NT> acc = {};
@@ -116,28 +163,49 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
         if (d + 1 < u.diag_end) prefetch_diag_c(diags + d + 1, false, tab, lane);
         const int nsteps = dr.send - dr.sbeg;
         if (dr.nwA == 1) {
-            // software pipeline: table words four k-steps ahead in registers, shared-memory gathers one ahead
+            // software pipeline: table words four k-steps ahead in registers, shared-memory gathers one ahead, the
+            // operands of k-step s + 1 formed (into the other operand buffer) while the MMAs of k-step s run
             const uint32_t* tA = tab + dr.offA + dr.sbeg * 16 + kk * 4 + c;
             const uint32_t* tB = tab + dr.offB + dr.sbeg * 16 + kk * 4 + c;
             const uint32_t wa0 = ldw(tA), wb0 = ldw(tB);
             uint32_t wa1 = ldw(tA + 16), wb1 = ldw(tB + 16), wa2 = ldw(tA + 32), wb2 = ldw(tB + 32);
             uint32_t wa3 = ldw(tA + 48), wb3 = ldw(tB + 48), wa4 = ldw(tA + 64), wb4 = ldw(tB + 64);
-            double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
+            double2 A0[NT], B0[NT], A1[NT], B1[NT], ua[NT], va[NT], ub[NT], vb[NT];
             ldc<NT>(sd.a0, sd.a1, wa0, ua, va);
             ldc<NT>(sd.b0, sd.b1, wb0, ub, vb);
-            subc<NT, true>(ua, va, wa0, A);
-            subc<NT, true>(ub, vb, wb0, B);
-            for (int s = 0; s < nsteps; ++s) {
+            subc<NT, true>(ua, va, wa0, A0);
+            subc<NT, true>(ub, vb, wb0, B0);
+            // one k-step: MMAs on (A, B), operands of the next k-step into (An, Bn)
+            auto kstep = [&](const double2 (&A)[NT], const double2 (&B)[NT], double2 (&An)[NT], double2 (&Bn)[NT]) {
                 tA += 16; tB += 16;
                 ldc<NT>(sd.a0, sd.a1, wa1, ua, va); // k-step s + 1 (one step past the end: a valid, unused entry)
                 ldc<NT>(sd.b0, sd.b1, wb1, ub, vb);
                 const uint32_t na = ldw(tA + 64), nb = ldw(tB + 64); // k-step s + 5
-                mma_square(acc, A, B);
-                subc<NT, true>(ua, va, wa1, A);
-                subc<NT, true>(ub, vb, wb1, B);
+                double sA[NT], sB[NT];
+#pragma unroll
+                for (int i = 0; i < NT; ++i) { sA[i] = A[i].x + A[i].y; sB[i] = B[i].x + B[i].y; }
+#pragma unroll
+                for (int i = 0; i < NT; ++i)
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) {
+                        dmma884(acc.p1[i][j][0], acc.p1[i][j][1], A[i].x, B[j].x);
+                        dmma884(acc.p2[i][j][0], acc.p2[i][j][1], A[i].y, B[j].y);
+                    }
+                subc<NT, true>(ua, va, wa1, An);
+                subc<NT, true>(ub, vb, wb1, Bn);
+#pragma unroll
+                for (int i = 0; i < NT; ++i)
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) dmma884(acc.p3[i][j][0], acc.p3[i][j][1], sA[i], sB[j]);
                 wa1 = wa2; wa2 = wa3; wa3 = wa4; wa4 = na;
                 wb1 = wb2; wb2 = wb3; wb3 = wb4; wb4 = nb;
+            };
+            int s = 0;
+            for (; s + 1 < nsteps; s += 2) {
+                kstep(A0, B0, A1, B1);
+                kstep(A1, B1, A0, B0);
             }
+            if (s < nsteps) kstep(A0, B0, A1, B1);
         } else {
             const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry): 16-byte groups of four words
             const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA + ((dr.sbeg * 4 + kk) * 4 + c) * nw);
@@ -175,34 +243,11 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
             }
 }
 
-__device__ __forceinline__ void wide_loads_A_c(const char* a0, const char* a1, uint4 w, double2 (&ua)[4][2], double2 (&va)[4][2]) {
-    ldc<2>(a0, a1, w.x, ua[0], va[0]);
-    ldc<2>(a0, a1, w.y, ua[1], va[1]);
-    ldc<2>(a0, a1, w.z, ua[2], va[2]);
-    ldc<2>(a0, a1, w.w, ua[3], va[3]);
-}
-__device__ __forceinline__ void wide_subs_A_c(const double2 (&ua)[4][2], const double2 (&va)[4][2], uint4 w, double2 (&A)[4][2]) {
-    subc<2, true>(ua[0], va[0], w.x, A[0]);
-    subc<2, true>(ua[1], va[1], w.y, A[1]);
-    subc<2, true>(ua[2], va[2], w.z, A[2]);
-    subc<2, true>(ua[3], va[3], w.w, A[3]);
-}
-// B entry (8 gather terms = 4 pairs): the lanes hi = 0 and hi = 1 of one (aY, k) need the same entry, so each gathers
-// two of the four pairs and the halves are exchanged with a shuffle (lane ^ 16 flips hi)
-__device__ __forceinline__ void wide_loads_B_c(const char* sB, uint2 bw, double2 (&ub)[2][1], double2 (&vb)[2][1]) {
-    ldc<1>(sB, sB, bw.x, ub[0], vb[0]);
-    ldc<1>(sB, sB, bw.y, ub[1], vb[1]);
-}
-__device__ __forceinline__ void wide_fold_B_c(const double2 (&ub)[2][1], const double2 (&vb)[2][1], uint2 bw, double2 (&Bv)[1]) {
-    double2 part[1];
-    subc<1, true>(ub[0], vb[0], bw.x, part);
-    subc<1, false>(ub[1], vb[1], bw.y, part);
-    const double ox = __shfl_xor_sync(0xffffffffu, part[0].x, 16), oy = __shfl_xor_sync(0xffffffffu, part[0].y, 16);
-    Bv[0] = make_double2(part[0].x + ox, part[0].y + oy);
-}
-
+// 64 x 4 classes, B operand folded one k-step ahead: the fold of step s + 1 (DADDs and a shuffle) is issued at the top of
+// step s, from gathers issued during step s - 1, so that the 16 MMAs of a step never wait for it.
 __device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec* diags, const uint32_t* __restrict__ tab,
-                                                const CSides sd, double2* __restrict__ out, int lane) {
+                                                 const char* smem, const int* item, double2* __restrict__ out, int lane) {
+    const CSides sd = make_sides(smem, item, lane);
     const int r = lane >> 2, kk = lane & 3, hi = r >> 2;
     const char* a0 = (u.cls == 2) ? sd.a0 : sd.b0; // operand A = the block that carries a3 and a4
     const char* a1 = (u.cls == 2) ? sd.a1 : sd.b1;
@@ -213,27 +258,27 @@ __device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec
         const Diag3Rec dr = load_diag(diags + d); // nwA == 1, nwB == 4
         if (d + 1 < u.diag_end) prefetch_diag_c(diags + d + 1, true, tab, lane);
         const int nsteps = dr.send - dr.sbeg;
-        // A table [k][cX & 3][g] (one uint4 per lane and k-step), B table [k][4 pairs] (one uint2 per lane: pairs 2 hi, 2 hi + 1)
         const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA) + (dr.sbeg * 4 + kk) * 4 + (r >> 1);
         const uint2* tB = reinterpret_cast<const uint2*>(tab + dr.offB) + (dr.sbeg * 4 + kk) * 2 + hi;
-        // software pipeline: table words three k-steps ahead in registers; the A gathers of step s + 1 fly under the
-        // MMAs of step s, the (8-term) B gather of step s + 1 is issued after them and folded at the top of step s + 1
-        double2 A[4][NJ], Bv[1], ua[4][NJ], va[4][NJ], ub[2][1], vb[2][1];
-        uint4 a_c = __ldg(tA), a_1 = __ldg(tA + 16), a_2 = __ldg(tA + 32), a_3 = __ldg(tA + 48);
+        double2 A[4][NJ], Bc[1], Bn[1], ua[4][NJ], va[4][NJ], ub[2][1], vb[2][1];
+        uint4 a_c = __ldg(tA), a_1 = __ldg(tA + 16), a_2 = __ldg(tA + 32);
         uint2 b_c = __ldg(tB), b_1 = __ldg(tB + 8), b_2 = __ldg(tB + 16), b_3 = __ldg(tB + 24);
         wide_loads_A_c(a0, a1, a_c, ua, va);
         wide_loads_B_c(sB, b_c, ub, vb);
         wide_subs_A_c(ua, va, a_c, A);
+        wide_fold_B_c(ub, vb, b_c, Bc);   // step 0
+        wide_loads_B_c(sB, b_1, ub, vb);  // step 1, folded at the top of step 0
         for (int s = 0; s < nsteps; ++s) {
             tA += 16; tB += 8;
-            wide_fold_B_c(ub, vb, b_c, Bv);
-            wide_loads_A_c(a0, a1, a_1, ua, va); // k-step s + 1 (one step past the end: valid, unused entries)
-            const uint4 na = __ldg(tA + 48);     // k-step s + 4
-            const uint2 nb = __ldg(tB + 24);
-            mma_wide<NJ>(acc, A, Bv[0], hi);
+            wide_fold_B_c(ub, vb, b_1, Bn);       // k-step s + 1
+            wide_loads_A_c(a0, a1, a_1, ua, va);  // k-step s + 1 (one step past the end: valid, unused entries)
+            wide_loads_B_c(sB, b_2, ub, vb);      // k-step s + 2
+            const uint4 na = __ldg(tA + 32);      // k-step s + 3
+            const uint2 nb = __ldg(tB + 24);      // k-step s + 4
+            mma_wide<NJ>(acc, A, Bc[0], hi);
             wide_subs_A_c(ua, va, a_1, A);
-            wide_loads_B_c(sB, b_1, ub, vb);
-            a_c = a_1; a_1 = a_2; a_2 = a_3; a_3 = na;
+            Bc[0] = Bn[0];
+            a_c = a_1; a_1 = a_2; a_2 = na;
             b_c = b_1; b_1 = b_2; b_2 = b_3; b_3 = nb;
         }
     }
@@ -257,7 +302,7 @@ __device__ __forceinline__ void prefetch_unit_c(const Unit3Rec* urec, const Diag
     prefetch_diag_c(drecs + uv.x, uv.z >= 2, tab, lane);
 }
 
-__global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a) {
+__global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
     extern __shared__ __align__(128) char prod_smem[];
     char* smem = prod_smem;
     char* s_rec = smem + SMC_REC;
@@ -283,15 +328,16 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
         const int4 h1 = __ldg(reinterpret_cast<const int4*>(a.prog + pos) + 1); // diag_begin, ...
         const uint32_t ubytes = (uint32_t)h0.y * (uint32_t)sizeof(Unit3Rec), dbytes = (uint32_t)h0.w * (uint32_t)sizeof(Diag3Rec);
         void* bar = &ctlp->bar_rec[rb];
-        mbar_expect_tx(bar, ubytes + dbytes);
-        bulk_g2s(s_rec + rb * a.rec_stride, a.units + h0.z, ubytes, bar);
-        bulk_g2s(s_rec + rb * a.rec_stride + a.units_bytes, a.diags + h1.x, dbytes, bar);
+        mbar_expect_tx(bar, C_ITEM_BYTES + ubytes + dbytes);
+        bulk_g2s(s_rec + rb * a.rec_stride, a.prog + pos, C_ITEM_BYTES, bar);
+        bulk_g2s(s_rec + rb * a.rec_stride + C_ITEM_BYTES, a.units + h0.z, ubytes, bar);
+        bulk_g2s(s_rec + rb * a.rec_stride + C_ITEM_BYTES + a.units_bytes, a.diags + h1.x, dbytes, bar);
     };
 
     if (tid == 0) {
         for (int i = 0; i < C_NSLOT; ++i) mbar_init(&ctlp->bar_slot[i], 1);
         for (int i = 0; i < C_NREC; ++i) mbar_init(&ctlp->bar_rec[i], 1);
-        for (int i = 0; i < PROD_NBUF; ++i) { mbar_init(&ctlp->full[i], PROD_CWARPS); mbar_init(&ctlp->empty[i], 1); }
+        for (int i = 0; i < PROD_NBUF; ++i) { mbar_init(&ctlp->full[i], C_CWARPS); mbar_init(&ctlp->empty[i], 1); }
         for (int i = 0; i < 8; ++i) { ctl->next_unit[i] = 0; ctl->done_cnt[i] = 0; }
         const long long t0 = (long long)atomicAdd(a.base.counter, 1ull);
         ctl->qtask[0] = t0;
@@ -313,18 +359,28 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
     }
     __syncthreads();
 
-    if (tid >= PROD_CTHREADS) {
+    if (tid >= C_CTHREADS) {
         // ---------------- epilogue warps: combine item i while the compute warps run the following items
-        const int et = tid - PROD_CTHREADS;
+        const int et = tid - C_CTHREADS;
+#ifdef NBS_PROF
+        long long pf[PF_N] = {};
+        const long long pf_start = clock64();
+#endif
         for (unsigned it = 0;; ++it) {
             const int b = it % PROD_NBUF;
             mbar_wait(&ctlp->full[b], (it / PROD_NBUF) & 1u);
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
+            PF_T(t_c);
             combine_item<false>(a.base, ip, q, false, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
+            PF_ADD(PF_EPI_BUSY, t_c);
             if (et == 0) mbar_arrive(&ctlp->empty[b]); // combine_item ends with a barrier of the epilogue threads
         }
+#ifdef NBS_PROF
+        pf[PF_EPI_TOTAL] = clock64() - pf_start;
+        if ((et & 31) == 0) { atomicAdd(&g_cprof[PF_EPI_TOTAL], (unsigned long long)pf[PF_EPI_TOTAL]); atomicAdd(&g_cprof[PF_EPI_BUSY], (unsigned long long)pf[PF_EPI_BUSY]); }
+#endif
         return;
     }
 
@@ -342,17 +398,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
         const size_t q = (size_t)__ldg(a.qhalf + qt), mq = minus_q(a.base.L, q);
         const long long qn = ctl->qtask[(ntask + 1) & 3];
         const bool next_valid = qn < a.ntasks;
-        int4 h0 = __ldg(reinterpret_cast<const int4*>(a.prog));
-        int4 h1 = __ldg(reinterpret_cast<const int4*>(a.prog) + 1);
-        int4 h2 = __ldg(reinterpret_cast<const int4*>(a.prog) + 2);
         for (int pos = 0; pos < a.nitems; ++pos, ++seq) {
-            const int4 c0 = h0, c1 = h1, c2 = h2; // this item; fetch the next one under it
-            if (pos + 1 < a.nitems) {
-                h0 = __ldg(reinterpret_cast<const int4*>(a.prog + pos + 1));
-                h1 = __ldg(reinterpret_cast<const int4*>(a.prog + pos + 1) + 1);
-                h2 = __ldg(reinterpret_cast<const int4*>(a.prog + pos + 1) + 2);
-            }
-            const int ip = c0.x, nunits = c0.y, flags = c2.y;
             const int b = seq % PROD_NBUF, rb = seq % C_NREC, cs = seq & 7;
             PF_T(t_e);
             if (seq >= PROD_NBUF) mbar_wait(&ctlp->empty[b], ((seq / PROD_NBUF) - 1u) & 1u); // ring buffer b is free again
@@ -361,24 +407,20 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
             mbar_wait(&ctlp->bar_rec[rb], (seq / C_NREC) & 1u);
             PF_ADD(PF_REC, t_r);
             PF_T(t_s);
+            // the item, its unit and diagram records: staged in record buffer rb (nothing of it is held in registers
+            // across the units)
+            const int* item = reinterpret_cast<const int*>(s_rec + rb * a.rec_stride);
+            const int nunits = item[1], flags = item[9];
             const int w1 = flags & 7, w2 = (flags >> 3) & 7;
             if (w1) { mbar_wait(&ctlp->bar_slot[w1 - 1], (par >> (w1 - 1)) & 1u); par ^= 1u << (w1 - 1); }
             if (w2) { mbar_wait(&ctlp->bar_slot[w2 - 1], (par >> (w2 - 1)) & 1u); par ^= 1u << (w2 - 1); }
             PF_ADD(PF_SLOT, t_s);
             if (lane == 0) { // every warp writes the same descriptor (the epilogue reads it after the last arrival)
                 ctl->meta_q[b] = (int)((flags & 64) ? mq : q);
-                ctl->meta_pair[b] = ip;
+                ctl->meta_pair[b] = item[0];
             }
-            const Unit3Rec* s_units = reinterpret_cast<const Unit3Rec*>(s_rec + rb * a.rec_stride);
-            const Diag3Rec* s_diags = reinterpret_cast<const Diag3Rec*>(s_rec + rb * a.rec_stride + a.units_bytes);
-            CSides sd; // c1.w / c2.x: byte stride of two planes of B~1 / B~2
-            {
-                const uint32_t ps1 = (uint32_t)c1.w, ps2 = (uint32_t)c2.x, r = (uint32_t)lane >> 2;
-                sd.a0 = smem + (uint32_t)c1.y + (r & 1u) * (ps1 >> 1); sd.a1 = sd.a0 + ps1;
-                sd.b0 = smem + (uint32_t)c1.z + (r & 1u) * (ps2 >> 1); sd.b1 = sd.b0 + ps2;
-                sd.w1 = smem + (uint32_t)c1.y + (r & 3u) * (ps1 >> 1);
-                sd.w2 = smem + (uint32_t)c1.z + (r & 3u) * (ps2 >> 1);
-            }
+            const Unit3Rec* s_units = reinterpret_cast<const Unit3Rec*>(s_rec + rb * a.rec_stride + C_ITEM_BYTES);
+            const Diag3Rec* s_diags = reinterpret_cast<const Diag3Rec*>(s_rec + rb * a.rec_stride + C_ITEM_BYTES + a.units_bytes);
             double2* scr = scr0 + b * scr_stride;
             int* next_unit = const_cast<int*>(&ctl->next_unit[cs]);
             auto grab = [&]() {
@@ -391,11 +433,11 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
                 const int4 uv = *reinterpret_cast<const int4*>(s_units + i);
                 Unit3Rec u;
                 u.diag_begin = uv.x; u.diag_end = uv.y; u.cls = uv.z; u.slot = uv.w;
-                if (i + PROD_CWARPS < nunits) prefetch_unit_c(s_units + i + PROD_CWARPS, s_diags, a.tab, lane);
+                if (i + C_CWARPS < nunits) prefetch_unit_c(s_units + i + C_CWARPS, s_diags, a.tab, lane);
                 double2* out = scr + (size_t)u.slot * 256;
                 PF_T(t_u);
-                if (u.cls < 2) run_unit_square_c(u, s_diags, a.tab, sd, out, lane);
-                else run_unit_wide_c(u, s_diags, a.tab, sd, out, lane);
+                if (u.cls < 2) run_unit_square_c(u, s_diags, a.tab, smem, item, out, lane);
+                else run_unit_wide_c(u, s_diags, a.tab, smem, item, out, lane);
                 PF_ADD(PF_UNITS, t_u);
                 i = grab();
             }
@@ -408,14 +450,14 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
             }
             old = __shfl_sync(0xffffffffu, old, 0);
             PF_T(t_l);
-            if (old == PROD_CWARPS - 1) {
+            if (old == C_CWARPS - 1) {
                 // this warp completed the item: its blocks and records are free.  Lanes issue the release list in
                 // parallel; lane 31 loads the records of the item C_NREC positions ahead into the buffer just vacated.
                 __threadfence_block();
                 if (lane == 0) { ctl->done_cnt[cs] = 0; ctl->next_unit[cs] = 0; }
                 if (lane == 30 && pos == 0) ctl->qtask[(ntask + 2) & 3] = (long long)atomicAdd(a.base.counter, 1ull);
                 __threadfence_block();
-                const int rel_begin = c2.z, nrel = c2.w - c2.z;
+                const int rel_begin = item[10], nrel = item[11] - item[10];
                 if (lane < nrel) {
                     const int4 lv = __ldg(reinterpret_cast<const int4*>(a.loads + rel_begin + lane));
                     CLoad ld; ld.src = lv.x; ld.dst = (uint32_t)lv.y; ld.bytes = (uint32_t)lv.z; ld.bar = lv.w;
@@ -441,7 +483,7 @@ __global__ void __launch_bounds__(PROD_THREADS, 1) k_product_c(const CProdArgs a
 #ifdef NBS_PROF
     pf[PF_TOTAL] = clock64() - pf_start;
     if (lane == 0)
-        for (int i = 0; i < PF_N; ++i) atomicAdd(&g_cprof[i], (unsigned long long)pf[i]);
+        for (int i = 0; i < PF_EPI_TOTAL; ++i) atomicAdd(&g_cprof[i], (unsigned long long)pf[i]);
 #endif
     // no work left: tell the epilogue warps (every warp arrives; lane 0 of each writes the same end marker)
     {

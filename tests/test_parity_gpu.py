@@ -660,10 +660,10 @@ def test_fp64_probe(torch_cuda, nbs):
     with nbs.Nbs(2, 1, [("p", "n", "p", "n")]) as ctx:
         dmma = ctx.probe_fp64(0, 20000)["tflops"]
         assert 10.0 < dmma < 60.0, dmma
-        for mode in (1, 2, 3, 4):
+        for mode in (1, 2, 3, 4, 5, 6, 7, 8):
             assert ctx.probe_fp64(mode, 5000)["tflops"] > 1.0
         with pytest.raises(nbs.NbsError):
-            ctx.probe_fp64(7, 10)
+            ctx.probe_fp64(9, 10)
 
 
 # ------------------------------------------------------------------------------ tile-wise plan (configs[4], g1)
