@@ -467,6 +467,21 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
                         issue_load(ld, q2, minus_q(a.base.L, q2));
                     }
                 }
+                // the loads the NEXT item will release are pulled into L2 now, one item ahead of their bulk copies
+                // (a load that has to wait for the item before it -- no free slot -- then costs an L2 round trip only)
+                if (lane >= 16 && lane < 24 && pos + 1 < a.nitems) {
+                    const int4 nh2 = __ldg(reinterpret_cast<const int4*>(a.prog + pos + 1) + 2); // ps2, flags, rel_begin, rel_end
+                    const int j = nh2.z + (lane - 16);
+                    if (j < nh2.w) {
+                        const int4 lv = __ldg(reinterpret_cast<const int4*>(a.loads + j));
+                        const bool nxt = (lv.x >> 9) & 1;
+                        if (!nxt || next_valid) {
+                            const size_t qq = nxt ? (size_t)__ldg(a.qhalf + qn) : q;
+                            const size_t mom = ((lv.x >> 8) & 1) ? minus_q(a.base.L, qq) : qq;
+                            bulk_prefetch_l2(a.B + mom * a.R + __ldg(a.slot_off + (lv.x & 255)), (uint32_t)lv.z);
+                        }
+                    }
+                }
                 if (lane == 31) {
                     const int pr = pos + C_NREC;
                     if (pr < a.nitems) issue_records(pr, rb);

@@ -638,15 +638,22 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
     // A11)  F~_{a1 a2 ..}(-q) = - F~_{a2 a1 ..}(q)  gives the -q result from the q result.
     auto make_chain = [&](const std::vector<int>& ids) {
         const int n = (int)ids.size();
+        // cost of walking from pair a to pair b: block slots (of C_SLOT_BYTES) to stage, plus a penalty when the new
+        // blocks do not fit beside those of a in the four shared-memory slots of the pipelined kernel -- such a
+        // transition cannot be prefetched: the loads wait for a to complete and every warp waits for the loads
+        auto nsl = [&](int slot) { return plan.slot_kind[slot] == BK_FULL ? 2 : 1; };
         auto tcost = [&](int a, int b) {
-            return (plan.pairs3[ids[a]].slot1 != plan.pairs3[ids[b]].slot1) + (plan.pairs3[ids[a]].slot2 != plan.pairs3[ids[b]].slot2);
+            const Pair3Rec &pa = plan.pairs3[ids[a]], &pb = plan.pairs3[ids[b]];
+            const int used = nsl(pa.slot1) + nsl(pa.slot2);
+            const int fresh = (pa.slot1 != pb.slot1 ? nsl(pb.slot1) : 0) + (pa.slot2 != pb.slot2 ? nsl(pb.slot2) : 0);
+            return fresh + (fresh > C_NSLOT - used ? 8 : 0);
         };
         std::vector<int> best;
         if (n == 0) return;
         if (n <= 16) { // exact: shortest Hamiltonian path by subset DP
             const int N = 1 << n, INF = 1 << 28;
             std::vector<int> dp((size_t)N * n, INF), from((size_t)N * n, -1);
-            for (int i = 0; i < n; ++i) dp[((size_t)1 << i) * n + i] = 2;
+            for (int i = 0; i < n; ++i) dp[((size_t)1 << i) * n + i] = nsl(plan.pairs3[ids[i]].slot1) + nsl(plan.pairs3[ids[i]].slot2);
             for (int m = 1; m < N; ++m)
                 for (int i = 0; i < n; ++i) {
                     const int cur = dp[(size_t)m * n + i];
