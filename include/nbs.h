@@ -224,6 +224,20 @@ int nbs_set_timing(nbs_ctx* ctx, int enable);
  * walks all sites X, no FFT.  Results equal the FFT path up to rounding.  Cost O(V^2): NBS_EINVAL for L > 8.
  */
 int nbs_set_direct(nbs_ctx* ctx, int enable);
+
+/*
+ * nbs_set_pipelined -- which product kernel the resident plan runs (eqs. 4.2-4.3).
+ *   enable != 0 (the default whenever it is available): k_product_c -- antisymmetric blocks staged in their compact
+ *     form, four block slots in shared memory filled by a host-written load program, warps moving from one sink pair
+ *     to the next without a barrier;
+ *   enable == 0: k_product_t -- two staged blocks, antisymmetric blocks expanded to full blocks by an extra pass
+ *     (a second buffer of nbs_workspace_bytes grows by V * 6 * 6960 * 16 bytes per slot on the first call);
+ *   enable < 0: query, returns 1 / 0.
+ * Both give the same correlators up to the rounding order of sums of more than two gather terms.  NBS_EINVAL if the
+ * pipelined kernel is asked for but the plan has none (fewer than three sink-pair items per momentum pair, tile-wise
+ * plan); the tile-wise plan and the direct shifted sum always run k_product_t.  Takes effect at the next nbs_correlator.
+ */
+int nbs_set_pipelined(nbs_ctx* ctx, int enable);
 int nbs_stage_times(nbs_ctx* ctx, double* ms, long long* calls, int reset);
 
 int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);

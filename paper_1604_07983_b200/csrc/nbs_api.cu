@@ -60,7 +60,8 @@ struct nbs_ctx {
     int* d_qorder = nullptr;
     int prod_grid = 0;
     // pipelined product kernel (nbs_product_c.cuh): compact antisymmetric blocks staged as they are, no expansion
-    bool use_c = false;
+    bool use_c = false;    // the pipelined kernel is available (program, shared memory) ...
+    bool pipelined = false; // ... and selected (nbs_set_pipelined; default: yes when available)
     uint32_t* d_tabc = nullptr;
     Diag3Rec* d_diagsc = nullptr;
     CItem* d_cprog = nullptr;
@@ -664,9 +665,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         c->c_rec_stride = C_ITEM_BYTES + c->c_units_bytes + (uint32_t)c->plan.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
         c->c_smem = cprod_smem_bytes(c->c_rec_stride);
         c->use_c = c->plan.cprog_ok && c->c_smem <= (size_t)prop.sharedMemPerBlockOptin && c->plan.baryons.size() < 256;
-#ifdef NBS_NO_PIPELINE
-        c->use_c = false;
-#endif
+        c->pipelined = c->use_c;
     }
     if (c->use_c) {
         CUC(upload(c, c->d_tabc, c->plan.tabc));
@@ -739,6 +738,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
             return NBS_ENOMEM;
         }
         c->tiled = true;
+        c->use_c = c->pipelined = false;
         c->nslices = 1;
         c->ft_rows = maxchan;
         c->chunks.resize(std::min<size_t>(nfit, 2 * c->plan.baryons.size()));
@@ -891,7 +891,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
             rc = fft3d(c, sl.B, c->R, false, st, nullptr, iso ? (size_t)c->plan.row_elems_iso : 0);
             if (rc) return rc;
         }
-        const bool pipelined = c->use_c && !c->direct;
+        const bool pipelined = c->pipelined && !c->direct;
         if (c->Re && !pipelined) { // antisymmetric blocks: mirror halves restored for the gathers of the one-buffer kernel
             k_expand<<<(unsigned)c->V, 256, 0, st>>>(sl.B, c->R, iso ? c->d_gather_iso : c->d_gather, (int)c->Re, sl.Be);
             CU(c, cudaGetLastError());
@@ -902,7 +902,7 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     {
         StageTimer tm(c, NBS_STAGE_PRODUCT, st);
         CU(c, cudaMemsetAsync(sl.counter, 0, sizeof(unsigned long long), st));
-        const bool pipelined = c->use_c && !c->direct;
+        const bool pipelined = c->pipelined && !c->direct;
         ProdArgs pa;
         pa.Bc = sl.B; pa.Rc = c->R; pa.Be = sl.Be; pa.Re = c->Re; pa.L = c->L;
         pa.slot_src = reinterpret_cast<const int2*>(c->d_slot_src);
@@ -953,18 +953,39 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
     return slot_release(c, sl, st);
 }
 
+// the expanded antisymmetric blocks of the one-buffer kernel exist only once somebody asks for that kernel
+static int ensure_expanded(nbs_ctx* c) {
+    if (!c->Re || c->tiled) return NBS_OK;
+    for (int i = 0; i < c->nslices; ++i)
+        if (!c->slice[i].Be) {
+            CU(c, cudaSetDevice(c->device));
+            int rc = dev_alloc(c, c->slice[i].Be, c->V * c->Re);
+            if (rc) return rc;
+        }
+    return NBS_OK;
+}
+
 int nbs_set_direct(nbs_ctx* c, int enable) {
     if (!c) return NBS_EINVAL;
     if (enable && c->L > 8) return fail(c, NBS_EINVAL, "the direct shifted sum is O(V^2): allowed for L <= 8 only");
     if (enable && c->tiled) return fail(c, NBS_EINVAL, "the direct shifted sum is not available with the tile-wise plan");
-    if (enable && c->Re) // the direct sum runs the one-buffer kernel on expanded x-space blocks
-        for (int i = 0; i < c->nslices; ++i)
-            if (!c->slice[i].Be) {
-                CU(c, cudaSetDevice(c->device));
-                int rc = dev_alloc(c, c->slice[i].Be, c->V * c->Re);
-                if (rc) return rc;
-            }
+    if (enable) { // the direct sum runs the one-buffer kernel on expanded x-space blocks
+        int rc = ensure_expanded(c);
+        if (rc) return rc;
+    }
     c->direct = enable != 0;
+    return NBS_OK;
+}
+
+int nbs_set_pipelined(nbs_ctx* c, int enable) {
+    if (!c) return NBS_EINVAL;
+    if (enable < 0) return c->pipelined ? 1 : 0; // query
+    if (enable && !c->use_c) return fail(c, NBS_EINVAL, "the pipelined product kernel is not available for this plan (fewer than 3 sink-pair items per momentum pair, tile-wise plan, or too many unit records for shared memory)");
+    if (!enable) {
+        int rc = ensure_expanded(c);
+        if (rc) return rc;
+    }
+    c->pipelined = enable != 0;
     return NBS_OK;
 }
 

@@ -55,6 +55,7 @@ struct BlockRec {
 constexpr int BLOCKS_THREADS = 256;
 constexpr int BLOCKS_TILES = 216;               // 6 x 6 x 6 tiles of 2 x 2 x 2 source triples
 constexpr int BLOCKS_HALF = 2 * SM_PLANE;       // complex entries of a half row
+static_assert(AS_BLOCK <= BLOCKS_HALF, "a compact antisymmetric block is assembled in the half-row buffer");
 // Shared-memory operand layouts of k_blocks, chosen so that the register tiles of a warp (tile origins
 // 2 i per index, lanes on consecutive i) read without bank conflicts: a source index xi sits at
 // dq_rank(xi) = (xi & 1) * 6 + (xi >> 1) (even and odd values de-interleaved: the lanes' even origins

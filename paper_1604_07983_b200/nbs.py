@@ -27,7 +27,7 @@ BARYON_NAME = {v: k for k, v in BARYON_ID.items()}
 EXPORTS = ["nbs_create", "nbs_load_propagators", "nbs_correlator", "nbs_destroy", "nbs_last_error",
            "nbs_workspace_bytes", "nbs_num_channels", "nbs_channel_info", "nbs_std_channels",
            "nbs_diagram_stats", "nbs_blocks_x", "nbs_model_flops", "nbs_exec_flops", "nbs_fft3d",
-           "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_num_slots",
+           "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_set_pipelined", "nbs_num_slots",
            "nbs_probe_fp64", "nbs_tiled_info", "nbs_pair_order", "nbs_plan_selfcheck"]
 
 
@@ -70,6 +70,7 @@ def lib() -> ctypes.CDLL:
         L.nbs_fft3d.argtypes = [c_void_p, c_void_p, c_size_t, c_int, c_void_p]
         L.nbs_set_timing.argtypes = [c_void_p, c_int]
         L.nbs_set_direct.argtypes = [c_void_p, c_int]
+        L.nbs_set_pipelined.argtypes = [c_void_p, c_int]
         L.nbs_stage_times.argtypes = [c_void_p, POINTER(c_double), POINTER(c_longlong), c_int]
         L.nbs_kernel_launches.argtypes = [c_void_p]
         L.nbs_num_slots.argtypes = [c_void_p]
@@ -241,6 +242,13 @@ class Nbs:
     def set_direct(self, enable: bool = True):
         """nbs_set_direct: eq. 2.4 as a shifted sum in x-space (tiny lattices, L <= 8)."""
         _check(self.ctx, lib().nbs_set_direct(self.ctx, 1 if enable else 0))
+
+    def set_pipelined(self, enable: bool = True):
+        """nbs_set_pipelined: choose the pipelined product kernel (compact blocks, default) or the one-buffer one."""
+        _check(self.ctx, lib().nbs_set_pipelined(self.ctx, 1 if enable else 0))
+
+    def pipelined(self) -> bool:
+        return bool(_check(self.ctx, lib().nbs_set_pipelined(self.ctx, -1)))
 
     def set_timing(self, enable: bool = True):
         _check(self.ctx, lib().nbs_set_timing(self.ctx, 1 if enable else 0))

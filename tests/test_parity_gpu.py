@@ -771,3 +771,74 @@ def test_repeated_runs_are_bitwise_identical(torch_cuda, nbs):
                 assert torch.equal(F, first), ("tile-wise", rep)
         # against the resident plan: the same product arithmetic, another order of the inverse FFT passes
         assert float((first - ref).abs().max()) <= 1e-13 * float(ref.abs().max())
+
+
+# ------------------------------------------------------------------------------ the two product kernels
+@pytest.mark.parametrize("L,same", [(4, ()), (6, ()), (4, (("d", "u"),))])
+def test_pipelined_kernel_equals_one_buffer_kernel_and_oracle(torch_cuda, nbs, oracle, L, same):
+    """nbs_set_pipelined: k_product_c (compact antisymmetric blocks staged as stored, load program, no barrier between
+    sink pairs) and k_product_t (expanded blocks, two buffers) evaluate the same gather terms -- all 52 channels
+    agree to rounding, and both match the oracle (eq. 2.6 path).  With d == u the pipelined kernel reads the blocks of
+    n, Sigma-, Xi- from their partners' compact blocks with a sign."""
+    torch = torch_cuda
+    S = props(L, seed=77, t=1, same=same)
+    chans = oracle.channels52()
+    with nbs.Nbs(L, 2) as ctx:
+        assert ctx.pipelined()
+        ws0 = ctx.workspace_bytes()
+        d = to_dev(torch, S)
+        ctx.load(1, d["u"], d["d"], d["s"])
+        Fp = ctx.correlator(1).clone()
+        n0 = ctx.kernel_launches()
+        ctx.set_pipelined(False)                      # allocates the expanded-block buffer
+        assert not ctx.pipelined() and ctx.workspace_bytes() > ws0
+        Fo1 = ctx.correlator(1).clone()
+        n1 = ctx.kernel_launches()
+        ctx.set_pipelined(True)
+        Fp2 = ctx.correlator(1)
+        torch.cuda.synchronize()
+        assert n1 - n0 == (ctx.kernel_launches() - n1) + 1  # the one-buffer path has one more launch: the expansion pass
+        assert torch.equal(Fp, Fp2)                   # bitwise reproducible, also after switching back
+        scale = float(Fo1.abs().max())
+        assert float((Fp - Fo1).abs().max()) <= 1e-13 * scale
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    Fo = oracle.correlator_fft(L, B, chans)
+    assert_parity(Fp.cpu().numpy(), Fo, chans)
+    assert_parity(Fo1.cpu().numpy(), Fo, chans)
+
+
+def test_pipelined_kernel_needs_three_items(torch_cuda, nbs, oracle):
+    """A plan with a single sink pair has fewer than three items per momentum pair: the library runs the one-buffer
+    kernel, says so, and refuses the switch."""
+    torch = torch_cuda
+    chans = [("p", "n", "p", "n")]
+    with nbs.Nbs(4, 1, chans) as ctx:
+        assert not ctx.pipelined()
+        with pytest.raises(nbs.NbsError):
+            ctx.set_pipelined(True)
+        S = props(4, seed=5)
+        d = to_dev(torch, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        F = ctx.correlator(0).cpu().numpy()
+    B = oracle.all_blocks(S, oracle.sink_names(chans))
+    assert_parity(F, oracle.correlator_fft(4, B, chans), chans)
+
+
+def test_pipelined_kernel_user_channel_lists(torch_cuda, nbs, oracle):
+    """Load programs for other channel lists: a full-full-only list (every transition waits for the previous item), a
+    mixed list with elementary operators, a list whose half chain is empty (identical sink baryons only)."""
+    torch = torch_cuda
+    lists = [
+        [("L", "L", "L", "L"), ("S0", "L", "S0", "L"), ("S0", "S0", "L", "L"), ("S0", "S0", "Sp", "Sm")],
+        [("p", "L", "p", "L"), ("Sp", "n", "p", "L"), ("S0", "p", "Sp", "n"), ("Xm", "L", "Xm", "L"), ("p", "n", "p", "n")],
+        [("L", "L", "L", "L"), ("S0", "S0", "S0", "S0"), ("p", "p", "p", "p")],
+    ]
+    for L, chans in zip((4, 3, 4), lists):
+        S = props(L, seed=31 + L)
+        with nbs.Nbs(L, 1, chans) as ctx:
+            assert ctx.pipelined()
+            d = to_dev(torch, S)
+            ctx.load(0, d["u"], d["d"], d["s"])
+            F = ctx.correlator(0).cpu().numpy()
+        B = oracle.all_blocks(S, oracle.sink_names(chans))
+        assert_parity(F, oracle.correlator_fft(L, B, chans), chans)
