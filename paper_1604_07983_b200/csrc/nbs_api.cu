@@ -477,26 +477,36 @@ int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
         if (P.cprog_ok) {
             if ((int)P.cprog.size() != P.chain_full_n + P.chain_half_n || (int)P.cprog.size() < C_NREC) return -136;
             std::vector<int> fresh(C_NSLOT, 0), loaded(C_NSLOT, 0);
+            // half slots (nbs_tables.hpp) covered by a block of `kind` whose first slot starts at byte offset `off`
+            auto halves = [&](uint32_t off, int kind, unsigned& mask) {
+                mask = 0;
+                if (off % C_HALF_BYTES) return false;
+                const int h = (int)(off / C_HALF_BYTES);
+                if (kind == BK_FULL) { if (h % 4) return false; mask = 0xfu << h; }
+                else { if (h % 4 > 1) return false; mask = (1u << h) | (1u << (h + 2)); }
+                return h < 2 * C_NSLOT && (mask >> (2 * C_NSLOT)) == 0;
+            };
+            auto slot_of_off = [&](uint32_t off) { const int h = (int)(off / C_HALF_BYTES); return (h / 4) * 2 + (h % 4); };
             for (size_t i = 0; i < P.cprog.size(); ++i) {
                 const CItem& it = P.cprog[i];
                 const Pair3Rec& pr = P.pairs3[it.pair];
-                const uint32_t n1 = (uint32_t)block_elems(P.slot_kind[pr.slot1]) * 16u, n2 = (uint32_t)block_elems(P.slot_kind[pr.slot2]) * 16u;
-                if (it.off1 % C_SLOT_BYTES || it.off2 % C_SLOT_BYTES) return -137;
-                if (it.off1 + n1 > C_NSLOT * C_SLOT_BYTES || it.off2 + n2 > C_NSLOT * C_SLOT_BYTES) return -138;
-                if (it.off1 < it.off2 + n2 && it.off2 < it.off1 + n1) return -139; // the two blocks of an item do not overlap
-                if (it.ps1 != 2u * (uint32_t)plane_elems(P.slot_kind[pr.slot1]) * 16u || it.ps2 != 2u * (uint32_t)plane_elems(P.slot_kind[pr.slot2]) * 16u) return -140;
+                unsigned m1, m2;
+                if (!halves(it.off1, P.slot_kind[pr.slot1], m1) || !halves(it.off2, P.slot_kind[pr.slot2], m2)) return -137;
+                if (m1 & m2) return -139; // the two blocks of an item do not overlap
+                if (it.ps1 != (uint32_t)plane_elems(P.slot_kind[pr.slot1]) * 16u || it.ps2 != (uint32_t)plane_elems(P.slot_kind[pr.slot2]) * 16u) return -140;
                 if (it.rel_begin > it.rel_end || it.rel_end > (int)P.cloads.size()) return -141;
                 for (int side = 0; side < 2; ++side) {
                     const int w = (it.flags >> (3 * side)) & 7;
                     if (w > C_NSLOT) return -142;
-                    if (w && (uint32_t)(w - 1) * C_SLOT_BYTES != (side ? it.off2 : it.off1)) return -143;
+                    if (w && w - 1 != slot_of_off(side ? it.off2 : it.off1)) return -143;
                     if (w) ++fresh[w - 1];
                 }
             }
             for (auto& ld : P.cloads) {
                 if ((ld.src & 255) >= (int)P.baryons.size() || ld.bar < 0 || ld.bar >= C_NSLOT) return -144;
-                if (ld.dst != (uint32_t)ld.bar * C_SLOT_BYTES || ld.bytes != (uint32_t)block_elems(P.slot_kind[ld.src & 255]) * 16u) return -145;
-                if (ld.dst + ld.bytes > C_NSLOT * C_SLOT_BYTES || ld.bytes % 64) return -146;
+                unsigned m;
+                if (!halves(ld.dst, P.slot_kind[ld.src & 255], m) || slot_of_off(ld.dst) != ld.bar) return -145;
+                if (ld.bytes != (uint32_t)block_elems(P.slot_kind[ld.src & 255]) * 16u || ld.bytes % 64) return -146;
                 ++loaded[ld.bar];
             }
             for (int s = 0; s < C_NSLOT; ++s)

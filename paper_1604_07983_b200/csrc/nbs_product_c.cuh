@@ -52,7 +52,7 @@ struct CCtrl {
     long long qtask[4];                   // task indices of this CTA (task number modulo 4)
     int meta_q[PROD_NBUF], meta_pair[PROD_NBUF];
 };
-constexpr uint32_t SMC_REC = C_NSLOT * C_SLOT_BYTES; // 222 720
+constexpr uint32_t SMC_REC = C_BLOCKS_BYTES; // 222 720: the block slots come first
 constexpr uint32_t C_ITEM_BYTES = 48;
 static_assert(sizeof(CItem) == C_ITEM_BYTES, "CItem is read as three int4");
 inline size_t cprod_smem_bytes(uint32_t rec_stride) {
@@ -66,16 +66,16 @@ __device__ __forceinline__ void mbar_arrive(void* bar) {
 __device__ __forceinline__ double flipd(double v, uint32_t w) {
     return __hiloint2double(__double2hiint(v) ^ (int)(w & 0x80000000u), __double2loint(v));
 }
-// One packed table word (nbs_tables.hpp) = one (+, -) pair of gather terms.  p0 / p1: the lane's sink-spin plane a
-// and plane a + 2 of the staged block.
+// One packed table word (nbs_tables.hpp) = one (+, -) pair of gather terms.  p0: the lane's sink-spin plane a of the
+// staged block; plane a + 2 lies C_PAIR_BYTES further in both kinds of block (an immediate offset of the load).
 template <int NP>
-__device__ __forceinline__ void ldc(const char* p0, const char* p1, uint32_t w, double2 (&u)[NP], double2 (&v)[NP]) {
+__device__ __forceinline__ void ldc(const char* p0, uint32_t w, double2 (&u)[NP], double2 (&v)[NP]) {
     const uint32_t ox = w & 0x7ff0u, oy = (w >> 16) & 0x7ff0u;
     u[0] = *reinterpret_cast<const double2*>(p0 + ox);
     v[0] = *reinterpret_cast<const double2*>(p0 + oy);
     if (NP == 2) {
-        u[NP - 1] = *reinterpret_cast<const double2*>(p1 + ox);
-        v[NP - 1] = *reinterpret_cast<const double2*>(p1 + oy);
+        u[NP - 1] = *reinterpret_cast<const double2*>(p0 + ox + C_PAIR_BYTES);
+        v[NP - 1] = *reinterpret_cast<const double2*>(p0 + oy + C_PAIR_BYTES);
     }
 }
 template <int NP, bool FIRST>
@@ -101,18 +101,18 @@ __device__ unsigned long long g_cprof[PF_N];
 #define PF_ADD(idx, t0)
 #endif
 
-// Per-lane views of the two staged blocks of an item: a0 / a1 = B~1 at the lane's plane (r & 1) and two planes
-// further, b0 / b1 the same for B~2; w1 / w2 = plane (r & 3) of B~1 / B~2 (operand B of the 64 x 4 classes).
-struct CSides { const char *a0, *a1, *b0, *b1, *w1, *w2; };
-// item: the staged CItem (shared memory); words 5-8 = off1, off2, ps1, ps2
+// Per-lane views of the two staged blocks of an item: a0 = B~1 at the lane's plane (r & 1), b0 the same for B~2;
+// w1 / w2 = plane (r & 3) of B~1 / B~2 (operand B of the 64 x 4 classes).
+struct CSides { const char *a0, *b0, *w1, *w2; };
+// item: the staged CItem (shared memory); words 5-8 = off1, off2, ps1, ps2 (ps: bytes of one plane)
 __device__ __forceinline__ CSides make_sides(const char* smem, const int* item, int lane) {
     const uint32_t off1 = (uint32_t)item[5], off2 = (uint32_t)item[6], ps1 = (uint32_t)item[7], ps2 = (uint32_t)item[8];
     const uint32_t r = (uint32_t)lane >> 2;
     CSides sd;
-    sd.a0 = smem + off1 + (r & 1u) * (ps1 >> 1); sd.a1 = sd.a0 + ps1;
-    sd.b0 = smem + off2 + (r & 1u) * (ps2 >> 1); sd.b1 = sd.b0 + ps2;
-    sd.w1 = smem + off1 + (r & 3u) * (ps1 >> 1);
-    sd.w2 = smem + off2 + (r & 3u) * (ps2 >> 1);
+    sd.a0 = smem + off1 + (r & 1u) * ps1;
+    sd.b0 = smem + off2 + (r & 1u) * ps2;
+    sd.w1 = sd.a0 + ((r >> 1) & 1u) * C_PAIR_BYTES;
+    sd.w2 = sd.b0 + ((r >> 1) & 1u) * C_PAIR_BYTES;
     return sd;
 }
 
@@ -126,11 +126,11 @@ __device__ __forceinline__ void prefetch_diag_c(const Diag3Rec* dp, bool wide, c
     }
 }
 
-__device__ __forceinline__ void wide_loads_A_c(const char* a0, const char* a1, uint4 w, double2 (&ua)[4][2], double2 (&va)[4][2]) {
-    ldc<2>(a0, a1, w.x, ua[0], va[0]);
-    ldc<2>(a0, a1, w.y, ua[1], va[1]);
-    ldc<2>(a0, a1, w.z, ua[2], va[2]);
-    ldc<2>(a0, a1, w.w, ua[3], va[3]);
+__device__ __forceinline__ void wide_loads_A_c(const char* a0, uint4 w, double2 (&ua)[4][2], double2 (&va)[4][2]) {
+    ldc<2>(a0, w.x, ua[0], va[0]);
+    ldc<2>(a0, w.y, ua[1], va[1]);
+    ldc<2>(a0, w.z, ua[2], va[2]);
+    ldc<2>(a0, w.w, ua[3], va[3]);
 }
 __device__ __forceinline__ void wide_subs_A_c(const double2 (&ua)[4][2], const double2 (&va)[4][2], uint4 w, double2 (&A)[4][2]) {
     subc<2, true>(ua[0], va[0], w.x, A[0]);
@@ -141,8 +141,8 @@ __device__ __forceinline__ void wide_subs_A_c(const double2 (&ua)[4][2], const d
 // B entry (8 gather terms = 4 pairs): the lanes hi = 0 and hi = 1 of one (aY, k) need the same entry, so each gathers
 // two of the four pairs and the halves are exchanged with a shuffle (lane ^ 16 flips hi)
 __device__ __forceinline__ void wide_loads_B_c(const char* sB, uint2 bw, double2 (&ub)[2][1], double2 (&vb)[2][1]) {
-    ldc<1>(sB, sB, bw.x, ub[0], vb[0]);
-    ldc<1>(sB, sB, bw.y, ub[1], vb[1]);
+    ldc<1>(sB, bw.x, ub[0], vb[0]);
+    ldc<1>(sB, bw.y, ub[1], vb[1]);
 }
 __device__ __forceinline__ void wide_fold_B_c(const double2 (&ub)[2][1], const double2 (&vb)[2][1], uint2 bw, double2 (&Bv)[1]) {
     double2 part[1];
@@ -171,15 +171,15 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
             uint32_t wa1 = ldw(tA + 16), wb1 = ldw(tB + 16), wa2 = ldw(tA + 32), wb2 = ldw(tB + 32);
             uint32_t wa3 = ldw(tA + 48), wb3 = ldw(tB + 48), wa4 = ldw(tA + 64), wb4 = ldw(tB + 64);
             double2 A0[NT], B0[NT], A1[NT], B1[NT], ua[NT], va[NT], ub[NT], vb[NT];
-            ldc<NT>(sd.a0, sd.a1, wa0, ua, va);
-            ldc<NT>(sd.b0, sd.b1, wb0, ub, vb);
+            ldc<NT>(sd.a0, wa0, ua, va);
+            ldc<NT>(sd.b0, wb0, ub, vb);
             subc<NT, true>(ua, va, wa0, A0);
             subc<NT, true>(ub, vb, wb0, B0);
             // one k-step: MMAs on (A, B), operands of the next k-step into (An, Bn)
             auto kstep = [&](const double2 (&A)[NT], const double2 (&B)[NT], double2 (&An)[NT], double2 (&Bn)[NT]) {
                 tA += 16; tB += 16;
-                ldc<NT>(sd.a0, sd.a1, wa1, ua, va); // k-step s + 1 (one step past the end: a valid, unused entry)
-                ldc<NT>(sd.b0, sd.b1, wb1, ub, vb);
+                ldc<NT>(sd.a0, wa1, ua, va); // k-step s + 1 (one step past the end: a valid, unused entry)
+                ldc<NT>(sd.b0, wb1, ub, vb);
                 const uint32_t na = ldw(tA + 64), nb = ldw(tB + 64); // k-step s + 5
                 double sA[NT], sB[NT];
 #pragma unroll
@@ -219,8 +219,8 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
                     const uint32_t xa[4] = {qa.x, qa.y, qa.z, qa.w}, xb[4] = {qb.x, qb.y, qb.z, qb.w};
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
-                        ldc<NT>(sd.a0, sd.a1, xa[e], ua, va);
-                        ldc<NT>(sd.b0, sd.b1, xb[e], ub, vb);
+                        ldc<NT>(sd.a0, xa[e], ua, va);
+                        ldc<NT>(sd.b0, xb[e], ub, vb);
                         subc<NT, false>(ua, va, xa[e], A);
                         subc<NT, false>(ub, vb, xb[e], B);
                     }
@@ -250,7 +250,6 @@ __device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec
     const CSides sd = make_sides(smem, item, lane);
     const int r = lane >> 2, kk = lane & 3, hi = r >> 2;
     const char* a0 = (u.cls == 2) ? sd.a0 : sd.b0; // operand A = the block that carries a3 and a4
-    const char* a1 = (u.cls == 2) ? sd.a1 : sd.b1;
     const char* sB = (u.cls == 2) ? sd.w2 : sd.w1; // operand B at the lane's plane aY = r & 3
     constexpr int NJ = 2;
     double acc[NJ * 4][2] = {};
@@ -263,7 +262,7 @@ __device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec
         double2 A[4][NJ], Bc[1], Bn[1], ua[4][NJ], va[4][NJ], ub[2][1], vb[2][1];
         uint4 a_c = __ldg(tA), a_1 = __ldg(tA + 16), a_2 = __ldg(tA + 32);
         uint2 b_c = __ldg(tB), b_1 = __ldg(tB + 8), b_2 = __ldg(tB + 16), b_3 = __ldg(tB + 24);
-        wide_loads_A_c(a0, a1, a_c, ua, va);
+        wide_loads_A_c(a0, a_c, ua, va);
         wide_loads_B_c(sB, b_c, ub, vb);
         wide_subs_A_c(ua, va, a_c, A);
         wide_fold_B_c(ub, vb, b_c, Bc);   // step 0
@@ -271,7 +270,7 @@ __device__ __forceinline__ void run_unit_wide_c(const Unit3Rec u, const Diag3Rec
         for (int s = 0; s < nsteps; ++s) {
             tA += 16; tB += 8;
             wide_fold_B_c(ub, vb, b_1, Bn);       // k-step s + 1
-            wide_loads_A_c(a0, a1, a_1, ua, va);  // k-step s + 1 (one step past the end: valid, unused entries)
+            wide_loads_A_c(a0, a_1, ua, va);  // k-step s + 1 (one step past the end: valid, unused entries)
             wide_loads_B_c(sB, b_2, ub, vb);      // k-step s + 2
             const uint4 na = __ldg(tA + 32);      // k-step s + 3
             const uint2 nb = __ldg(tB + 24);      // k-step s + 4
@@ -319,9 +318,13 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
         const char* src = reinterpret_cast<const char*>(a.B + mom * a.R + __ldg(a.slot_off + (ld.src & 255)));
         void* bar = &ctlp->bar_slot[ld.bar];
         mbar_expect_tx(bar, ld.bytes);
-        const uint32_t part = ld.bytes >> 2; // four copies in flight (a multiple of 16 bytes for both block kinds)
+        // four copies in flight, one per sink-spin plane: a full block is contiguous in shared memory, a compact block
+        // has its planes 2, 3 C_PAIR_BYTES after its planes 0, 1 (nbs_tables.hpp)
+        const uint32_t part = ld.bytes >> 2;
+        const bool full = ld.bytes == BLOCK_BYTES;
 #pragma unroll
-        for (int p = 0; p < 4; ++p) bulk_g2s(smem + ld.dst + p * part, src + (size_t)p * part, part, bar);
+        for (int p = 0; p < 4; ++p)
+            bulk_g2s(smem + ld.dst + (full ? p * part : (p >> 1) * C_PAIR_BYTES + (p & 1) * part), src + (size_t)p * part, part, bar);
     };
     auto issue_records = [&](int pos, int rb) {
         const int4 h0 = __ldg(reinterpret_cast<const int4*>(a.prog + pos));     // pair, nunits, unit_begin, ndiags

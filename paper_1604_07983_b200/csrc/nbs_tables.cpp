@@ -638,7 +638,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
     // A11)  F~_{a1 a2 ..}(-q) = - F~_{a2 a1 ..}(q)  gives the -q result from the q result.
     auto make_chain = [&](const std::vector<int>& ids) {
         const int n = (int)ids.size();
-        // cost of walking from pair a to pair b: block slots (of C_SLOT_BYTES) to stage, plus a penalty when the new
+        // cost of walking from pair a to pair b: block slots to stage, plus a penalty when the new
         // blocks do not fit beside those of a in the four shared-memory slots of the pipelined kernel -- such a
         // transition cannot be prefetched: the loads wait for a to complete and every warp waits for the loads
         auto nsl = [&](int slot) { return plan.slot_kind[slot] == BK_FULL ? 2 : 1; };
@@ -767,7 +767,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
                     base[side] = best; fresh[side] = true;
                     CLoad ld;
                     ld.src = (nd[side].id >> 1) | ((nd[side].id & 1) << 8);
-                    ld.dst = (uint32_t)best * C_SLOT_BYTES;
+                    ld.dst = c_slot_base(best);
                     ld.bytes = (uint32_t)block_elems(plan.slot_kind[nd[side].id >> 1]) * 16u;
                     ld.bar = best;
                     int dep = best_last; // the item whose completion frees the destination; < 0: an item of the previous task
@@ -780,9 +780,9 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
                 }
                 for (int side = 0; side < 2; ++side)
                     for (int k = base[side]; k < base[side] + nd[side].nslots; ++k) st[k].last = i;
-                it.off1 = (uint32_t)base[0] * C_SLOT_BYTES; it.off2 = (uint32_t)base[1] * C_SLOT_BYTES;
-                it.ps1 = 2u * (uint32_t)plane_elems(plan.slot_kind[nd[0].id >> 1]) * 16u;
-                it.ps2 = 2u * (uint32_t)plane_elems(plan.slot_kind[nd[1].id >> 1]) * 16u;
+                it.off1 = c_slot_base(base[0]); it.off2 = c_slot_base(base[1]);
+                it.ps1 = (uint32_t)plane_elems(plan.slot_kind[nd[0].id >> 1]) * 16u;
+                it.ps2 = (uint32_t)plane_elems(plan.slot_kind[nd[1].id >> 1]) * 16u;
                 if (fresh[0]) it.flags |= 1 + base[0];
                 if (fresh[1]) it.flags |= (1 + base[1]) << 3;
             }

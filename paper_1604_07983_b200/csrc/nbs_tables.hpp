@@ -146,8 +146,11 @@ struct ChainRec { // order in which one CTA walks the sink pairs of one momentum
 };
 
 // ---- pipelined product kernel (k_product_c): compact antisymmetric blocks staged as they are -------------
-// Shared memory holds four block slots of C_SLOT_BYTES: a compact antisymmetric block takes one, a full staged
-// block two adjacent ones (0-1 or 2-3).  One task = one momentum pair (q, -q): the full chain at q followed by
+// Shared memory holds four block slots: a compact antisymmetric block takes one, a full staged block two adjacent
+// ones (0-1 or 2-3).  The slots are interleaved in units of half slots (C_HALF_BYTES = one full plane = two compact
+// planes): slot s = 2 q + i owns the half slots 4 q + i and 4 q + i + 2, so that in BOTH kinds of block the sink-spin
+// planes a and a + 2 lie C_PAIR_BYTES apart (a full block in slots 2 q, 2 q + 1 is simply contiguous): the gathers
+// reach plane a + 2 through a compile-time offset.  One task = one momentum pair (q, -q): the full chain at q followed by
 // the half chain at -q.  The host simulates the walk once (build_plan) and writes a static program: for every
 // item the slots of its two blocks, which of them are fresh loads (the item waits for the slot's barrier), and
 // a release list -- the bulk copies that may be issued as soon as the item is complete, because they overwrite
@@ -159,14 +162,17 @@ struct ChainRec { // order in which one CTA walks the sink pairs of one momentum
 //   (a set flip flag: the loaded value enters with the opposite sign -- compact blocks only, see build_plan).
 //   16x16 sides  [k][c (carried spin)][nw]          64x4 A side  [k][cX & 3][g = cX >> 2]          64x4 B side  [k][nw = 4]
 constexpr int C_TAB_LOOKAHEAD = 5; // k-steps the kernel's register pipeline may read past the end of a range (tables are padded by as many)
-constexpr uint32_t C_SLOT_BYTES = 2u * SM_PLANE * 16u; // 55 680 >= AS_BLOCK * 16 = 55 552
+constexpr uint32_t C_HALF_BYTES = SM_PLANE * 16u;      // 27 840 >= 2 * AS_PLANE * 16 = 27 776
+constexpr uint32_t C_PAIR_BYTES = 2u * C_HALF_BYTES;   // distance of the planes a and a + 2 of a staged block
 constexpr int C_NSLOT = 4;
+constexpr uint32_t C_BLOCKS_BYTES = 2u * C_NSLOT * C_HALF_BYTES; // 222 720
+NBS_HD constexpr uint32_t c_slot_base(int s) { return (uint32_t)((s >> 1) * 4 + (s & 1)) * C_HALF_BYTES; }
 constexpr int C_NREC = 3; // unit / diagram record buffers: a warp may run two items ahead of the slowest one
 struct CItem { // 48 bytes, read as three int4
     int pair, nunits, unit_begin, ndiags;
     int diag_begin;
-    uint32_t off1, off2;     // shared-memory byte offsets of B~1 and B~2 of this item
-    uint32_t ps1, ps2;       // byte stride between the sink-spin planes a and a + 2 of the two blocks
+    uint32_t off1, off2;     // shared-memory byte offsets of B~1 and B~2 of this item (c_slot_base of their first slot)
+    uint32_t ps1, ps2;       // bytes of one sink-spin plane of the two blocks (planes a, a + 1 are adjacent)
     int flags;               // bits 0-2: 1 + slot to wait for on side 1 (0: resident); bits 3-5: same for side 2;
                              // bit 6: the item belongs to momentum -q of the task (half chain)
     int rel_begin, rel_end;  // release list (Plan::cloads) of this item
