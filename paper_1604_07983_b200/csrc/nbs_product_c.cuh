@@ -208,39 +208,21 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
             if (s < nsteps) kstep(A0, B0, A1, B1);
         } else {
             const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry): 16-byte groups of four words
-            const int ng = nw >> 2;
             const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA + ((dr.sbeg * 4 + kk) * 4 + c) * nw);
             const uint4* tB = reinterpret_cast<const uint4*>(tab + dr.offB + ((dr.sbeg * 4 + kk) * 4 + c) * nw);
-            // all table words of a k-step are fetched at once (one L2 round trip per step instead of one per group),
-            // those of the next step while the gathers of this one run
-            uint4 qa[3], qb[3];
-#pragma unroll
-            for (int j = 0; j < 3; ++j)
-                if (j < ng) { qa[j] = __ldg(tA + j); qb[j] = __ldg(tB + j); }
-            for (int s = 0; s < nsteps; ++s) {
+            for (int s = 0; s < nsteps; ++s, tA += 4 * nw, tB += 4 * nw) {
                 double2 A[NT], B[NT], ua[NT], va[NT], ub[NT], vb[NT];
-                uint4 ca[3], cb[3];
-#pragma unroll
-                for (int j = 0; j < 3; ++j) { ca[j] = qa[j]; cb[j] = qb[j]; }
-                tA += 4 * nw; tB += 4 * nw; // 4 k x 4 c x nw words per k-step
-                if (s + 1 < nsteps) {
-#pragma unroll
-                    for (int j = 0; j < 3; ++j)
-                        if (j < ng) { qa[j] = __ldg(tA + j); qb[j] = __ldg(tB + j); }
-                }
 #pragma unroll
                 for (int p = 0; p < NT; ++p) A[p] = B[p] = make_double2(0.0, 0.0);
+                for (int j = 0; j < nw / 4; ++j) {
+                    const uint4 qa = __ldg(tA + j), qb = __ldg(tB + j);
+                    const uint32_t xa[4] = {qa.x, qa.y, qa.z, qa.w}, xb[4] = {qb.x, qb.y, qb.z, qb.w};
 #pragma unroll
-                for (int j = 0; j < 3; ++j) {
-                    if (j < ng) {
-                        const uint32_t xa[4] = {ca[j].x, ca[j].y, ca[j].z, ca[j].w}, xb[4] = {cb[j].x, cb[j].y, cb[j].z, cb[j].w};
-#pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            ldc<NT>(sd.a0, xa[e], ua, va);
-                            ldc<NT>(sd.b0, xb[e], ub, vb);
-                            subc<NT, false>(ua, va, xa[e], A);
-                            subc<NT, false>(ub, vb, xb[e], B);
-                        }
+                    for (int e = 0; e < 4; ++e) {
+                        ldc<NT>(sd.a0, xa[e], ua, va);
+                        ldc<NT>(sd.b0, xb[e], ub, vb);
+                        subc<NT, false>(ua, va, xa[e], A);
+                        subc<NT, false>(ub, vb, xb[e], B);
                     }
                 }
                 mma_square(acc, A, B);
