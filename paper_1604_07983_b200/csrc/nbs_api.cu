@@ -1023,11 +1023,11 @@ int nbs_stage_times(nbs_ctx* c, double* ms, long long* calls, int reset) {
         unsigned long long pf[PF_N] = {}, zero[PF_N] = {};
         cudaMemcpyFromSymbol(pf, g_cprof, sizeof(pf));
         cudaMemcpyToSymbol(g_cprof, zero, sizeof(zero));
-        static const char* names[PF_N] = {"total", "units", "wait_empty", "wait_rec", "wait_slot", "release", "flush", "epi_total", "epi_busy"};
+        static const char* names[PF_N] = {"total", "units", "wait_empty", "wait_rec", "wait_slot", "release", "multi_term_diagrams"};
         if (pf[PF_TOTAL]) {
             fprintf(stderr, "[NBS_PROF] compute-warp cycles:");
-            for (int i = 0; i < PF_EPI_TOTAL; ++i) fprintf(stderr, " %s %.2f%%", names[i], 100.0 * (double)pf[i] / (double)pf[PF_TOTAL]);
-            fprintf(stderr, "; epilogue warps busy %.1f%%\n", 100.0 * (double)pf[PF_EPI_BUSY] / (double)pf[PF_EPI_TOTAL]);
+            for (int i = 0; i < PF_N; ++i) fprintf(stderr, " %s %.2f%%", names[i], 100.0 * (double)pf[i] / (double)pf[PF_TOTAL]);
+            fprintf(stderr, "\n");
         }
     }
 #endif

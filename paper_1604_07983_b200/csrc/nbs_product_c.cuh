@@ -90,9 +90,10 @@ __device__ __forceinline__ void subc(const double2 (&u)[NP], const double2 (&v)[
 }
 __device__ __forceinline__ uint32_t ldw(const uint32_t* p) { return __ldg(p); }
 
-// -DNBS_PROF: cycle counters of the compute warps, summed over the launch (read by nbs_stage_times, printed to stderr)
+// -DNBS_PROF: cycle counters of the compute warps, summed over the launch (read by nbs_stage_times, printed to stderr).
+// The epilogue warps carry none: clock reads around combine_item slowed the launch from 63 to 97 ms.
 #ifdef NBS_PROF
-enum { PF_TOTAL, PF_UNITS, PF_EMPTY, PF_REC, PF_SLOT, PF_RELEASE, PF_FLUSH, PF_EPI_TOTAL, PF_EPI_BUSY, PF_N };
+enum { PF_TOTAL, PF_UNITS, PF_EMPTY, PF_REC, PF_SLOT, PF_RELEASE, PF_MULTI, PF_N };
 __device__ unsigned long long g_cprof[PF_N];
 #define PF_T(var) const long long var = clock64()
 #define PF_ADD(idx, t0) pf[idx] += clock64() - (t0)
@@ -153,7 +154,11 @@ __device__ __forceinline__ void wide_fold_B_c(const double2 (&ub)[2][1], const d
 }
 
 __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3Rec* diags, const uint32_t* __restrict__ tab,
-                                                  const char* smem, const int* item, double2* __restrict__ out, int lane) {
+                                                  const char* smem, const int* item, double2* __restrict__ out, int lane
+#ifdef NBS_PROF
+                                                  , long long* pf
+#endif
+                                                  ) {
     const CSides sd = make_sides(smem, item, lane);
     const int r = lane >> 2, kk = lane & 3, c = r >> 1;
     constexpr int NT = 2;
@@ -207,6 +212,7 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
             }
             if (s < nsteps) kstep(A0, B0, A1, B1);
         } else {
+            PF_T(t_nw);
             const int nw = dr.nwA; // == nwB (4 or 12 term pairs per entry): 16-byte groups of four words
             const uint4* tA = reinterpret_cast<const uint4*>(tab + dr.offA + ((dr.sbeg * 4 + kk) * 4 + c) * nw);
             const uint4* tB = reinterpret_cast<const uint4*>(tab + dr.offB + ((dr.sbeg * 4 + kk) * 4 + c) * nw);
@@ -227,6 +233,7 @@ __device__ __forceinline__ void run_unit_square_c(const Unit3Rec u, const Diag3R
                 }
                 mma_square(acc, A, B);
             }
+            PF_ADD(PF_MULTI, t_nw); // time in diagrams with 4 or 12 term pairs per entry (K = 9, 1)
         }
     }
 #pragma unroll
@@ -365,25 +372,15 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
     if (tid >= C_CTHREADS) {
         // ---------------- epilogue warps: combine item i while the compute warps run the following items
         const int et = tid - C_CTHREADS;
-#ifdef NBS_PROF
-        long long pf[PF_N] = {};
-        const long long pf_start = clock64();
-#endif
         for (unsigned it = 0;; ++it) {
             const int b = it % PROD_NBUF;
             mbar_wait(&ctlp->full[b], (it / PROD_NBUF) & 1u);
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
-            PF_T(t_c);
             combine_item<false>(a.base, ip, q, false, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
-            PF_ADD(PF_EPI_BUSY, t_c);
             if (et == 0) mbar_arrive(&ctlp->empty[b]); // combine_item ends with a barrier of the epilogue threads
         }
-#ifdef NBS_PROF
-        pf[PF_EPI_TOTAL] = clock64() - pf_start;
-        if ((et & 31) == 0) { atomicAdd(&g_cprof[PF_EPI_TOTAL], (unsigned long long)pf[PF_EPI_TOTAL]); atomicAdd(&g_cprof[PF_EPI_BUSY], (unsigned long long)pf[PF_EPI_BUSY]); }
-#endif
         return;
     }
 
@@ -439,7 +436,11 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
                 if (i + C_CWARPS < nunits) prefetch_unit_c(s_units + i + C_CWARPS, s_diags, a.tab, lane);
                 double2* out = scr + (size_t)u.slot * 256;
                 PF_T(t_u);
+#ifdef NBS_PROF
+                if (u.cls < 2) run_unit_square_c(u, s_diags, a.tab, smem, item, out, lane, pf);
+#else
                 if (u.cls < 2) run_unit_square_c(u, s_diags, a.tab, smem, item, out, lane);
+#endif
                 else run_unit_wide_c(u, s_diags, a.tab, smem, item, out, lane);
                 PF_ADD(PF_UNITS, t_u);
                 i = grab();
@@ -501,7 +502,7 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
 #ifdef NBS_PROF
     pf[PF_TOTAL] = clock64() - pf_start;
     if (lane == 0)
-        for (int i = 0; i < PF_EPI_TOTAL; ++i) atomicAdd(&g_cprof[i], (unsigned long long)pf[i]);
+        for (int i = 0; i < PF_N; ++i) atomicAdd(&g_cprof[i], (unsigned long long)pf[i]);
 #endif
     // no work left: tell the epilogue warps (every warp arrives; lane 0 of each writes the same end marker)
     {
