@@ -255,6 +255,18 @@ int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);
  * 8*8*4*2 = 512, a DFMA 64, a DADD 32 per warp instruction); *ms = duration of the timed launch.  Either may be NULL.
  */
 int nbs_probe_fp64(nbs_ctx* ctx, int mode, int iters, double* tflops, double* ms);
+
+/*
+ * nbs_probe_kstep -- the unit code of the pipelined product kernel in isolation (eqs. 4.2-4.3):
+ * `warps` warps per SM (1..12; one CTA per SM, 4 sub-partitions) each run the kernel's own device function for the
+ * 16x16 accumulator class (cls = 0) or the 64x4 class (cls = 2) `reps` times on a synthetic unit of one diagram with
+ * `nsteps` k-steps (1..48): two compact blocks in shared memory, packed gather words read from L2 (another table
+ * region every repetition) with the bank-conflict-free offsets the real tables have.  Synchronous.
+ * *cycles_per_kstep = SM cycles per k-step of one warp, averaged over all warps (unit prologue and the flush of the
+ * 256 results included); divide by warps / 4 for the time a sub-partition needs per k-step and compare with the
+ * FP64-pipe time of a k-step from nbs_probe_fp64 (238 / 341 cycles).  *cycles_max = the slowest warp.  Either may be NULL.
+ */
+int nbs_probe_kstep(nbs_ctx* ctx, int cls, int warps, int nsteps, int reps, double* cycles_per_kstep, double* cycles_max);
 int nbs_fft3d(nbs_ctx* ctx, void* data_dev, size_t R, int inverse, void* stream);
 long long nbs_kernel_launches(const nbs_ctx* ctx);
 

@@ -1094,6 +1094,50 @@ int nbs_fft3d(nbs_ctx* c, void* data_dev, size_t R, int inverse, void* stream) {
     return fft3d(c, (double2*)data_dev, R, inverse != 0, (cudaStream_t)stream);
 }
 
+int nbs_probe_kstep(nbs_ctx* c, int cls, int warps, int nsteps, int reps, double* cycles_per_kstep, double* cycles_max) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    if ((cls != 0 && cls != 2) || warps < 1 || warps > C_THREADS / 32 || nsteps < 1 || nsteps > PROBE_KSTEP_MAX_STEPS || reps < 1)
+        return fail(c, NBS_EINVAL, "nbs_probe_kstep: cls 0 or 2, 1 <= warps <= 12, 1 <= nsteps <= 48, reps >= 1");
+    CU(c, cudaSetDevice(c->device));
+    // packed gather words whose four consecutive k fall into four different bank groups modulo 4 (what the real
+    // tables guarantee): offset = 16 * (4 * random + k mod 4); k = (word / 4) mod 4, or (word / 16) mod 4 in the
+    // A table of the 64 x 4 class ([k][cX & 3][g])
+    std::vector<uint32_t> tab(PROBE_KSTEP_TAB_WORDS);
+    uint32_t rng = 12345u;
+    auto next = [&] { rng = rng * 1664525u + 1013904223u; return (rng >> 10) % 200u; };
+    for (size_t i = 0; i < tab.size(); ++i) {
+        const uint32_t k = (cls >= 2 && i < 65536) ? (uint32_t)((i / 16) % 4) : (uint32_t)((i / 4) % 4);
+        tab[i] = ((next() * 4 + k) * 16u) | (((next() * 4 + k) * 16u) << 16);
+    }
+    const int grid = c->prod_grid, nw = C_THREADS / 32;
+    uint32_t* d_tab = nullptr; double2* d_out = nullptr; long long* d_cyc = nullptr;
+    CU(c, cudaMalloc((void**)&d_tab, tab.size() * sizeof(uint32_t)));
+    CU(c, cudaMalloc((void**)&d_out, (size_t)grid * nw * 256 * sizeof(double2)));
+    CU(c, cudaMalloc((void**)&d_cyc, (size_t)grid * nw * sizeof(long long)));
+    cudaError_t e = cudaMemcpy(d_tab, tab.data(), tab.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(d_cyc, 0, (size_t)grid * nw * sizeof(long long));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_probe_kstep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C_BLOCKS_BYTES);
+    std::vector<long long> cyc((size_t)grid * nw, 0);
+    if (e == cudaSuccess) {
+        k_probe_kstep<<<grid, C_THREADS, C_BLOCKS_BYTES>>>(d_tab, cls, nsteps, reps, warps, d_out, d_cyc);
+        e = cudaDeviceSynchronize();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(cyc.data(), d_cyc, cyc.size() * sizeof(long long), cudaMemcpyDeviceToHost);
+    cudaFree(d_tab); cudaFree(d_out); cudaFree(d_cyc);
+    if (e != cudaSuccess) return cuda_fail(c, e, "nbs_probe_kstep");
+    ++c->launches;
+    double sum = 0.0, mx = 0.0;
+    for (int b = 0; b < grid; ++b)
+        for (int w = 0; w < warps; ++w) {
+            const double v = (double)cyc[(size_t)b * nw + w] / ((double)reps * nsteps);
+            sum += v; mx = std::max(mx, v);
+        }
+    if (cycles_per_kstep) *cycles_per_kstep = sum / ((double)grid * warps);
+    if (cycles_max) *cycles_max = mx;
+    return NBS_OK;
+}
+
 long long nbs_kernel_launches(const nbs_ctx* c) { return c ? c->launches : 0; }
 
 int nbs_pair_order(const nbs_ctx* c, int* ch_begin, int* ch_end, int cap) {

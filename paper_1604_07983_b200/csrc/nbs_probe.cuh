@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 
 #include "nbs_product.cuh"
+#include "nbs_product_c.cuh"
 
 namespace nbs {
 
@@ -110,5 +111,51 @@ __global__ void __launch_bounds__(PROBE_THREADS, 1) k_probe_fp64(int iters, doub
     for (int i = 0; i < 8; ++i) s += (double)iw[i];
     if (s == 1.2345e-300) sink[blockIdx.x * PROBE_THREADS + threadIdx.x] = s; // keeps the arithmetic alive
 }
+
+// k-step probe (nbs_probe_kstep, include/nbs.h): the unit code of k_product_c in isolation.  Every one of `ncw`
+// warps per CTA (one CTA per SM) runs the SAME device functions the kernel runs -- run_unit_square_c (cls 0) or
+// run_unit_wide_c (cls 2) -- `reps` times on a synthetic unit of one diagram with `nsteps` k-steps: two compact blocks
+// in shared memory, packed gather words from L2 with bank-conflict-free offsets (the residue rule of
+// nbs_tables.hpp), another table region every repetition.  cyc[CTA * 12 + warp] = cycles of the warp's loop.
+__global__ void __launch_bounds__(C_THREADS, 1) k_probe_kstep(const uint32_t* __restrict__ tab, int cls, int nsteps, int reps,
+                                                              int ncw, double2* __restrict__ out, long long* __restrict__ cyc) {
+    extern __shared__ __align__(128) char prod_smem[];
+    char* sm = prod_smem;
+    __shared__ int item[12];
+    __shared__ __align__(16) Diag3Rec drec[C_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (uint32_t i = tid; i < C_BLOCKS_BYTES / 16; i += blockDim.x)
+        reinterpret_cast<double2*>(sm)[i] = make_double2(1e-3 * (double)(i % 97), -2e-3 * (double)(i % 89));
+    if (tid == 0) { // B~1 in slot 0, B~2 in slot 1, both compact
+        item[5] = (int)c_slot_base(0); item[6] = (int)c_slot_base(1);
+        item[7] = item[8] = AS_PLANE * 16;
+    }
+    __syncthreads();
+    if (warp >= ncw) return;
+    Unit3Rec u;
+    u.diag_begin = warp; u.diag_end = warp + 1; u.cls = cls; u.slot = 0;
+    double2* o = out + ((size_t)blockIdx.x * (C_THREADS / 32) + warp) * 256;
+    const long long t0 = clock64();
+    for (int r = 0; r < reps; ++r) {
+        if (lane == 0) {
+            Diag3Rec d;
+            d.offA = (uint32_t)(((r * (C_THREADS / 32) + warp) % 16) * 4096); d.offB = 65536u + d.offA;
+            d.sbeg = 0; d.send = (uint16_t)nsteps; d.nwA = 1; d.nwB = (uint8_t)(cls >= 2 ? 4 : 1); d.K = (uint16_t)(4 * nsteps);
+            drec[warp] = d;
+        }
+        __syncwarp();
+#ifdef NBS_PROF
+        long long pf[PF_N] = {};
+        if (cls < 2) run_unit_square_c(u, drec, tab, sm, item, o, lane, pf);
+#else
+        if (cls < 2) run_unit_square_c(u, drec, tab, sm, item, o, lane);
+#endif
+        else run_unit_wide_c(u, drec, tab, sm, item, o, lane);
+        __syncwarp();
+    }
+    if (lane == 0) cyc[blockIdx.x * (C_THREADS / 32) + warp] = clock64() - t0;
+}
+constexpr int PROBE_KSTEP_MAX_STEPS = 48;        // a table region holds 4096 words = 64 k-steps of the widest table
+constexpr size_t PROBE_KSTEP_TAB_WORDS = 1 << 17; // A tables in the first half, B tables in the second
 
 } // namespace nbs

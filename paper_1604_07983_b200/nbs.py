@@ -28,7 +28,7 @@ EXPORTS = ["nbs_create", "nbs_load_propagators", "nbs_correlator", "nbs_destroy"
            "nbs_workspace_bytes", "nbs_num_channels", "nbs_channel_info", "nbs_std_channels",
            "nbs_diagram_stats", "nbs_blocks_x", "nbs_model_flops", "nbs_exec_flops", "nbs_fft3d",
            "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_set_pipelined", "nbs_num_slots",
-           "nbs_probe_fp64", "nbs_tiled_info", "nbs_pair_order", "nbs_plan_selfcheck"]
+           "nbs_probe_fp64", "nbs_probe_kstep", "nbs_tiled_info", "nbs_pair_order", "nbs_plan_selfcheck"]
 
 
 class nbs_channel(ctypes.Structure):
@@ -78,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.nbs_pair_order.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), c_int]
         L.nbs_tiled_info.argtypes = [c_void_p, POINTER(c_int), POINTER(c_longlong)]
         L.nbs_probe_fp64.argtypes = [c_void_p, c_int, c_int, POINTER(c_double), POINTER(c_double)]
+        L.nbs_probe_kstep.argtypes = [c_void_p, c_int, c_int, c_int, c_int, POINTER(c_double), POINTER(c_double)]
         L.nbs_kernel_launches.restype = c_longlong
         _lib = L
     return _lib
@@ -274,6 +275,12 @@ class Nbs:
 
     def num_slots(self) -> int:
         return _check(self.ctx, lib().nbs_num_slots(self.ctx))
+
+    def probe_kstep(self, cls: int, warps: int, nsteps: int = 18, reps: int = 200) -> dict:
+        """nbs_probe_kstep: {cycles, cycles_max, per_subpartition} per k-step of the product kernel's unit code in isolation."""
+        avg, mx = c_double(), c_double()
+        _check(self.ctx, lib().nbs_probe_kstep(self.ctx, cls, warps, nsteps, reps, byref(avg), byref(mx)))
+        return dict(cycles=avg.value, cycles_max=mx.value, per_subpartition=avg.value / (warps / 4.0))
 
     def probe_fp64(self, mode: int, iters: int = 20000) -> dict:
         """nbs_probe_fp64: {tflops, ms} of a register-resident FP64 instruction mix (see include/nbs.h)."""

@@ -666,6 +666,20 @@ def test_fp64_probe(torch_cuda, nbs):
             ctx.probe_fp64(9, 10)
 
 
+def test_kstep_probe(torch_cuda, nbs):
+    """nbs_probe_kstep: the unit code of the pipelined kernel in isolation runs for both accumulator classes and its
+    time per k-step lies between the FP64-pipe bound (238 / 341 cycles per sub-partition) and a loose ceiling."""
+    with nbs.Nbs(2, 1, [("p", "n", "p", "n")]) as ctx:
+        for cls, floor in ((0, 238.0), (2, 341.0)):
+            r = ctx.probe_kstep(cls, 8, nsteps=18, reps=50)
+            assert 0.9 * floor < r["per_subpartition"] < 6 * floor, (cls, r)
+            assert r["cycles_max"] >= r["cycles"]
+        with pytest.raises(nbs.NbsError):
+            ctx.probe_kstep(1, 8)
+        with pytest.raises(nbs.NbsError):
+            ctx.probe_kstep(0, 13)
+
+
 # ------------------------------------------------------------------------------ tile-wise plan (configs[4], g1)
 @pytest.mark.parametrize("L", [4, 6])
 def test_tilewise_plan_equals_resident_plan_and_oracle(torch_cuda, nbs, oracle, L):
