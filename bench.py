@@ -35,7 +35,7 @@ UNIT = "time-slices/s"
 # Cross-check only: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz.  The roofline denominator is
 # MEASURED in this process by nbs_probe_fp64 (register-resident DMMA.8x8x4 on all SMs, include/nbs.h).
 FP64_PEAK_DERIVED_TFLOPS = 37.2
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_product launch on configs[2], parsed from the committed
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_product_c launch on configs[2], parsed from the committed
 # `ncu --set full` capture of the benched kernel (the .md beside it names the command and the commit)
 PRODUCT_NCU_CSV = os.path.join(ROOT, "profiles", "r2_product_ncu.csv")
 
@@ -345,7 +345,8 @@ def main():
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload, "channels": nch, "lattice": [L, L, L, T],
                    "l2_policy": "inputs (%.0f MB per slice) and intermediates (%.1f GB per slice) exceed the 126 MB L2"
-                                % (len({id(v) for v in host[0].values()}) * V * 144 * 16 / 1e6, V * 1.4e6 / 1e9),
+                                % (len({id(v) for v in host[0].values()}) * V * 144 * 16 / 1e6,
+                                   ctx.workspace_bytes() / max(ctx.num_slots(), 1) / 1e9),
                    "parallelism": "replicas only (T-parallel), no collective" if world > 1 else "1 GPU",
                    "plan": ("tile-wise: %d chunk buffers, %.1f chunk builds per slice, %d channel ranges per slice"
                             % (tiled["chunk_slots"], builds / K, len(ranges))) if tiled["tiled"] else "resident",
