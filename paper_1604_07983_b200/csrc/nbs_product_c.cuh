@@ -16,14 +16,19 @@
 //     to two items ahead of the slowest one, so the tail of a small sink pair is filled with units of the next.
 #pragma once
 #include "nbs_product.cuh"
+#include "nbs_epilogue_c.cuh"
 
 namespace nbs {
 
 // Warp split: 10 compute + 2 epilogue warps, as in k_product_t.  Measured alternatives (profiles/r2_summary.md):
 // 8 compute warps run within 2 % of 10 (the arithmetic nearly saturates at two warps per SM sub-partition); four
-// epilogue warps with a pipelined row reader remove the epilogue's own floor (49 ms per launch, latency-bound) but
-// take issue slots and shared-memory bandwidth from the compute warps of every sub-partition (67 against 63.6 ms).
+// epilogue warps take issue slots and shared-memory bandwidth from the compute warps of every sub-partition (67
+// against 63.6 ms); 13 warps leave 128 registers per thread (four warps on one sub-partition) and spill.
+// The epilogue reads the unit rows with a pipelined reader (nbs_epilogue_c.cuh), C_EPI_ROWS rows per batch: the compute
+// warps wait 0.3 % of their time for a free ring buffer (combine_item: 0.7 %), 62.0 against 62.5 ms, and the kernel
+// needs 152 instead of 168 registers.
 constexpr int C_CWARPS = PROD_CWARPS, C_EWARPS = PROD_EWARPS;
+constexpr int C_EPI_ROWS = 3;
 constexpr int C_CTHREADS = C_CWARPS * 32, C_ETHREADS = C_EWARPS * 32, C_THREADS = C_CTHREADS + C_ETHREADS;
 
 struct CProdArgs {
@@ -378,7 +383,7 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
-            combine_item<false>(a.base, ip, q, false, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
+            combine_item_c<C_ETHREADS, C_EPI_ROWS>(a.base, ip, q, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
             if (et == 0) mbar_arrive(&ctlp->empty[b]); // combine_item ends with a barrier of the epilogue threads
         }
         return;
