@@ -188,6 +188,27 @@ int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long lo
  *             (256 * sum_d K_d over the channels' diagrams), as doubles.
  */
 int nbs_blocks_x(nbs_ctx* ctx, int t, int baryon, void* out_dev, size_t out_bytes, void* stream);
+
+/*
+ * nbs_blocks_x_static -- nbs_blocks_x (eq. 4.1) for callers that must not allocate device memory
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, same
+ * kernels, same result bit for bit; the only difference is where the staged block rows live between the block kernel
+ * and the layout kernel: nbs_blocks_x takes them from the stream-ordered allocator (cudaMallocAsync / cudaFreeAsync),
+ * this entry point uses a scratch array that is part of the library image (`static __device__`,
+ * NBS_STATIC_SCRATCH_BYTES, resident on every GPU that loads the library until the process exits).  It calls no
+ * cudaMalloc, cudaFree or allocating library routine; the first call on a device looks the array's device address up
+ * once (cudaGetSymbolAddress, no allocation).
+ *   Limit: L^3 * E * 16 <= NBS_STATIC_SCRATCH_BYTES (32 MiB) with E = 3472 staged entries per site for p, n, Sigma+-,
+ *   Xi0- (antisymmetric blocks, compact rows) and 6960 for the others: L <= 8 resp. L <= 6.  Beyond it: NBS_EINVAL,
+ *   with the bytes needed and the maximum in nbs_last_error; nothing is launched.
+ *   Sharing: all calls on a device, from every context and stream, use the SAME array.  Calls ordered on one stream
+ *   are safe; calls that may overlap on the GPU (different streams without an event between them, different host
+ *   threads) race on it -- the caller serialises them.  Nothing in the array has to start at zero: the block kernel
+ *   writes every staged entry the layout kernel reads, so the previous call's contents are never seen.
+ * Errors as nbs_blocks_x, plus the limit above.
+ */
+#define NBS_STATIC_SCRATCH_BYTES (32u << 20)
+int nbs_blocks_x_static(nbs_ctx* ctx, int t, int baryon, void* out_dev, size_t out_bytes, void* stream);
 int nbs_model_flops(const nbs_ctx* ctx, double* blocks, double* fft, double* product);
 
 /*

@@ -2,8 +2,10 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -848,6 +850,66 @@ int nbs_blocks_x(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes,
     }
     CU(c, cudaFreeAsync(tmp, st));
     if (rc) return rc;
+    return slot_release(c, sl, st);
+}
+
+// ---- nbs_blocks_x without allocation (include/nbs.h, nbs_blocks_x_static) ----------------------------------------
+// Staged block rows of one baryon between k_blocks and k_unstage, in the library image: every GPU that loads the
+// library holds these NBS_STATIC_SCRATCH_BYTES until the process exits; all calls on a device share them.
+static __device__ __align__(256) unsigned char g_static_scratch[NBS_STATIC_SCRATCH_BYTES];
+
+namespace {
+// In host code `g_static_scratch` names a host-side stand-in, not device memory: the kernels get the address that
+// cudaGetSymbolAddress reports for the current device, looked up once per device and kept here.
+constexpr int STATIC_SCRATCH_MAX_DEVICES = 64;
+std::mutex g_static_scratch_mutex;
+void* g_static_scratch_addr[STATIC_SCRATCH_MAX_DEVICES] = {};
+
+int static_scratch_addr(nbs_ctx* c, double2** out) { // device c->device is current
+    if (c->device < 0 || c->device >= STATIC_SCRATCH_MAX_DEVICES) return fail(c, NBS_EINVAL, "device ordinal beyond the static scratch table");
+    std::lock_guard<std::mutex> lock(g_static_scratch_mutex);
+    void*& p = g_static_scratch_addr[c->device];
+    if (!p) {
+        void* q = nullptr;
+        CU(c, cudaGetSymbolAddress(&q, g_static_scratch));
+        if (!q || (reinterpret_cast<uintptr_t>(q) & 255u)) return fail(c, NBS_ECUDA, "static scratch array has no aligned device address");
+        p = q;
+    }
+    *out = static_cast<double2*>(p);
+    return NBS_OK;
+}
+} // namespace
+
+int nbs_blocks_x_static(nbs_ctx* c, int t, int baryon, void* out_dev, size_t out_bytes, void* stream) {
+    if (!c) return NBS_EINVAL;
+    if (c->cuda_failed) return NBS_ECUDA;
+    if (baryon < 0 || baryon >= NBS_NUM_BARYONS || !out_dev) return fail(c, NBS_EINVAL, "bad baryon id or NULL output");
+    if (t < 0 || t >= c->T) return fail(c, NBS_EINVAL, "bad slice index");
+    Slice& sl = c->slice[t % c->nslices];
+    if (sl.t != t) return fail(c, NBS_ESTATE, "time slice not loaded");
+    if (out_bytes < c->V * BLOCK_ELEMS * sizeof(double2)) return fail(c, NBS_EINVAL, "output buffer too small");
+    const int kind = block_kind(baryon);
+    const size_t need = c->V * (size_t)block_elems(kind) * sizeof(double2);
+    if (need > (size_t)NBS_STATIC_SCRATCH_BYTES)
+        return fail(c, NBS_EINVAL, "nbs_blocks_x_static: the staged block rows of this baryon need " + std::to_string(need) +
+                                       " bytes of scratch, the static scratch array holds " +
+                                       std::to_string((size_t)NBS_STATIC_SCRATCH_BYTES) + " (NBS_STATIC_SCRATCH_BYTES); use nbs_blocks_x");
+    CU(c, cudaSetDevice(c->device));
+    double2* tmp = nullptr;
+    int rc = static_scratch_addr(c, &tmp);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = slot_acquire(c, sl, st);
+    if (rc) return rc;
+    // k_blocks writes every staged entry k_unstage reads (zero pads of the compact rows included): nothing of the
+    // previous call's contents survives into this call's output, and nothing has to be cleared
+    rc = launch_blocks(c, sl, c->d_one_baryon + baryon, c->d_one_slot_info + baryon, 1, c->dq_mask_of[baryon], tmp,
+                       (size_t)block_elems(kind), st);
+    if (rc) return rc;
+    const size_t n = c->V * (size_t)BLOCK_ELEMS;
+    k_unstage<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(tmp, c->V, kind, (double2*)out_dev);
+    ++c->launches;
+    CU(c, cudaGetLastError());
     return slot_release(c, sl, st);
 }
 

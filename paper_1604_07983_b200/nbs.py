@@ -18,6 +18,7 @@ NBS_P, NBS_N, NBS_LAMBDA, NBS_SIGMA_P, NBS_SIGMA_0, NBS_SIGMA_M, NBS_XI_0, NBS_X
 NBS_XU, NBS_XD, NBS_XS = 8, 9, 10
 NBS_OK, NBS_EINVAL, NBS_ENOMEM, NBS_ESTATE, NBS_ECUDA = 0, -1, -2, -3, -4
 NBS_MEM_DEVICE, NBS_MEM_HOST = 0, 1
+STATIC_SCRATCH_BYTES = 32 << 20  # NBS_STATIC_SCRATCH_BYTES (include/nbs.h)
 
 # short names used by the tests and the oracle's channel tuples
 BARYON_ID = {"p": NBS_P, "n": NBS_N, "L": NBS_LAMBDA, "Sp": NBS_SIGMA_P, "S0": NBS_SIGMA_0, "Sm": NBS_SIGMA_M,
@@ -28,7 +29,8 @@ EXPORTS = ["nbs_create", "nbs_load_propagators", "nbs_correlator", "nbs_destroy"
            "nbs_workspace_bytes", "nbs_num_channels", "nbs_channel_info", "nbs_std_channels",
            "nbs_diagram_stats", "nbs_blocks_x", "nbs_model_flops", "nbs_exec_flops", "nbs_fft3d",
            "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_set_pipelined", "nbs_num_slots",
-           "nbs_probe_fp64", "nbs_probe_kstep", "nbs_tiled_info", "nbs_pair_order", "nbs_plan_selfcheck"]
+           "nbs_probe_fp64", "nbs_probe_kstep", "nbs_tiled_info", "nbs_pair_order", "nbs_plan_selfcheck",
+           "nbs_blocks_x_static"]
 
 
 class nbs_channel(ctypes.Structure):
@@ -65,6 +67,7 @@ def lib() -> ctypes.CDLL:
         L.nbs_diagram_stats.argtypes = [POINTER(nbs_channel), POINTER(c_int), POINTER(c_int), c_int,
                                         POINTER(c_longlong)]
         L.nbs_blocks_x.argtypes = [c_void_p, c_int, c_int, c_void_p, c_size_t, c_void_p]
+        L.nbs_blocks_x_static.argtypes = [c_void_p, c_int, c_int, c_void_p, c_size_t, c_void_p]
         L.nbs_model_flops.argtypes = [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double)]
         L.nbs_exec_flops.argtypes = [c_void_p, POINTER(c_double)]
         L.nbs_fft3d.argtypes = [c_void_p, c_void_p, c_size_t, c_int, c_void_p]
@@ -222,6 +225,15 @@ class Nbs:
         b = BARYON_ID[baryon] if isinstance(baryon, str) else int(baryon)
         out = torch.empty((self.V, 4, 12, 12, 12), dtype=torch.complex128, device=f"cuda:{self.device}")
         _check(self.ctx, lib().nbs_blocks_x(self.ctx, t, b, out.data_ptr(), out.numel() * 16, _stream_handle(stream)))
+        return out
+
+    def blocks_x_static(self, t, baryon, out, stream=None):
+        """nbs_blocks_x_static: eq. 4.1 into the caller's tensor `out` [V][4][12][12][12] complex128, staged rows in
+        the library's static scratch array (STATIC_SCRATCH_BYTES); no device memory is allocated."""
+        b = BARYON_ID[baryon] if isinstance(baryon, str) else int(baryon)
+        assert out.is_cuda and out.is_contiguous()
+        _check(self.ctx, lib().nbs_blocks_x_static(self.ctx, t, b, out.data_ptr(), out.numel() * out.element_size(),
+                                                   _stream_handle(stream)))
         return out
 
     def fft3d(self, data, inverse=False, stream=None):
