@@ -219,36 +219,40 @@ int launch_fft_axis(nbs_ctx* c, double2* data, size_t R, int axis, double scale,
     return NBS_OK;
 }
 
-template <int L>
-int launch_fft_xy_out(nbs_ctx* c, double2* data, size_t R, double scale, double2* tout, cudaStream_t st) {
+template <int L, bool INV, bool TOUT>
+int launch_fft_xy(nbs_ctx* c, double2* data, size_t R, size_t Rn, double scale, double2* tout, cudaStream_t st) {
     constexpr int C = fft_xy_comps<L>();
-    dim3 grid((unsigned)((R + C - 1) / C), (unsigned)L);
-    k_fft_xy<L, true, true><<<grid, L * C, fft_xy_smem_bytes<L>(), st>>>(data, R, scale, tout, c->V);
+    dim3 grid((unsigned)((Rn + C - 1) / C), (unsigned)L);
+    k_fft_xy<L, INV, TOUT><<<grid, L * C, fft_xy_smem_bytes<L, TOUT>(), st>>>(data, R, Rn, scale, tout, c->V);
     CU(c, cudaGetLastError());
     ++c->launches;
     return NBS_OK;
 }
-int launch_fft_xy_any(nbs_ctx* c, double2* data, size_t R, double scale, double2* tout, cudaStream_t st) {
+template <bool INV, bool TOUT>
+int launch_fft_xy_any(nbs_ctx* c, double2* data, size_t R, size_t Rn, double scale, double2* tout, cudaStream_t st) {
     switch (c->L) {
-    case 2: return launch_fft_xy_out<2>(c, data, R, scale, tout, st);
-    case 4: return launch_fft_xy_out<4>(c, data, R, scale, tout, st);
-    case 8: return launch_fft_xy_out<8>(c, data, R, scale, tout, st);
-    case 16: return launch_fft_xy_out<16>(c, data, R, scale, tout, st);
-    default: return launch_fft_xy_out<32>(c, data, R, scale, tout, st);
+    case 2: return launch_fft_xy<2, INV, TOUT>(c, data, R, Rn, scale, tout, st);
+    case 4: return launch_fft_xy<4, INV, TOUT>(c, data, R, Rn, scale, tout, st);
+    case 8: return launch_fft_xy<8, INV, TOUT>(c, data, R, Rn, scale, tout, st);
+    case 16: return launch_fft_xy<16, INV, TOUT>(c, data, R, Rn, scale, tout, st);
+    default: return launch_fft_xy<32, INV, TOUT>(c, data, R, Rn, scale, tout, st);
     }
 }
 bool fft_fused(const nbs_ctx* c) { return c->L == 2 || c->L == 4 || c->L == 8 || c->L == 16 || c->L == 32; }
 
-// 3-D transform of data[site][R].  Forward: three per-axis passes, each at the HBM copy rate (the
-// fused x-y kernel, one CTA per SM with 144 KB of shared memory, measured 20.8 ms against 17.7 ms
-// for the two passes it replaces at 32^3 and is not used forward).  Inverse with `tout` != NULL and
-// L a power of two <= 32: z pass, then the fused x-y kernel writes out[comp][r] directly, which
-// saves the transpose pass (8.4 -> 7.0 ms).  Other L: tout is ignored, the caller transposes.
+// 3-D transform of the first Rn components of data[site][R].  L a power of two <= 32: a z pass at the HBM copy rate,
+// then ONE pass for x and y (k_fft_xy: x-lines from HBM into registers, y-lines through shared memory); the last
+// inverse pass with `tout` != NULL writes out[comp][r] directly, which saves the transpose pass.  Other L: three
+// per-axis passes; tout is ignored and the caller transposes.
 int fft3d(nbs_ctx* c, double2* data, size_t R, bool inverse, cudaStream_t st, double2* tout = nullptr, size_t Rn = 0) {
-    if (fft_fused(c) && inverse && tout) {
-        int rc = launch_fft_axis<true>(c, data, R, 2, 1.0 / (double)c->L, st);
+    if (Rn == 0) Rn = R;
+    if (fft_fused(c)) {
+        const double sz = 1.0 / (double)c->L, sxy = 1.0 / ((double)c->L * c->L);
+        int rc = inverse ? launch_fft_axis<true>(c, data, R, 2, sz, st, Rn) : launch_fft_axis<false>(c, data, R, 2, 1.0, st, Rn);
         if (rc) return rc;
-        return launch_fft_xy_any(c, data, R, 1.0 / ((double)c->L * c->L), tout, st);
+        if (!inverse) return launch_fft_xy_any<false, false>(c, data, R, Rn, 1.0, nullptr, st);
+        if (tout) return launch_fft_xy_any<true, true>(c, data, R, Rn, sxy, tout, st);
+        return launch_fft_xy_any<true, false>(c, data, R, Rn, sxy, nullptr, st);
     }
     for (int axis = 0; axis < 3; ++axis) {
         int rc = inverse ? launch_fft_axis<true>(c, data, R, axis, 1.0 / (double)c->L, st, Rn)
@@ -777,8 +781,11 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<16>()));
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<16>()));
     CUX(cudaFuncSetAttribute(k_blocks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)blocks_smem_bytes(9)));
-    CUX(cudaFuncSetAttribute(k_fft_xy<32, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_xy_smem_bytes<32>()));
-    CUX(cudaFuncSetAttribute(k_fft_xy<16, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_xy_smem_bytes<16>()));
+#define NBS_XY_ATTR(L_, INV_, TOUT_) \
+    CUX(cudaFuncSetAttribute(k_fft_xy<L_, INV_, TOUT_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_xy_smem_bytes<L_, TOUT_>()))
+    NBS_XY_ATTR(32, false, false); NBS_XY_ATTR(32, true, false); NBS_XY_ATTR(32, true, true);
+    NBS_XY_ATTR(16, false, false); NBS_XY_ATTR(16, true, false); NBS_XY_ATTR(16, true, true);
+#undef NBS_XY_ATTR
     *out = c;
     return NBS_OK;
 #undef CUC
