@@ -259,6 +259,25 @@ int nbs_set_direct(nbs_ctx* ctx, int enable);
  * plan); the tile-wise plan and the direct shifted sum always run k_product_t.  Takes effect at the next nbs_correlator.
  */
 int nbs_set_pipelined(nbs_ctx* ctx, int enable);
+
+/*
+ * nbs_set_channel_relations -- isospin limit (the caller passed the same array for u and d): besides
+ * deriving the blocks of n, Sigma-, Xi- from those of p, Sigma+, Xi0, the library then leaves out every channel of the
+ * list that is the u <-> d image of an earlier one and writes it from that one in the epilogue of the product kernel:
+ *   <B1 B2 | B3 B4> = eta1 eta2 eta3 eta4 <B1' B2' | B3' B4'>,  <.. | B4' B3'>_{a3 a4} = - <.. | B3' B4'>_{a4 a3},
+ * with p <-> n, Sigma+ <-> Sigma-, Xi0 <-> Xi-, X_u <-> X_d (eta = -1 for Lambda, Xi0, Xi-, X_u, X_d, X_s; eqs. 2.2-2.3).
+ * In the standard list these are nine channels (n Xi0 -> anything: all six; Lambda Lambda -> n Xi0, Sigma0 Sigma0 ->
+ * n Xi0, Sigma0 Lambda -> n Xi0), so the sink pair n Xi0 is not contracted at all.  Results equal the full computation
+ * up to rounding.  Resident plan with the pipelined product kernel only.
+ *   enable != 0 (default): use the relations;  enable == 0: compute every channel;
+ *   enable < 0: query -- returns the number of channels that are derived this way (0: none / not available / off).
+ */
+int nbs_set_channel_relations(nbs_ctx* ctx, int enable);
+/*   nbs_iso_relations: the relations themselves, on the host only (no CUDA call): for channel i of the list (ch == NULL:
+ *             the standard 52) from[i] = -1 if it is computed, else F[i] = sign[i] * F[from[i]] with a3 <-> a4 exchanged
+ *             if swap34[i]; from[i] < i and channel from[i] is computed.  Writes at most `cap` entries (any array may be
+ *             NULL), returns the number of channels, NBS_EINVAL for an invalid baryon id. */
+int nbs_iso_relations(const nbs_channel* ch, int nch, int* from, int* sign, int* swap34, int cap);
 int nbs_stage_times(nbs_ctx* ctx, double* ms, long long* calls, int reset);
 
 int nbs_exec_flops(const nbs_ctx* ctx, double* product_executed);

@@ -74,6 +74,26 @@ struct nbs_ctx {
     double* d_pair_sign_iso = nullptr;
     uint32_t c_rec_stride = 0, c_units_bytes = 0;
     size_t c_smem = 0;
+    // Isospin limit (d == u), channel relations (nbs_tables.hpp, IsoRelation): a second plan over the channels that are
+    // not the u <-> d image of an earlier one; the epilogue writes the images from their originals.  Block rows, FFT
+    // and workspace are those of the full plan: only the product stage changes tables.
+    struct IsoChannels {
+        bool ok = false;
+        Plan plan;
+        int nderived = 0;
+        Pair3Rec* d_pairs3 = nullptr;
+        PairChanRec* d_pair_chans = nullptr;
+        Unit3Rec* d_units3 = nullptr;
+        Diag3Rec* d_diagsc = nullptr;
+        uint32_t* d_tabc = nullptr;
+        CItem* d_cprog = nullptr;
+        CLoad* d_cloads = nullptr;
+        int* d_slot_off = nullptr;
+        double* d_pair_sign = nullptr;
+        uint32_t rec_stride = 0, units_bytes = 0;
+        size_t smem = 0;
+    } isoch;
+    bool iso_relations = true; // nbs_set_channel_relations
     bool direct = false; // nbs_set_direct: eq. 2.4 as a shifted sum in x-space (tiny lattices)
     // Tile-wise plan (BASELINE.json configs[4], 96^3): chosen by nbs_create when the resident
     // workspace does not fit.  A chunk = two sink-spin planes of one baryon for all momenta, [V][2 * SM_PLANE],
@@ -430,6 +450,20 @@ int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long lo
     return (int)d.size();
 }
 
+int nbs_iso_relations(const nbs_channel* ch, int nch, int* from, int* sign, int* swap34, int cap) {
+    std::vector<nbs_channel> chans = ch ? std::vector<nbs_channel>(ch, ch + nch) : standard_channels();
+    for (auto& x : chans)
+        for (int b : {x.b1, x.b2, x.b3, x.b4})
+            if (b < 0 || b >= NBS_NUM_BARYONS) return NBS_EINVAL;
+    const std::vector<IsoRelation> rel = iso_channel_relations(chans);
+    for (size_t i = 0; i < rel.size() && (int)i < cap; ++i) {
+        if (from) from[i] = rel[i].from;
+        if (sign) sign[i] = rel[i].sign;
+        if (swap34) swap34[i] = rel[i].swap34;
+    }
+    return (int)rel.size();
+}
+
 int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
     // Host-side bounds check of everything the kernels index with table data (compute-sanitizer is not available on
     // the target pool): returns 0, or the negative number of the first violated invariant.
@@ -565,6 +599,63 @@ int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
     return NBS_OK;
 }
 
+// Second plan for the isospin limit: the channels that are not the u <-> d image of an earlier channel of the list
+// (nbs_tables.hpp, iso_channel_relations).  Its tables address the block rows of the FULL plan (what k_blocks and the
+// forward FFT write when d == u: the blocks of p, Sigma+, Xi0 stand in for n, Sigma-, Xi-), its channel records
+// carry the numbers of the full list and the image each of them has to be copied to.  Not available -> isoch.ok stays
+// false and the isospin limit runs the full plan (same results).
+static int build_iso_channels(nbs_ctx* c, size_t smem_optin) {
+    const std::vector<IsoRelation> rel = iso_channel_relations(c->plan.channels);
+    std::vector<nbs_channel> red;
+    std::vector<int> orig;
+    for (size_t i = 0; i < rel.size(); ++i)
+        if (rel[i].from < 0) { red.push_back(c->plan.channels[i]); orig.push_back((int)i); }
+    nbs_ctx::IsoChannels& ic = c->isoch;
+    ic.nderived = (int)(rel.size() - red.size());
+    if (ic.nderived == 0) return NBS_OK;
+    Plan& rp = ic.plan;
+    if (!build_plan(red, rp).empty() || !rp.cprog_ok || rp.max_pair_units > c->plan.max_pair_units || rp.baryons.size() >= 256) return NBS_OK;
+    ic.units_bytes = (uint32_t)rp.max_pair_units * (uint32_t)sizeof(Unit3Rec);
+    ic.rec_stride = C_ITEM_BYTES + ic.units_bytes + (uint32_t)rp.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
+    ic.smem = cprod_smem_bytes(ic.rec_stride);
+    if (ic.smem > smem_optin) return NBS_OK;
+    for (auto& pc : rp.pair_chans) pc.ch = orig[pc.ch]; // channel numbers of the full list
+    for (size_t i = 0; i < rel.size(); ++i) {
+        if (rel[i].from < 0) continue;
+        bool found = false;
+        for (auto& pc : rp.pair_chans)
+            if (pc.ch == rel[i].from) { pc.alias_ch = (int)i; pc.alias_sign = (double)rel[i].sign; pc.alias_swap = rel[i].swap34; found = true; }
+        if (!found) return NBS_OK; // the original has no record (cannot happen for a valid channel): keep the full plan
+    }
+    // blocks are staged from the rows of the full plan: a derived baryon from its partner's block, with its sign
+    std::vector<int> off, sgn;
+    for (int b : rp.baryons) {
+        int fs = -1;
+        for (size_t s = 0; s < c->plan.baryons.size(); ++s)
+            if (c->plan.baryons[s] == b) fs = (int)s;
+        if (fs < 0) return NBS_OK;
+        off.push_back(c->plan.slot_off[c->plan.slot_partner_iso[fs]]);
+        sgn.push_back(c->plan.slot_sign_iso[fs]);
+    }
+    std::vector<double> psg;
+    for (auto& pr : rp.pairs3) psg.push_back((double)(sgn[pr.slot1] * sgn[pr.slot2]));
+    int rc;
+    if ((rc = upload(c, ic.d_pairs3, rp.pairs3)) || (rc = upload(c, ic.d_pair_chans, rp.pair_chans)) ||
+        (rc = upload(c, ic.d_units3, rp.units3)) || (rc = upload(c, ic.d_diagsc, rp.diagsc)) || (rc = upload(c, ic.d_tabc, rp.tabc)) ||
+        (rc = upload(c, ic.d_cprog, rp.cprog)) || (rc = upload(c, ic.d_cloads, rp.cloads)) || (rc = upload(c, ic.d_slot_off, off)) ||
+        (rc = upload(c, ic.d_pair_sign, psg)))
+        return rc;
+    ic.ok = true;
+    return NBS_OK;
+}
+
+int nbs_set_channel_relations(nbs_ctx* c, int enable) {
+    if (!c) return NBS_EINVAL;
+    if (enable < 0) return (c->isoch.ok && c->iso_relations) ? c->isoch.nderived : 0; // query
+    c->iso_relations = enable != 0;
+    return NBS_OK;
+}
+
 int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int device, size_t budget) {
     if (!out) return fail(nullptr, NBS_EINVAL, "out is NULL");
     *out = nullptr;
@@ -667,6 +758,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         CUC(upload(c, c->d_gather_pp[0], c->plan.gather_pp[0]));
         CUC(upload(c, c->d_gather_pp[1], c->plan.gather_pp[1]));
     }
+    size_t smem_optin = 0;
     {
         cudaDeviceProp prop;
         CUX(cudaGetDeviceProperties(&prop, device));
@@ -676,6 +768,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
             return NBS_ECUDA;
         }
         c->prod_grid = prop.multiProcessorCount;
+        smem_optin = (size_t)prop.sharedMemPerBlockOptin;
         // pipelined kernel: needs a program (Plan::cprog_ok) and room for three record buffers
         c->c_units_bytes = (uint32_t)c->plan.max_pair_units * (uint32_t)sizeof(Unit3Rec);
         c->c_rec_stride = C_ITEM_BYTES + c->c_units_bytes + (uint32_t)c->plan.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
@@ -702,6 +795,7 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         CUC(upload(c, c->d_slot_off_iso, off_iso));
         CUC(upload(c, c->d_pair_sign, sg));
         CUC(upload(c, c->d_pair_sign_iso, sg_iso));
+        CUC(build_iso_channels(c, smem_optin));
     }
     CUC(upload(c, c->d_baryon_of_slot, c->plan.baryons));
     CUC(upload(c, c->d_one_baryon, std::vector<int>(NBS_NUM_BARYONS, 0)));
@@ -775,7 +869,8 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
     }
     CUX(cudaFuncSetAttribute(k_product_t<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
     CUX(cudaFuncSetAttribute(k_product_t<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PROD_SMEM));
-    if (c->use_c) CUX(cudaFuncSetAttribute(k_product_c, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->c_smem));
+    if (c->use_c) CUX(cudaFuncSetAttribute(k_product_c<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->c_smem));
+    if (c->isoch.ok) CUX(cudaFuncSetAttribute(k_product_c<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->isoch.smem));
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<32>()));
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<32>()));
     CUX(cudaFuncSetAttribute(k_fft_axis_r3<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_r3_smem_bytes<16>()));
@@ -1007,8 +1102,20 @@ int nbs_correlator(nbs_ctx* c, int t, int ch_begin, int ch_end, void* out, size_
             ca.prog = c->d_cprog; ca.nitems = (int)c->plan.cprog.size(); ca.loads = c->d_cloads;
             ca.units = c->d_units3; ca.diags = c->d_diagsc; ca.tab = c->d_tabc;
             ca.rec_stride = c->c_rec_stride; ca.units_bytes = c->c_units_bytes;
+            size_t smem = c->c_smem;
+            const bool alias = iso && c->isoch.ok && c->iso_relations;
+            if (alias) { // channels that are u <-> d images are written from their originals
+                const nbs_ctx::IsoChannels& ic = c->isoch;
+                ca.base.pairs = ic.d_pairs3; ca.base.pair_chans = ic.d_pair_chans; ca.base.max_pair_units = ic.plan.max_pair_units;
+                ca.slot_off = ic.d_slot_off; ca.pair_sign = ic.d_pair_sign;
+                ca.prog = ic.d_cprog; ca.nitems = (int)ic.plan.cprog.size(); ca.loads = ic.d_cloads;
+                ca.units = ic.d_units3; ca.diags = ic.d_diagsc; ca.tab = ic.d_tabc;
+                ca.rec_stride = ic.rec_stride; ca.units_bytes = ic.units_bytes;
+                smem = ic.smem;
+            }
             grid = (unsigned)std::min<long long>(c->prod_grid, ca.ntasks);
-            k_product_c<<<grid, C_THREADS, c->c_smem, st>>>(ca);
+            if (alias) k_product_c<true><<<grid, C_THREADS, smem, st>>>(ca);
+            else k_product_c<false><<<grid, C_THREADS, smem, st>>>(ca);
         } else
         k_product_t<false><<<grid, PROD_THREADS, PROD_SMEM, st>>>(pa);
         CU(c, cudaGetLastError());

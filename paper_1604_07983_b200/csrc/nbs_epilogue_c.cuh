@@ -10,7 +10,7 @@
 
 namespace nbs {
 
-template <int ET, int EG>
+template <int ET, int EG, bool ALIAS>
 __device__ __forceinline__ void combine_item_c(const ProdArgs& a, int ip, size_t q, const double2* __restrict__ scr, int et,
                                                char* s_epi, double osign) {
     constexpr int NMT = 256 / ET;          // components per thread ...
@@ -118,6 +118,19 @@ __device__ __forceinline__ void combine_item_c(const ProdArgs& a, int ip, size_t
                             const double2 val = make_double2(acc[c][m].x * osign, acc[c][m].y * osign); // +-1: sign of a derived block (isospin limit)
                             __stcs(a.Ft + (q * a.nch_out + ch) * 256 + comp(m), val);
                             if (mirror) __stcs(a.Ft + (mq * a.nch_out + ch) * 256 + mirror_comp(m), make_double2(-val.x, -val.y));
+                        }
+                    }
+                    // isospin limit, reduced channel list: the u <-> d image of this channel is written from it (nbs_tables.hpp, IsoRelation)
+                    const int cha = pcs[c].alias_ch - a.ch_begin;
+                    if (ALIAS && pcs[c].alias_ch >= 0 && cha >= 0 && cha < a.nch_out) {
+                        const double asg = osign * pcs[c].alias_sign;
+                        const bool asw = pcs[c].alias_swap != 0;
+                        auto swap34 = [&](int i) { return asw ? ((i & ~15) | ((i & 3) << 2) | ((i >> 2) & 3)) : i; };
+#pragma unroll
+                        for (int m = 0; m < NM; ++m) {
+                            const double2 val = make_double2(acc[c][m].x * asg, acc[c][m].y * asg);
+                            __stcs(a.Ft + (q * a.nch_out + cha) * 256 + swap34(comp(m)), val);
+                            if (mirror) __stcs(a.Ft + (mq * a.nch_out + cha) * 256 + swap34(mirror_comp(m)), make_double2(-val.x, -val.y));
                         }
                     }
                 }

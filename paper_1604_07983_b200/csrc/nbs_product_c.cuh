@@ -313,6 +313,8 @@ __device__ __forceinline__ void prefetch_unit_c(const Unit3Rec* urec, const Diag
     prefetch_diag_c(drecs + uv.x, uv.z >= 2, tab, lane);
 }
 
+// ALIAS: the channel records carry u <-> d images to write (isospin limit with channel relations, nbs_tables.hpp)
+template <bool ALIAS>
 __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
     extern __shared__ __align__(128) char prod_smem[];
     char* smem = prod_smem;
@@ -383,7 +385,7 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
-            combine_item_c<C_ETHREADS, C_EPI_ROWS>(a.base, ip, q, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
+            combine_item_c<C_ETHREADS, C_EPI_ROWS, ALIAS>(a.base, ip, q, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
             if (et == 0) mbar_arrive(&ctlp->empty[b]); // combine_item ends with a barrier of the epilogue threads
         }
         return;

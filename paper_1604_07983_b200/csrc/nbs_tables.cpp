@@ -244,6 +244,54 @@ int diagram_K(const int* P) {
 
 const BaryonDef& baryon_def(int id) { return kBaryons[id]; }
 
+int baryon_iso_mirror(int baryon, int* eta) {
+    const BaryonDef& B = kBaryons[baryon];
+    auto flip = [](int f) { return f == U ? D : f == D ? U : f; };
+    for (int cand = 0; cand < NBS_NUM_BARYONS; ++cand) {
+        const BaryonDef& Bc = kBaryons[cand];
+        if (Bc.nterm != B.nterm) continue;
+        for (int e = +1; e >= -1; e -= 2) {
+            bool all = true;
+            for (int i = 0; i < B.nterm && all; ++i) {
+                // image of term i: coef * eps (q_f0' C g5 q_f1') q_f2'  =  -coef * eps (q_f1' C g5 q_f0') q_f2'
+                const int f0 = flip(B.term[i].f[0]), f1 = flip(B.term[i].f[1]), f2 = flip(B.term[i].f[2]);
+                bool found = false;
+                for (int j = 0; j < Bc.nterm && !found; ++j) {
+                    const ElemTerm& t = Bc.term[j];
+                    if (t.f[2] != f2) continue;
+                    if (t.f[0] == f0 && t.f[1] == f1 && std::fabs(e * t.coef - B.term[i].coef) < 1e-14) found = true;
+                    if (t.f[0] == f1 && t.f[1] == f0 && std::fabs(e * t.coef + B.term[i].coef) < 1e-14) found = true;
+                }
+                all = found;
+            }
+            if (all) { if (eta) *eta = e; return cand; }
+        }
+    }
+    return -1;
+}
+
+std::vector<IsoRelation> iso_channel_relations(const std::vector<nbs_channel>& channels) {
+    std::vector<IsoRelation> rel(channels.size(), IsoRelation{-1, 1, 0});
+    std::vector<char> has_alias(channels.size(), 0);
+    for (size_t i = 0; i < channels.size(); ++i) {
+        if (rel[i].from >= 0 || has_alias[i]) continue;
+        const nbs_channel& c = channels[i];
+        int e1, e2, e3, e4;
+        const int m1 = baryon_iso_mirror(c.b1, &e1), m2 = baryon_iso_mirror(c.b2, &e2), m3 = baryon_iso_mirror(c.b3, &e3),
+                  m4 = baryon_iso_mirror(c.b4, &e4);
+        if (m1 < 0 || m2 < 0 || m3 < 0 || m4 < 0) continue;
+        const int s = e1 * e2 * e3 * e4;
+        for (size_t j = i + 1; j < channels.size(); ++j) {
+            if (rel[j].from >= 0 || has_alias[j]) continue;
+            const nbs_channel& d = channels[j];
+            if (d.b1 != m1 || d.b2 != m2) continue;
+            if (d.b3 == m3 && d.b4 == m4) { rel[j] = IsoRelation{(int)i, s, 0}; has_alias[i] = 1; break; }
+            if (d.b3 == m4 && d.b4 == m3) { rel[j] = IsoRelation{(int)i, -s, 1}; has_alias[i] = 1; break; }
+        }
+    }
+    return rel;
+}
+
 int block_kind(int baryon) {
     const BaryonDef& B = kBaryons[baryon];
     if (B.slot[0] == B.slot[2]) return BK_ASYM13;
@@ -614,6 +662,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             if (plan.chan_pair[ic] != (int)ip) continue;
             PairChanRec pc;
             pc.ch = (int)ic; pc.local = (int)plan.pair_chans.size() - pr.chan_begin;
+            pc.alias_ch = -1; pc.alias_swap = 0; pc.alias_sign = 1.0;
             bool any = false;
             for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = pc.coefS[e] = 0.0;
             for (auto& ct : chan_ct[ic])
@@ -629,7 +678,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
         pr.nchan = (int)plan.pair_chans.size() - pr.chan_begin;
         plan.pairs3.push_back(pr);
     }
-    plan.tab3.insert(plan.tab3.end(), 1024, uint2x{0, 0}); // the kernel prefetches a few k-steps past a table's end
+    plan.tab3.insert(plan.tab3.end(), 4096, uint2x{0, 0}); // the kernel prefetches a few k-steps past a table's end (4096: also covers nbs_plan_selfcheck's class-blind bound)
     plan.tabc.insert(plan.tabc.end(), 256, 0u); // L1 prefetches run a little past a table's end
 
     // ---- chains: order of the sink pairs inside one momentum task that reloads the fewest blocks.

@@ -134,6 +134,10 @@ struct Pair3Rec {
 };
 struct PairChanRec {
     int ch, local; // channel index; position of the channel among the channels of its sink pair (row of the tile-wise plan's Ft)
+    // isospin limit, reduced channel list (IsoRelation): a second channel that the epilogue writes from this one,
+    // F[alias_ch] = alias_sign * F[ch], with the source spins a3 <-> a4 exchanged if alias_swap; alias_ch = -1: none
+    int alias_ch, alias_swap;
+    double alias_sign;
     double coef[MAX_PAIR_ELEMS];  // channel = sum_e coef[e] * E_e + coefS[e] * (E_e with a3 <-> a4), eqs. 2.2-2.3;
     double coefS[MAX_PAIR_ELEMS]; // coefS carries the minus sign of the source swap (reading A11)
 };
@@ -249,6 +253,17 @@ struct Plan {
 // Returns "" on success, else an error message (invalid id, flavour violation).
 std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps = 18,
                        int unit_cost_max = 80);
+
+// Channel relations of the isospin limit (u and d propagators identical): relabelling u <-> d maps every
+// interpolating field of eqs. 2.2-2.3 to +-1 times another one (p <-> n, Sigma+ <-> Sigma-, Xi0 <-> -Xi-, Lambda -> -Lambda,
+// Sigma0 -> Sigma0, X_u <-> -X_d, X_s -> -X_s) and leaves the path integral unchanged, so
+//   <B1 B2 | B3 B4> = eta1 eta2 eta3 eta4 <B1' B2' | B3' B4'>,   and   <.. | B4' B3'>_{a3 a4} = - <.. | B3' B4'>_{a4 a3}.
+// rel[i].from = -1: channel i is computed; else channel i = sign * channel `from` (a3 <-> a4 exchanged if swap34),
+// `from` < i and itself computed.  The signs come from the operator table (baryon_iso_mirror), not from a list.
+struct IsoRelation { int from, sign, swap34; };
+std::vector<IsoRelation> iso_channel_relations(const std::vector<nbs_channel>& channels);
+// u <-> d image of an interpolating field: returns the field id and writes eta = +-1; -1 if the image is no field of the table
+int baryon_iso_mirror(int baryon, int* eta);
 
 // Diagrams of one channel in enumeration order (source terms major, permutations lexicographic).
 std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& out);

@@ -30,7 +30,7 @@ EXPORTS = ["nbs_create", "nbs_load_propagators", "nbs_correlator", "nbs_destroy"
            "nbs_diagram_stats", "nbs_blocks_x", "nbs_model_flops", "nbs_exec_flops", "nbs_fft3d",
            "nbs_kernel_launches", "nbs_set_timing", "nbs_stage_times", "nbs_set_direct", "nbs_set_pipelined", "nbs_num_slots",
            "nbs_probe_fp64", "nbs_probe_kstep", "nbs_tiled_info", "nbs_pair_order", "nbs_plan_selfcheck",
-           "nbs_blocks_x_static"]
+           "nbs_blocks_x_static", "nbs_set_channel_relations", "nbs_iso_relations"]
 
 
 class nbs_channel(ctypes.Structure):
@@ -74,6 +74,8 @@ def lib() -> ctypes.CDLL:
         L.nbs_set_timing.argtypes = [c_void_p, c_int]
         L.nbs_set_direct.argtypes = [c_void_p, c_int]
         L.nbs_set_pipelined.argtypes = [c_void_p, c_int]
+        L.nbs_set_channel_relations.argtypes = [c_void_p, c_int]
+        L.nbs_iso_relations.argtypes = [POINTER(nbs_channel), c_int, POINTER(c_int), POINTER(c_int), POINTER(c_int), c_int]
         L.nbs_stage_times.argtypes = [c_void_p, POINTER(c_double), POINTER(c_longlong), c_int]
         L.nbs_kernel_launches.argtypes = [c_void_p]
         L.nbs_num_slots.argtypes = [c_void_p]
@@ -116,6 +118,17 @@ def nbs_plan_selfcheck(channels=None) -> int:
         return lib().nbs_plan_selfcheck(None, 0)
     arr = _as_channels(channels)
     return lib().nbs_plan_selfcheck(arr, len(channels))
+
+
+def nbs_iso_relations(channels=None) -> list:
+    """Host-only: [(from, sign, swap34)] per channel; from = -1 for a computed channel (include/nbs.h)."""
+    n = 52 if channels is None else len(channels)
+    arr = None if channels is None else _as_channels(channels)
+    fr, sg, sw = (c_int * n)(), (c_int * n)(), (c_int * n)()
+    got = lib().nbs_iso_relations(arr, 0 if channels is None else n, fr, sg, sw, n)
+    if got < 0:
+        raise NbsError(got, "invalid channel list")
+    return [(fr[i], sg[i], sw[i]) for i in range(got)]
 
 
 def nbs_diagram_stats(channel) -> dict:
@@ -262,6 +275,14 @@ class Nbs:
 
     def pipelined(self) -> bool:
         return bool(_check(self.ctx, lib().nbs_set_pipelined(self.ctx, -1)))
+
+    def set_channel_relations(self, enable: bool = True):
+        """nbs_set_channel_relations: in the isospin limit (d is u) write the u <-> d images of channels from their originals."""
+        _check(self.ctx, lib().nbs_set_channel_relations(self.ctx, 1 if enable else 0))
+
+    def derived_channels(self) -> int:
+        """Number of channels the isospin limit derives from others (0: none, not available, or switched off)."""
+        return int(_check(self.ctx, lib().nbs_set_channel_relations(self.ctx, -1)))
 
     def set_timing(self, enable: bool = True):
         _check(self.ctx, lib().nbs_set_timing(self.ctx, 1 if enable else 0))

@@ -89,3 +89,21 @@ def test_plan_tables_stay_in_bounds():
     assert nbs.nbs_plan_selfcheck([("p", "n", "p", "n")]) == 0
     assert nbs.nbs_plan_selfcheck([("L", "L", "L", "L"), ("S0", "S0", "Sp", "Sm"), ("p", "L", "p", "Xu"), ("Xu", "Xs", "Xd", "Xs")]) == 0
     assert nbs.nbs_plan_selfcheck([("p", "p", "p", "p"), ("n", "n", "n", "n"), ("p", "n", "p", "n")] * 40) == 0
+
+
+def test_isospin_channel_relations_of_the_standard_list():
+    """include/nbs.h nbs_iso_relations: the u <-> d images in the standard list are the nine relations the oracle pins
+    (tests/test_oracle_pins.py::test_isospin_relations_u_equals_d), with their signs, found from the operator table;
+    the reduced list passes the table self-check."""
+    rel = nbs.nbs_iso_relations()
+    derived = {i: r for i, r in enumerate(rel) if r[0] >= 0}
+    assert derived == {12: (11, -1, 0), 21: (15, -1, 0), 22: (17, +1, 0), 23: (16, +1, 0), 24: (18, +1, 1),
+                       25: (19, -1, 0), 26: (20, +1, 0), 35: (34, -1, 0), 39: (38, +1, 0)}
+    for i, (src, _sign, _swap) in derived.items():
+        assert src < i and rel[src][0] < 0
+    reduced = [c for c, r in zip(nbs.nbs_std_channels(), rel) if r[0] < 0]
+    assert len(reduced) == 43 and ("n", "X0") not in {(c[0], c[1]) for c in reduced}
+    assert nbs.nbs_plan_selfcheck(reduced) == 0
+    # no image in the list: nothing is derived; an image with exchanged source baryons carries the a3 <-> a4 flag
+    assert all(r[0] < 0 for r in nbs.nbs_iso_relations([("p", "n", "p", "n"), ("Xm", "L", "Xm", "L")]))
+    assert nbs.nbs_iso_relations([("p", "Xm", "Sp", "Sm"), ("n", "X0", "Sp", "Sm")]) == [(-1, 1, 0), (0, 1, 1)]

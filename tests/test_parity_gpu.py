@@ -373,6 +373,54 @@ def test_isospin_fast_path_matches_general_path(torch_cuda, nbs, oracle):
     assert_parity(F_iso, F_gen, chans)
 
 
+def test_isospin_channel_relations(torch_cuda, nbs, oracle):
+    """VERDICT r1 item 8 / include/nbs.h nbs_set_channel_relations: with d == u nine of the 52 channels are the u <-> d
+    images of earlier ones (the whole sink pair n Xi0 among them) and are written by the epilogue from their originals.
+    Against the oracle and against the same run with the relations switched off, at L = 4 and at L = 6 (radix-3 FFT,
+    momenta with q != -q for the mirror of the identical-baryon pairs); channel ranges that hold images without their
+    originals; a user list with X fields (<n L | n Xd> = <p L | p Xu>)."""
+    torch = torch_cuda
+    chans = oracle.channels52()
+    keep = {}
+    for L, seed in ((4, 14), (6, 15)):
+        S = props(L, seed=seed, same=(("d", "u"),))
+        with nbs.Nbs(L, 1) as ctx:
+            d = to_dev(torch, S)
+            ctx.load(0, d["u"], d["d"], d["s"])
+            assert ctx.derived_channels() == 9
+            F_rel = ctx.correlator(0).cpu().numpy()
+            part = ctx.correlator(0, 21, 27).cpu().numpy()      # all of n Xi0: nothing but images
+            one = ctx.correlator(0, 24, 25).cpu().numpy()       # the image with a3 <-> a4
+            launches = ctx.kernel_launches()
+            ctx.set_channel_relations(False)
+            assert ctx.derived_channels() == 0
+            F_all = ctx.correlator(0).cpu().numpy()
+            ctx.set_channel_relations(True)
+            assert ctx.kernel_launches() > launches
+        if L == 4:
+            B = oracle.all_blocks(S, oracle.sink_names(chans))
+            assert_parity(F_rel, oracle.correlator_fft(L, B, chans), chans)
+        assert_parity(F_rel, F_all, chans)
+        assert np.array_equal(part, F_rel[21:27]) and np.array_equal(one, F_rel[24:25])
+        # the relations as the oracle's pins state them (tests/test_oracle_pins.py): exact in the derived run
+        assert np.array_equal(F_rel[23], F_rel[16]) and np.array_equal(F_rel[12], -F_rel[11])
+        assert np.array_equal(F_rel[24], np.swapaxes(F_rel[18], 2, 3))
+        keep[L] = F_rel
+    # general path (d is another array): nothing is derived
+    L = 4
+    S = props(L, seed=14, same=(("d", "u"),))
+    with nbs.Nbs(L, 1) as ctx:
+        u = torch.from_numpy(S["u"]).cuda()
+        ctx.load(0, u, u.clone(), torch.from_numpy(S["s"]).cuda())
+        F_gen = ctx.correlator(0).cpu().numpy()
+    assert_parity(keep[4], F_gen, chans)
+    user = [("p", "L", "p", "Xu"), ("n", "L", "n", "Xd"), ("p", "L", "Sp", "n"), ("n", "L", "Sm", "p"), ("p", "n", "p", "n")]
+    assert [r[0] for r in nbs.nbs_iso_relations(user)] == [-1, 0, -1, 2, -1]
+    Fu = run_gpu(torch, nbs, L, S, user)
+    B = oracle.all_blocks(S, oracle.sink_names(user))
+    assert_parity(Fu, oracle.correlator_fft(L, B, user), user)
+
+
 def test_8cubed_selected_channels(torch_cuda, nbs, oracle):
     """L = 8: the remaining power-of-two instance of the in-register FFT and of the fused inverse x-y kernel."""
     L = 8
