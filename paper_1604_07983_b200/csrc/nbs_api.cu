@@ -120,6 +120,7 @@ struct nbs_ctx {
     int2x* d_slot_src = nullptr;     // where the product kernel stages every slot from
     int2* d_one_slot_info = nullptr; // the same for a single baryon (nbs_blocks_x)
     BlockRec* d_brec = nullptr;
+    uint16_t* d_blk_out = nullptr; // k_blocks: where a thread's tile goes in the half-row buffer (blocks_out_offsets)
     BTermRec* d_bterm = nullptr;
     double2* d_tw = nullptr;
     unsigned dq_mask = 0;
@@ -288,7 +289,7 @@ int launch_blocks(nbs_ctx* c, const Slice& s, const int* d_list, const int2* d_i
     for (int b = 0; b < 9; ++b) ndq += (dq_mask >> b) & 1u;
     if (nslots > BLOCKS_MAX_SLOTS) return fail(c, NBS_EINVAL, "too many block slots");
     k_blocks<<<(unsigned)c->V, BLOCKS_THREADS, blocks_smem_bytes(ndq), st>>>(s.S[0], s.S[1], s.S[2], d_list, nslots, dq_mask,
-                                                                          c->d_brec, c->d_bterm, d_info, out, row_stride, pp);
+                                                                          c->d_brec, c->d_bterm, d_info, c->d_blk_out, out, row_stride, pp);
     CU(c, cudaGetLastError());
     ++c->launches;
     return NBS_OK;
@@ -815,6 +816,11 @@ int nbs_create(nbs_ctx** out, int L, int T, const nbs_channel* ch, int nch, int 
         CUC(upload(c, c->d_one_slot_info, one));
     }
     CUC(upload(c, c->d_brec, brec));
+    {
+        std::vector<uint16_t> oo(3 * BLOCKS_THREADS * 16);
+        blocks_out_offsets(oo.data());
+        CUC(upload(c, c->d_blk_out, oo));
+    }
     CUC(upload(c, c->d_bterm, bterm));
     CUC(upload(c, c->d_tw, tw));
 

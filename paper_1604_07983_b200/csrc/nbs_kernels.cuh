@@ -63,6 +63,52 @@ static_assert(AS_BLOCK <= BLOCKS_HALF, "a compact antisymmetric block is assembl
 constexpr int DQ_ROW = 13, DQ_C = 12 * DQ_ROW, DQ_SIZE = 3 * DQ_C; // per diquark type: [c][rank(xi)][rank(xi')]
 __host__ __device__ constexpr int dq_rank(int xi) { return (xi & 1) * 6 + (xi >> 1); }
 constexpr int BLOCKS_MAX_SLOTS = 16; // per-slot records kept in shared memory (there are 11 interpolating fields)
+// Register tile of thread `tid` for a block of `kind`: origins (x0, x1, x2) of its 2 x 2 x 2 source triples, first sink
+// spin a0 of its two (full kind: 2 * pass), whether the thread has a tile at all.  Full blocks: 216 tiles per pass of two
+// sink spins; antisymmetric blocks: one pass, 2 x 126 tiles on or above the diagonal of the antisymmetric slot pair.
+struct BlocksTile { int x0, x1, x2, a0; bool active; };
+__host__ __device__ inline BlocksTile blocks_tile(int kind, int tid, int pass) {
+    BlocksTile t;
+    if (kind == BK_FULL) {
+        t.active = tid < BLOCKS_TILES; t.a0 = 2 * pass;
+        t.x0 = 2 * (tid / 36); t.x1 = 2 * ((tid / 6) % 6); t.x2 = 2 * (tid % 6);
+    } else {
+        const int h = tid / 126, tt = tid - h * 126;
+        t.active = tid < 252;
+        int ia = 0, rem = tt / 6;
+        while (rem >= 6 - ia) { rem -= 6 - ia; ++ia; }
+        const int ib = ia + rem, ic = tt % 6;
+        t.a0 = 2 * h; t.x2 = 2 * ib;
+        if (kind == BK_ASYM13) { t.x0 = 2 * ia; t.x1 = 2 * ic; }
+        else { t.x1 = 2 * ia; t.x0 = 2 * ic; }
+    }
+    return t;
+}
+// Where the 16 results of a thread's tile go in the half-row buffer (index ((a * 2 + e0) * 2 + e1) * 2 + e2), per block
+// kind: the same for every slot of a kind, so the host writes them once ([kind][tid][16] uint16, 24 KB, read through L1 /
+// L2 as two 16-byte loads per pass) instead of every thread evaluating the layout functions 16 times per pass -- that
+// index arithmetic was as many instructions as the arithmetic of a two-term block.  0xffff: no entry (an antisymmetric
+// pair with xi_a >= xi_b, a thread without a tile).
+constexpr int BLOCKS_OUT_SKIP = 0xffff;
+inline void blocks_out_offsets(uint16_t* tab) { // [3][BLOCKS_THREADS][16]
+    for (int kind = 0; kind < 3; ++kind)
+        for (int tid = 0; tid < 256; ++tid) {
+            const BlocksTile t = blocks_tile(kind, tid, 0);
+            for (int i = 0; i < 16; ++i) {
+                const int a = i >> 3, e0 = (i >> 2) & 1, e1 = (i >> 1) & 1, e2 = i & 1;
+                const int xi0 = t.x0 + e0, xi1 = t.x1 + e1, xi2 = t.x2 + e2;
+                int off = BLOCKS_OUT_SKIP;
+                if (t.active) {
+                    if (kind == BK_FULL) off = a * SM_PLANE + sm_index(xi0, xi1, xi2);
+                    else {
+                        const int xa = (kind == BK_ASYM13) ? xi0 : xi1, xc = (kind == BK_ASYM13) ? xi1 : xi0;
+                        if (xa < xi2) off = (t.a0 + a) * AS_PLANE + as_index(xa, xi2, xc);
+                    }
+                }
+                tab[(kind * 256 + tid) * 16 + i] = (uint16_t)off;
+            }
+        }
+}
 inline size_t blocks_smem_bytes(int ndq) { return (size_t)(3 * 144 + ndq * DQ_SIZE + BLOCKS_HALF + BLOCKS_MAX_SLOTS) * sizeof(double2); }
 
 // acc[a][e0][e1][e2] += coef * sum_c D_c(xi_P0, xi_P1) * S[(c, a0 + a), xi_P2] over the thread's tile
@@ -106,7 +152,7 @@ __global__ void __launch_bounds__(BLOCKS_THREADS, 2)
 k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const double2* __restrict__ Ss,
          const int* __restrict__ baryon_of_slot, int nslots, unsigned dq_mask,
          const BlockRec* __restrict__ brec, const BTermRec* __restrict__ bterm,
-         const int2* __restrict__ slot_info, double2* __restrict__ out, size_t row_stride, int pp) {
+         const int2* __restrict__ slot_info, const uint16_t* __restrict__ out_off, double2* __restrict__ out, size_t row_stride, int pp) {
     // pp < 0: whole blocks.  pp = 0, 1 (tile-wise plan, one slot): only the sink-spin planes {2 pp, 2 pp + 1},
     // written as a two-plane chunk row (staged planes for a full-kind block, compact planes for an antisymmetric one)
     extern __shared__ double2 smem[];
@@ -164,22 +210,12 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
         const int npass = (kind == BK_FULL) ? 2 : 1;
         for (int pass = 0; pass < npass; ++pass) {
             if (pp >= 0 && kind == BK_FULL && pass != pp) continue; // uniform over the CTA
-            int x0, x1, x2, a0 = 2 * pass;
-            bool active;
-            if (kind == BK_FULL) {
-                active = tid < BLOCKS_TILES;
-                x0 = 2 * (tid / 36); x1 = 2 * ((tid / 6) % 6); x2 = 2 * (tid % 6);
-            } else {
-                const int h = tid / 126, tt = tid - h * 126;
-                active = tid < 252 && (pp < 0 || h == pp);
-                int ia = 0, rem = tt / 6;
-                while (rem >= 6 - ia) { rem -= 6 - ia; ++ia; }
-                const int ib = ia + rem, ic = tt % 6;
-                a0 = 2 * h;
-                x2 = 2 * ib;
-                if (kind == BK_ASYM13) { x0 = 2 * ia; x1 = 2 * ic; }
-                else { x1 = 2 * ia; x0 = 2 * ic; }
-            }
+            const BlocksTile tl = blocks_tile(kind, tid, pass);
+            const int x0 = tl.x0, x1 = tl.x1, x2 = tl.x2, a0 = tl.a0;
+            const bool active = tl.active && (kind == BK_FULL || pp < 0 || (a0 >> 1) == pp);
+            // where the tile's results go (host table, see blocks_out_offsets): fetched under the arithmetic
+            const uint4* otab = reinterpret_cast<const uint4*>(out_off + (kind * BLOCKS_THREADS + tid) * 16);
+            const uint4 o0 = __ldg(otab), o1 = __ldg(otab + 1);
             double2 acc[2][2][2][2];
             if (active) {
 #pragma unroll
@@ -216,22 +252,12 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                 }
             }
             if (active) {
+                const uint32_t ow[8] = {o0.x, o0.y, o0.z, o0.w, o1.x, o1.y, o1.z, o1.w};
 #pragma unroll
-                for (int a = 0; a < 2; ++a)
-#pragma unroll
-                    for (int e0 = 0; e0 < 2; ++e0)
-#pragma unroll
-                        for (int e1 = 0; e1 < 2; ++e1)
-#pragma unroll
-                            for (int e2 = 0; e2 < 2; ++e2) {
-                                const int xi0 = x0 + e0, xi1 = x1 + e1, xi2 = x2 + e2;
-                                if (kind == BK_FULL) {
-                                    sO[a * SM_PLANE + sm_index(xi0, xi1, xi2)] = acc[a][e0][e1][e2];
-                                } else {
-                                    const int xa = (kind == BK_ASYM13) ? xi0 : xi1, xc = (kind == BK_ASYM13) ? xi1 : xi0;
-                                    if (xa < xi2) sO[(a0 + a) * AS_PLANE + as_index(xa, xi2, xc)] = acc[a][e0][e1][e2];
-                                }
-                            }
+                for (int i = 0; i < 16; ++i) {
+                    const uint32_t off = (ow[i >> 1] >> (16 * (i & 1))) & 0xffffu;
+                    if (off != (uint32_t)BLOCKS_OUT_SKIP) sO[off] = (&acc[0][0][0][0])[i];
+                }
             }
             // the half row leaves through the async proxy (one bulk copy shared -> global), under the next pass
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
