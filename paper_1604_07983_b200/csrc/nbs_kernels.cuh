@@ -213,9 +213,6 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
             const BlocksTile tl = blocks_tile(kind, tid, pass);
             const int x0 = tl.x0, x1 = tl.x1, x2 = tl.x2, a0 = tl.a0;
             const bool active = tl.active && (kind == BK_FULL || pp < 0 || (a0 >> 1) == pp);
-            // where the tile's results go (host table, see blocks_out_offsets): fetched under the arithmetic
-            const uint4* otab = reinterpret_cast<const uint4*>(out_off + (kind * BLOCKS_THREADS + tid) * 16);
-            const uint4 o0 = __ldg(otab), o1 = __ldg(otab + 1);
             double2 acc[2][2][2][2];
             if (active) {
 #pragma unroll
@@ -237,6 +234,9 @@ k_blocks(const double2* __restrict__ Su, const double2* __restrict__ Sd, const d
                     }
                 }
             }
+            // where the tile's results go (host table, see blocks_out_offsets): fetched under the barrier wait
+            const uint4* otab = reinterpret_cast<const uint4*>(out_off + (kind * BLOCKS_THREADS + tid) * 16);
+            const uint4 o0 = __ldg(otab), o1 = __ldg(otab + 1);
             // the bulk store of the previous half row (issued by thread 0) must have read sO before it is rewritten
             if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
             __syncthreads();
