@@ -267,7 +267,11 @@ int nbs_set_pipelined(nbs_ctx* ctx, int enable);
  *   <B1 B2 | B3 B4> = eta1 eta2 eta3 eta4 <B1' B2' | B3' B4'>,  <.. | B4' B3'>_{a3 a4} = - <.. | B3' B4'>_{a4 a3},
  * with p <-> n, Sigma+ <-> Sigma-, Xi0 <-> Xi-, X_u <-> X_d (eta = -1 for Lambda, Xi0, Xi-, X_u, X_d, X_s; eqs. 2.2-2.3).
  * In the standard list these are nine channels (n Xi0 -> anything: all six; Lambda Lambda -> n Xi0, Sigma0 Sigma0 ->
- * n Xi0, Sigma0 Lambda -> n Xi0), so the sink pair n Xi0 is not contracted at all.  Results equal the full computation
+ * n Xi0, Sigma0 Lambda -> n Xi0), so the sink pair n Xi0 is not contracted at all.  A sink pair made of a field and its
+ * image (p n, Sigma+ Sigma-, Xi- Xi0) is, in addition, contracted for half of the momenta only, like a pair of identical
+ * baryons: with the sink swap F^{B1 B2}_{a1 a2}(r) = - F^{B2 B1}_{a2 a1}(-r) the relation above gives
+ *   F[B B' | B3 B4](q)_{a1 a2 a3 a4} = - eta eta' eta3 eta4 F[B B' | B3' B4'](-q)_{a2 a1 a3 a4}
+ * whenever the channels of the pair are closed under B3 B4 -> B3' B4'.  Results equal the full computation
  * up to rounding.  Resident plan with the pipelined product kernel only.
  *   enable != 0 (default): use the relations;  enable == 0: compute every channel;
  *   enable < 0: query -- returns the number of channels that are derived this way (0: none / not available / off).

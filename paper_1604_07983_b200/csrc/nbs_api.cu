@@ -615,12 +615,18 @@ static int build_iso_channels(nbs_ctx* c, size_t smem_optin) {
     ic.nderived = (int)(rel.size() - red.size());
     if (ic.nderived == 0) return NBS_OK;
     Plan& rp = ic.plan;
-    if (!build_plan(red, rp).empty() || !rp.cprog_ok || rp.max_pair_units > c->plan.max_pair_units || rp.baryons.size() >= 256) return NBS_OK;
+    // channels that carry an image to write take no part in the mirror relation of conjugate sink pairs
+    std::vector<char> carries(red.size(), 0);
+    for (size_t i = 0; i < rel.size(); ++i)
+        if (rel[i].from >= 0)
+            for (size_t k = 0; k < orig.size(); ++k)
+                if (orig[k] == rel[i].from) carries[k] = 1;
+    if (!build_plan(red, rp, 18, 80, &carries).empty() || !rp.cprog_ok || rp.max_pair_units > c->plan.max_pair_units || rp.baryons.size() >= 256) return NBS_OK;
     ic.units_bytes = (uint32_t)rp.max_pair_units * (uint32_t)sizeof(Unit3Rec);
     ic.rec_stride = C_ITEM_BYTES + ic.units_bytes + (uint32_t)rp.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
     ic.smem = cprod_smem_bytes(ic.rec_stride);
     if (ic.smem > smem_optin) return NBS_OK;
-    for (auto& pc : rp.pair_chans) pc.ch = orig[pc.ch]; // channel numbers of the full list
+    for (auto& pc : rp.pair_chans) { pc.ch = orig[pc.ch]; pc.mirror_ch = orig[pc.mirror_ch]; } // channel numbers of the full list
     for (size_t i = 0; i < rel.size(); ++i) {
         if (rel[i].from < 0) continue;
         bool found = false;

@@ -117,7 +117,19 @@ __device__ __forceinline__ void combine_item_c(const ProdArgs& a, int ip, size_t
                         for (int m = 0; m < NM; ++m) {
                             const double2 val = make_double2(acc[c][m].x * osign, acc[c][m].y * osign); // +-1: sign of a derived block (isospin limit)
                             __stcs(a.Ft + (q * a.nch_out + ch) * 256 + comp(m), val);
-                            if (mirror) __stcs(a.Ft + (mq * a.nch_out + ch) * 256 + mirror_comp(m), make_double2(-val.x, -val.y));
+                            if (!ALIAS && mirror) __stcs(a.Ft + (mq * a.nch_out + ch) * 256 + mirror_comp(m), make_double2(-val.x, -val.y));
+                        }
+                    }
+                    if (ALIAS && mirror) { // reduced plan of the isospin limit: the mirror may be another channel (PairChanRec::mirror_*)
+                        const int mch = pcs[c].mirror_ch - a.ch_begin;
+                        if (mch >= 0 && mch < a.nch_out) {
+                            const double msg = osign * pcs[c].mirror_sign;
+                            const bool msw = pcs[c].mirror_swap != 0;
+#pragma unroll
+                            for (int m = 0; m < NM; ++m) {
+                                const int i = mirror_comp(m), im = msw ? ((i & ~15) | ((i & 3) << 2) | ((i >> 2) & 3)) : i;
+                                __stcs(a.Ft + (mq * a.nch_out + mch) * 256 + im, make_double2(acc[c][m].x * msg, acc[c][m].y * msg));
+                            }
                         }
                     }
                     // isospin limit, reduced channel list: the u <-> d image of this channel is written from it (nbs_tables.hpp, IsoRelation)

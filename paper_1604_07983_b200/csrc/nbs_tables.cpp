@@ -356,7 +356,8 @@ std::string channel_diagrams(const nbs_channel& ch, std::vector<DiagramInfo>& ou
     return "";
 }
 
-std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps, int unit_cost_max) {
+std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps, int unit_cost_max,
+                       const std::vector<char>* iso_conj) {
     plan = Plan();
     plan.channels = channels;
     if (channels.empty()) return "empty channel list";
@@ -663,6 +664,7 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             PairChanRec pc;
             pc.ch = (int)ic; pc.local = (int)plan.pair_chans.size() - pr.chan_begin;
             pc.alias_ch = -1; pc.alias_swap = 0; pc.alias_sign = 1.0;
+            pc.mirror_ch = pc.ch; pc.mirror_swap = 0; pc.mirror_sign = -1.0;
             bool any = false;
             for (int e = 0; e < MAX_PAIR_ELEMS; ++e) pc.coef[e] = pc.coefS[e] = 0.0;
             for (auto& ct : chan_ct[ic])
@@ -676,6 +678,32 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             if (any) plan.pair_chans.push_back(pc);
         }
         pr.nchan = (int)plan.pair_chans.size() - pr.chan_begin;
+        // isospin limit: sink pair of a field and its u <-> d image, channel set closed under the images of the sources
+        if (iso_conj && !pr.self_swap) {
+            const int b1 = pair_list[ip].first, b2 = pair_list[ip].second;
+            int e1 = 0, e2 = 0;
+            bool ok = baryon_iso_mirror(b1, &e1) == b2 && baryon_iso_mirror(b2, &e2) == b1 && pr.nchan > 0;
+            std::vector<PairChanRec> recs(plan.pair_chans.begin() + pr.chan_begin, plan.pair_chans.end());
+            for (auto& pc : recs) {
+                const nbs_channel& c = channels[pc.ch];
+                int e3 = 0, e4 = 0;
+                const int m3 = baryon_iso_mirror(c.b3, &e3), m4 = baryon_iso_mirror(c.b4, &e4);
+                ok = ok && m3 >= 0 && m4 >= 0 && !(*iso_conj)[pc.ch];
+                if (!ok) break;
+                const int s = e1 * e2 * e3 * e4;
+                bool found = false;
+                for (auto& other : recs) {
+                    const nbs_channel& d = channels[other.ch];
+                    if (d.b3 == m3 && d.b4 == m4) { pc.mirror_ch = other.ch; pc.mirror_swap = 0; pc.mirror_sign = -(double)s; found = true; break; }
+                    if (d.b3 == m4 && d.b4 == m3) { pc.mirror_ch = other.ch; pc.mirror_swap = 1; pc.mirror_sign = (double)s; found = true; break; }
+                }
+                ok = found;
+            }
+            if (ok) {
+                std::copy(recs.begin(), recs.end(), plan.pair_chans.begin() + pr.chan_begin);
+                pr.self_swap = 2;
+            }
+        }
         plan.pairs3.push_back(pr);
     }
     plan.tab3.insert(plan.tab3.end(), 4096, uint2x{0, 0}); // the kernel prefetches a few k-steps past a table's end (4096: also covers nbs_plan_selfcheck's class-blind bound)

@@ -130,7 +130,8 @@ struct Pair3Rec {
     int elem_unit_begin[MAX_PAIR_ELEMS + 1]; // scratch-row ranges per elementary correlator
     int chan_begin, nchan;   // range in Plan::pair_chans
     int swap_mask;           // bit e: some channel needs elementary correlator e with a3 <-> a4 exchanged
-    int self_swap;           // 1: identical sink baryons; computed for q <= -q only, mirrored to -q by the epilogue
+    int self_swap;           // 1: identical sink baryons; 2: a field and its u <-> d image (reduced plan of the isospin limit);
+                             // computed for q <= -q only, mirrored to -q by the epilogue (PairChanRec::mirror_*)
 };
 struct PairChanRec {
     int ch, local; // channel index; position of the channel among the channels of its sink pair (row of the tile-wise plan's Ft)
@@ -138,6 +139,12 @@ struct PairChanRec {
     // F[alias_ch] = alias_sign * F[ch], with the source spins a3 <-> a4 exchanged if alias_swap; alias_ch = -1: none
     int alias_ch, alias_swap;
     double alias_sign;
+    // what the epilogue writes at -q for a pair that is computed for the momenta q <= -q only (Pair3Rec::self_swap):
+    // F[mirror_ch](-q)_{a2 a1 ..} = mirror_sign * F[ch](q)_{a1 a2 ..}, with a3 <-> a4 exchanged as well if mirror_swap.
+    // Identical sink baryons (reading A11): the channel itself, sign -1.  Isospin limit, sink pair (B, B') of a field
+    // and its u <-> d image (p n, Sigma+ Sigma-, Xi- Xi0): the channel with the images of the source baryons.
+    int mirror_ch, mirror_swap;
+    double mirror_sign;
     double coef[MAX_PAIR_ELEMS];  // channel = sum_e coef[e] * E_e + coefS[e] * (E_e with a3 <-> a4), eqs. 2.2-2.3;
     double coefS[MAX_PAIR_ELEMS]; // coefS carries the minus sign of the source swap (reading A11)
 };
@@ -251,8 +258,12 @@ struct Plan {
 };
 
 // Returns "" on success, else an error message (invalid id, flavour violation).
+// iso_conj (reduced plan of the isospin limit only): per channel, 1 = this channel may not take part in a mirror relation
+// (it carries a u <-> d image to write); a non-NULL vector switches the relation
+//   F[B B' | B3 B4](q)_{a1 a2 a3 a4} = - eta_B eta_B' eta_3 eta_4 F[B B' | B3' B4'](-q)_{a2 a1 a3 a4}      (B' = image of B)
+// on for every sink pair whose channel set is closed under it: such a pair is computed for q <= -q only.
 std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps = 18,
-                       int unit_cost_max = 80);
+                       int unit_cost_max = 80, const std::vector<char>* iso_conj = nullptr);
 
 // Channel relations of the isospin limit (u and d propagators identical): relabelling u <-> d maps every
 // interpolating field of eqs. 2.2-2.3 to +-1 times another one (p <-> n, Sigma+ <-> Sigma-, Xi0 <-> -Xi-, Lambda -> -Lambda,
