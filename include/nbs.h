@@ -175,7 +175,10 @@ int nbs_channel_info(const nbs_ctx* ctx, int i, nbs_channel* out);
 int nbs_std_channels(nbs_channel* out, int cap);
 /*   nbs_plan_selfcheck: host-only bounds check of the tables the kernels index with (gather offsets inside the staged
  *             blocks, table extents including the software pipeline's look-ahead, unit / diagram / chain / channel record
- *             ranges, expansion maps); ch == NULL checks the standard 52 channels.  Returns 0 or a negative check number. */
+ *             ranges, expansion maps); ch == NULL checks the standard 52 channels.  If the list holds u <-> d images
+ *             (nbs_iso_relations), the reduced plan of the isospin limit is built and checked the same way (check numbers
+ *             minus 1000), together with the mirror relation of its conjugate sink pairs (an involution inside the pair,
+ *             signs +-1: -1151 ... -1155).  Returns 0 or a negative check number. */
 int nbs_plan_selfcheck(const nbs_channel* ch, int nch);
 int nbs_diagram_stats(const nbs_channel* ch, int* K, int* sign, int cap, long long* literal_terms);
 
@@ -274,7 +277,8 @@ int nbs_set_pipelined(nbs_ctx* ctx, int enable);
  * whenever the channels of the pair are closed under B3 B4 -> B3' B4'.  Results equal the full computation
  * up to rounding.  Resident plan with the pipelined product kernel only.
  *   enable != 0 (default): use the relations;  enable == 0: compute every channel;
- *   enable < 0: query -- returns the number of channels that are derived this way (0: none / not available / off).
+ *   enable == -1: query -- returns the number of channels that are derived this way (0: none / not available / off);
+ *   enable == -2: query -- the number of sink pairs that are contracted for half of the momenta by the second relation.
  */
 int nbs_set_channel_relations(nbs_ctx* ctx, int enable);
 /*   nbs_iso_relations: the relations themselves, on the host only (no CUDA call): for channel i of the list (ch == NULL:

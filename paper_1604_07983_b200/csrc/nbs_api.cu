@@ -465,13 +465,67 @@ int nbs_iso_relations(const nbs_channel* ch, int nch, int* from, int* sign, int*
     return (int)rel.size();
 }
 
+static int plan_selfcheck(const Plan& P);
+
+// The reduced plan of the isospin limit (build_iso_channels): the channels that are no u <-> d image, with the mirror
+// relation of conjugate sink pairs switched on.  Returns false if the list has neither an image nor a conjugate pair.
+static bool reduced_iso_plan(const std::vector<nbs_channel>& chans, Plan& rp, std::vector<int>& orig, std::string& err) {
+    const std::vector<IsoRelation> rel = iso_channel_relations(chans);
+    std::vector<nbs_channel> red;
+    orig.clear();
+    for (size_t i = 0; i < rel.size(); ++i)
+        if (rel[i].from < 0) { red.push_back(chans[i]); orig.push_back((int)i); }
+    std::vector<char> carries(red.size(), 0); // channels that carry an image to write take no part in the mirror relation
+    for (size_t i = 0; i < rel.size(); ++i)
+        if (rel[i].from >= 0)
+            for (size_t k = 0; k < orig.size(); ++k)
+                if (orig[k] == rel[i].from) carries[k] = 1;
+    err = build_plan(red, rp, 18, 80, &carries);
+    if (!err.empty()) return true;
+    bool conj = false;
+    for (auto& pr : rp.pairs3) conj = conj || pr.self_swap == 2;
+    return conj || red.size() < chans.size();
+}
+
 int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
     // Host-side bounds check of everything the kernels index with table data (compute-sanitizer is not available on
     // the target pool): returns 0, or the negative number of the first violated invariant.
     std::vector<nbs_channel> chans = ch ? std::vector<nbs_channel>(ch, ch + nch) : standard_channels();
+    for (auto& x : chans)
+        for (int b : {x.b1, x.b2, x.b3, x.b4})
+            if (b < 0 || b >= NBS_NUM_BARYONS) return NBS_EINVAL;
     Plan P;
     std::string err = build_plan(chans, P);
     if (!err.empty()) { g_create_error = err; return NBS_EINVAL; }
+    int rc = plan_selfcheck(P);
+    if (rc) return rc;
+    // the reduced plan of the isospin limit: the same invariants (1000 is subtracted from the check number), and the
+    // mirror relation of its conjugate sink pairs: an involution inside the pair, signs +-1, no channel that carries an image
+    Plan R;
+    std::vector<int> orig;
+    if (!reduced_iso_plan(chans, R, orig, err)) return 0;
+    if (!err.empty()) { g_create_error = err; return -1150; }
+    rc = plan_selfcheck(R);
+    if (rc) return rc - 1000;
+    for (auto& pr : R.pairs3)
+        for (int k = 0; k < pr.nchan; ++k) {
+            const PairChanRec& pc = R.pair_chans[pr.chan_begin + k];
+            if (pr.self_swap != 2) {
+                if (pc.mirror_ch != pc.ch || pc.mirror_swap != 0 || pc.mirror_sign != -1.0) return -1151;
+                continue;
+            }
+            const PairChanRec* m = nullptr;
+            for (int j = 0; j < pr.nchan; ++j)
+                if (R.pair_chans[pr.chan_begin + j].ch == pc.mirror_ch) m = &R.pair_chans[pr.chan_begin + j];
+            if (!m) return -1152;                                   // the mirror channel belongs to the same sink pair
+            if (m->mirror_ch != pc.ch || m->mirror_swap != pc.mirror_swap || m->mirror_sign != pc.mirror_sign) return -1153; // involution
+            if (pc.mirror_sign != 1.0 && pc.mirror_sign != -1.0) return -1154;
+            if (R.baryons[pr.slot1] == R.baryons[pr.slot2]) return -1155;
+        }
+    return 0;
+}
+
+static int plan_selfcheck(const Plan& P) {
     const size_t ntab = P.tab3.size();
     for (auto& w : P.tab3) // 1: gather offsets are 16-byte aligned positions inside a staged block
         if (w.x % 16 || w.y % 16 || w.x >= BLOCK_BYTES || w.y >= BLOCK_BYTES) return -101;
@@ -570,7 +624,7 @@ int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
         if (pr.chan_begin + pr.nchan > (int)P.pair_chans.size()) return -113;
         for (int k = 0; k < pr.nchan; ++k) {
             const PairChanRec& pc = P.pair_chans[pr.chan_begin + k];
-            if (pc.ch < 0 || pc.ch >= (int)chans.size() || pc.local != k) return -114;
+            if (pc.ch < 0 || pc.ch >= (int)P.channels.size() || pc.local != k) return -114;
         }
     }
     if ((int)P.chain.size() != P.chain_full_n + P.chain_half_n + (int)P.pairs3.size()) return -115;
@@ -607,21 +661,14 @@ int nbs_plan_selfcheck(const nbs_channel* ch, int nch) {
 // false and the isospin limit runs the full plan (same results).
 static int build_iso_channels(nbs_ctx* c, size_t smem_optin) {
     const std::vector<IsoRelation> rel = iso_channel_relations(c->plan.channels);
-    std::vector<nbs_channel> red;
-    std::vector<int> orig;
-    for (size_t i = 0; i < rel.size(); ++i)
-        if (rel[i].from < 0) { red.push_back(c->plan.channels[i]); orig.push_back((int)i); }
     nbs_ctx::IsoChannels& ic = c->isoch;
-    ic.nderived = (int)(rel.size() - red.size());
-    if (ic.nderived == 0) return NBS_OK;
+    ic.nderived = 0;
+    for (auto& r : rel) ic.nderived += r.from >= 0;
     Plan& rp = ic.plan;
-    // channels that carry an image to write take no part in the mirror relation of conjugate sink pairs
-    std::vector<char> carries(red.size(), 0);
-    for (size_t i = 0; i < rel.size(); ++i)
-        if (rel[i].from >= 0)
-            for (size_t k = 0; k < orig.size(); ++k)
-                if (orig[k] == rel[i].from) carries[k] = 1;
-    if (!build_plan(red, rp, 18, 80, &carries).empty() || !rp.cprog_ok || rp.max_pair_units > c->plan.max_pair_units || rp.baryons.size() >= 256) return NBS_OK;
+    std::vector<int> orig;
+    std::string err;
+    if (!reduced_iso_plan(c->plan.channels, rp, orig, err)) return NBS_OK;
+    if (!err.empty() || !rp.cprog_ok || rp.max_pair_units > c->plan.max_pair_units || rp.baryons.size() >= 256) return NBS_OK;
     ic.units_bytes = (uint32_t)rp.max_pair_units * (uint32_t)sizeof(Unit3Rec);
     ic.rec_stride = C_ITEM_BYTES + ic.units_bytes + (uint32_t)rp.max_pair_diags * (uint32_t)sizeof(Diag3Rec);
     ic.smem = cprod_smem_bytes(ic.rec_stride);
@@ -658,6 +705,12 @@ static int build_iso_channels(nbs_ctx* c, size_t smem_optin) {
 
 int nbs_set_channel_relations(nbs_ctx* c, int enable) {
     if (!c) return NBS_EINVAL;
+    if (enable == -2) { // query: sink pairs contracted for half of the momenta thanks to the relations
+        int n = 0;
+        if (c->isoch.ok && c->iso_relations)
+            for (auto& pr : c->isoch.plan.pairs3) n += pr.self_swap == 2;
+        return n;
+    }
     if (enable < 0) return (c->isoch.ok && c->iso_relations) ? c->isoch.nderived : 0; // query
     c->iso_relations = enable != 0;
     return NBS_OK;

@@ -684,20 +684,34 @@ std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int
             int e1 = 0, e2 = 0;
             bool ok = baryon_iso_mirror(b1, &e1) == b2 && baryon_iso_mirror(b2, &e2) == b1 && pr.nchan > 0;
             std::vector<PairChanRec> recs(plan.pair_chans.begin() + pr.chan_begin, plan.pair_chans.end());
-            for (auto& pc : recs) {
+            // the relation pairs the channel records up (a record may be its own partner); a list may hold a channel twice
+            std::vector<char> matched(recs.size(), 0);
+            for (size_t i = 0; i < recs.size() && ok; ++i) {
+                if (matched[i]) continue;
+                PairChanRec& pc = recs[i];
                 const nbs_channel& c = channels[pc.ch];
                 int e3 = 0, e4 = 0;
                 const int m3 = baryon_iso_mirror(c.b3, &e3), m4 = baryon_iso_mirror(c.b4, &e4);
-                ok = ok && m3 >= 0 && m4 >= 0 && !(*iso_conj)[pc.ch];
+                ok = m3 >= 0 && m4 >= 0 && !(*iso_conj)[pc.ch];
                 if (!ok) break;
                 const int s = e1 * e2 * e3 * e4;
-                bool found = false;
-                for (auto& other : recs) {
-                    const nbs_channel& d = channels[other.ch];
-                    if (d.b3 == m3 && d.b4 == m4) { pc.mirror_ch = other.ch; pc.mirror_swap = 0; pc.mirror_sign = -(double)s; found = true; break; }
-                    if (d.b3 == m4 && d.b4 == m3) { pc.mirror_ch = other.ch; pc.mirror_swap = 1; pc.mirror_sign = (double)s; found = true; break; }
-                }
-                ok = found;
+                auto relation = [&](const nbs_channel& d, int& swap, double& sign) {
+                    if (d.b3 == m3 && d.b4 == m4) { swap = 0; sign = -(double)s; return true; }
+                    if (d.b3 == m4 && d.b4 == m3) { swap = 1; sign = (double)s; return true; }
+                    return false;
+                };
+                int swap = 0;
+                double sign = 0.0;
+                size_t j = recs.size();
+                if (relation(c, swap, sign)) j = i; // its own partner
+                else
+                    for (size_t k = i + 1; k < recs.size(); ++k)
+                        if (!matched[k] && !(*iso_conj)[recs[k].ch] && relation(channels[recs[k].ch], swap, sign)) { j = k; break; }
+                ok = j < recs.size();
+                if (!ok) break;
+                pc.mirror_ch = recs[j].ch; pc.mirror_swap = swap; pc.mirror_sign = sign;
+                recs[j].mirror_ch = pc.ch; recs[j].mirror_swap = swap; recs[j].mirror_sign = sign;
+                matched[i] = matched[j] = 1;
             }
             if (ok) {
                 std::copy(recs.begin(), recs.end(), plan.pair_chans.begin() + pr.chan_begin);

@@ -284,6 +284,10 @@ class Nbs:
         """Number of channels the isospin limit derives from others (0: none, not available, or switched off)."""
         return int(_check(self.ctx, lib().nbs_set_channel_relations(self.ctx, -1)))
 
+    def conjugate_pairs(self) -> int:
+        """Number of sink pairs (a field and its u <-> d image) the isospin limit contracts for half of the momenta."""
+        return int(_check(self.ctx, lib().nbs_set_channel_relations(self.ctx, -2)))
+
     def set_timing(self, enable: bool = True):
         _check(self.ctx, lib().nbs_set_timing(self.ctx, 1 if enable else 0))
 

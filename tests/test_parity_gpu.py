@@ -387,7 +387,7 @@ def test_isospin_channel_relations(torch_cuda, nbs, oracle):
         with nbs.Nbs(L, 1) as ctx:
             d = to_dev(torch, S)
             ctx.load(0, d["u"], d["d"], d["s"])
-            assert ctx.derived_channels() == 9
+            assert ctx.derived_channels() == 9 and ctx.conjugate_pairs() == 3  # p n, Sigma+ Sigma-, Xi- Xi0
             F_rel = ctx.correlator(0).cpu().numpy()
             part = ctx.correlator(0, 21, 27).cpu().numpy()      # all of n Xi0: nothing but images
             one = ctx.correlator(0, 24, 25).cpu().numpy()       # the image with a3 <-> a4
@@ -419,6 +419,25 @@ def test_isospin_channel_relations(torch_cuda, nbs, oracle):
     Fu = run_gpu(torch, nbs, L, S, user)
     B = oracle.all_blocks(S, oracle.sink_names(user))
     assert_parity(Fu, oracle.correlator_fft(L, B, user), user)
+    # a list that holds channels twice: the mirror relation of the conjugate sink pairs (p n and Sigma+ Sigma- are computed
+    # for half of the momenta) has to pair the records up one to one, or leave the pair alone when it cannot
+    dup = [("p", "n", "p", "n")] * 3 + [("Sp", "Sm", "p", "Xm"), ("Sp", "Sm", "n", "X0"), ("Sp", "Sm", "n", "X0"),
+                                          ("Xm", "X0", "Xm", "X0"), ("Sp", "Sm", "Sp", "Sm")]
+    assert nbs.nbs_plan_selfcheck(dup) == 0
+    with nbs.Nbs(L, 1, dup) as ctx:  # no image in this list: the reduced plan exists for the conjugate pairs alone
+        d = to_dev(torch, S)
+        ctx.load(0, d["u"], d["d"], d["s"])
+        assert ctx.derived_channels() == 0 and ctx.conjugate_pairs() == 2  # p n and Xi- Xi0; Sigma+ Sigma- is not closed
+    Fd = run_gpu(torch, nbs, L, S, dup)
+    B = oracle.all_blocks(S, oracle.sink_names(dup))
+    assert_parity(Fd, oracle.correlator_fft(L, B, dup), dup)
+    dup2 = [("Sp", "Sm", "p", "Xm"), ("Sp", "Sm", "n", "X0"), ("Sp", "Sm", "L", "L"), ("Sp", "Sm", "L", "L"), ("p", "n", "p", "n"),
+            ("Xm", "L", "Xm", "L"), ("S0", "p", "S0", "p")]  # four sink pairs: the pipelined kernel needs three items per task
+    with nbs.Nbs(L, 1, dup2) as ctx:
+        assert ctx.conjugate_pairs() == 2  # Sigma+ Sigma- (two records that are their own partners, one exchanged pair), p n
+    Fd2 = run_gpu(torch, nbs, L, S, dup2)
+    B = oracle.all_blocks(S, oracle.sink_names(dup2))
+    assert_parity(Fd2, oracle.correlator_fft(L, B, dup2), dup2)
 
 
 def test_8cubed_selected_channels(torch_cuda, nbs, oracle):
