@@ -219,7 +219,8 @@ int nbs_model_flops(const nbs_ctx* ctx, double* blocks, double* fft, double* pro
  *             the DISTINCT elementary correlators: source Lambda / Sigma0 terms shared between
  *             channels of one sink pair are evaluated once).  <= the `product` model count.
  *   nbs_fft3d : rows a2 / a5 alone (eq. 2.6): in-place 3-D transform of a device
- *             array data[site][R] complex128, every one of the R components independently.
+ *             array data[site][R] complex128 (16-byte aligned: the x-y pass uses 16-byte asynchronous copies), every
+ *             one of the R components independently.
  *             inverse == 0: sum_x f(x) exp(-i q.x);  inverse != 0: L^-3 sum_q f(q) exp(+i q.r).
  *   nbs_kernel_launches : number of CUDA kernels this context has launched so far (bench.py's
  *             `gpu_launches`).

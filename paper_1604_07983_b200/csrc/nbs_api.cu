@@ -1331,6 +1331,7 @@ int nbs_fft3d(nbs_ctx* c, void* data_dev, size_t R, int inverse, void* stream) {
     if (!c) return NBS_EINVAL;
     if (c->cuda_failed) return NBS_ECUDA;
     if (!data_dev || R == 0) return fail(c, NBS_EINVAL, "NULL data or R == 0");
+    if (reinterpret_cast<uintptr_t>(data_dev) & 15u) return fail(c, NBS_EINVAL, "data must be 16-byte aligned");
     CU(c, cudaSetDevice(c->device));
     return fft3d(c, (double2*)data_dev, R, inverse != 0, (cudaStream_t)stream);
 }
