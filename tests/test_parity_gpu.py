@@ -96,6 +96,17 @@ def test_fft3d_matches_numpy(torch_cuda, nbs, L):
         assert np.abs(x.cpu().numpy() - a.reshape(L ** 3, R)).max() <= 1e-13 * np.abs(a).max()
 
 
+def test_fft3d_rejects_misaligned_data(torch_cuda, nbs):
+    """include/nbs.h: nbs_fft3d wants 16-byte aligned data (the x-y pass copies 16 bytes at a time)."""
+    torch = torch_cuda
+    with nbs.Nbs(4, 1, [("p", "n", "p", "n")]) as ctx:
+        buf = torch.zeros(64 * 8 * 2 + 2, dtype=torch.float64, device="cuda")
+        rc = nbs.lib().nbs_fft3d(ctx.ctx, buf.data_ptr() + 8, 8, 0, None)
+        assert rc == nbs.NBS_EINVAL and b"aligned" in nbs.lib().nbs_last_error(ctx.ctx)
+        assert nbs.lib().nbs_fft3d(ctx.ctx, buf.data_ptr(), 8, 0, None) == 0
+        torch.cuda.synchronize()
+
+
 # ------------------------------------------------------------------------------ whole path
 def test_config0_4cubed_NN(torch_cuda, nbs, oracle):
     """BASELINE.json configs[0]: 4^3 x 1, NN channel, u = d, seed 0.  Against tier B (all r) and
