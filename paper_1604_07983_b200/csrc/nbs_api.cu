@@ -480,7 +480,7 @@ static bool reduced_iso_plan(const std::vector<nbs_channel>& chans, Plan& rp, st
         if (rel[i].from >= 0)
             for (size_t k = 0; k < orig.size(); ++k)
                 if (orig[k] == rel[i].from) carries[k] = 1;
-    err = build_plan(red, rp, 18, 80, &carries);
+    err = build_plan(red, rp, UNIT_SPLIT_STEPS_DEFAULT, UNIT_COST_MAX_DEFAULT, &carries);
     if (!err.empty()) return true;
     bool conj = false;
     for (auto& pr : rp.pairs3) conj = conj || pr.self_swap == 2;
@@ -1339,7 +1339,7 @@ int nbs_fft3d(nbs_ctx* c, void* data_dev, size_t R, int inverse, void* stream) {
 int nbs_probe_kstep(nbs_ctx* c, int cls, int warps, int nsteps, int reps, double* cycles_per_kstep, double* cycles_max) {
     if (!c) return NBS_EINVAL;
     if (c->cuda_failed) return NBS_ECUDA;
-    if ((cls != 0 && cls != 2) || warps < 1 || warps > C_THREADS / 32 || nsteps < 1 || nsteps > PROBE_KSTEP_MAX_STEPS || reps < 1)
+    if ((cls != 0 && cls != 2) || warps < 1 || warps > PROBE_KSTEP_THREADS / 32 || nsteps < 1 || nsteps > PROBE_KSTEP_MAX_STEPS || reps < 1)
         return fail(c, NBS_EINVAL, "nbs_probe_kstep: cls 0 or 2, 1 <= warps <= 12, 1 <= nsteps <= 48, reps >= 1");
     CU(c, cudaSetDevice(c->device));
     // packed gather words whose four consecutive k fall into four different bank groups modulo 4 (what the real
@@ -1352,7 +1352,7 @@ int nbs_probe_kstep(nbs_ctx* c, int cls, int warps, int nsteps, int reps, double
         const uint32_t k = (cls >= 2 && i < 65536) ? (uint32_t)((i / 16) % 4) : (uint32_t)((i / 4) % 4);
         tab[i] = ((next() * 4 + k) * 16u) | (((next() * 4 + k) * 16u) << 16);
     }
-    const int grid = c->prod_grid, nw = C_THREADS / 32;
+    const int grid = c->prod_grid, nw = PROBE_KSTEP_THREADS / 32;
     uint32_t* d_tab = nullptr; double2* d_out = nullptr; long long* d_cyc = nullptr;
     CU(c, cudaMalloc((void**)&d_tab, tab.size() * sizeof(uint32_t)));
     CU(c, cudaMalloc((void**)&d_out, (size_t)grid * nw * 256 * sizeof(double2)));
@@ -1362,7 +1362,7 @@ int nbs_probe_kstep(nbs_ctx* c, int cls, int warps, int nsteps, int reps, double
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_probe_kstep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C_BLOCKS_BYTES);
     std::vector<long long> cyc((size_t)grid * nw, 0);
     if (e == cudaSuccess) {
-        k_probe_kstep<<<grid, C_THREADS, C_BLOCKS_BYTES>>>(d_tab, cls, nsteps, reps, warps, d_out, d_cyc);
+        k_probe_kstep<<<grid, PROBE_KSTEP_THREADS, C_BLOCKS_BYTES>>>(d_tab, cls, nsteps, reps, warps, d_out, d_cyc);
         e = cudaDeviceSynchronize();
     }
     if (e == cudaSuccess) e = cudaMemcpy(cyc.data(), d_cyc, cyc.size() * sizeof(long long), cudaMemcpyDeviceToHost);

@@ -10,11 +10,11 @@
 
 namespace nbs {
 
-template <int ET, int EG, bool ALIAS>
+template <int ET, int EG, int NM, bool ALIAS>
 __device__ __forceinline__ void combine_item_c(const ProdArgs& a, int ip, size_t q, const double2* __restrict__ scr, int et,
                                                char* s_epi, double osign) {
-    constexpr int NMT = 256 / ET;          // components per thread ...
-    constexpr int NM = NMT > 2 ? 2 : NMT;  // ... taken NM at a time (register budget: two batches of EG rows in flight)
+    constexpr int NMT = 256 / ET;          // components per thread, taken NM at a time (register budget: two batches of EG rows in flight)
+    static_assert(NMT % NM == 0, "NM divides the components of a thread");
     Pair3Rec* pr = reinterpret_cast<Pair3Rec*>(s_epi);
     PairChanRec* pcs = reinterpret_cast<PairChanRec*>(s_epi + EPI_PAIR_BYTES);
     {

@@ -117,12 +117,13 @@ __global__ void __launch_bounds__(PROBE_THREADS, 1) k_probe_fp64(int iters, doub
 // run_unit_wide_c (cls 2) -- `reps` times on a synthetic unit of one diagram with `nsteps` k-steps: two compact blocks
 // in shared memory, packed gather words from L2 with bank-conflict-free offsets (the residue rule of
 // nbs_tables.hpp), another table region every repetition.  cyc[CTA * 12 + warp] = cycles of the warp's loop.
-__global__ void __launch_bounds__(C_THREADS, 1) k_probe_kstep(const uint32_t* __restrict__ tab, int cls, int nsteps, int reps,
+constexpr int PROBE_KSTEP_THREADS = 384; // up to 12 warps per SM, 168 registers: no setmaxnreg needed
+__global__ void __launch_bounds__(PROBE_KSTEP_THREADS, 1) k_probe_kstep(const uint32_t* __restrict__ tab, int cls, int nsteps, int reps,
                                                               int ncw, double2* __restrict__ out, long long* __restrict__ cyc) {
     extern __shared__ __align__(128) char prod_smem[];
     char* sm = prod_smem;
     __shared__ int item[12];
-    __shared__ __align__(16) Diag3Rec drec[C_THREADS / 32];
+    __shared__ __align__(16) Diag3Rec drec[PROBE_KSTEP_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (uint32_t i = tid; i < C_BLOCKS_BYTES / 16; i += blockDim.x)
         reinterpret_cast<double2*>(sm)[i] = make_double2(1e-3 * (double)(i % 97), -2e-3 * (double)(i % 89));
@@ -134,12 +135,12 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_probe_kstep(const uint32_t* __
     if (warp >= ncw) return;
     Unit3Rec u;
     u.diag_begin = warp; u.diag_end = warp + 1; u.cls = cls; u.slot = 0;
-    double2* o = out + ((size_t)blockIdx.x * (C_THREADS / 32) + warp) * 256;
+    double2* o = out + ((size_t)blockIdx.x * (PROBE_KSTEP_THREADS / 32) + warp) * 256;
     const long long t0 = clock64();
     for (int r = 0; r < reps; ++r) {
         if (lane == 0) {
             Diag3Rec d;
-            d.offA = (uint32_t)(((r * (C_THREADS / 32) + warp) % 16) * 4096); d.offB = 65536u + d.offA;
+            d.offA = (uint32_t)(((r * (PROBE_KSTEP_THREADS / 32) + warp) % 16) * 4096); d.offB = 65536u + d.offA;
             d.sbeg = 0; d.send = (uint16_t)nsteps; d.nwA = 1; d.nwB = (uint8_t)(cls >= 2 ? 4 : 1); d.K = (uint16_t)(4 * nsteps);
             drec[warp] = d;
         }
@@ -153,7 +154,7 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_probe_kstep(const uint32_t* __
         else run_unit_wide_c(u, drec, tab, sm, item, o, lane);
         __syncwarp();
     }
-    if (lane == 0) cyc[blockIdx.x * (C_THREADS / 32) + warp] = clock64() - t0;
+    if (lane == 0) cyc[blockIdx.x * (PROBE_KSTEP_THREADS / 32) + warp] = clock64() - t0;
 }
 constexpr int PROBE_KSTEP_MAX_STEPS = 48;        // a table region holds 4096 words = 64 k-steps of the widest table
 constexpr size_t PROBE_KSTEP_TAB_WORDS = 1 << 17; // A tables in the first half, B tables in the second

@@ -20,15 +20,22 @@
 
 namespace nbs {
 
-// Warp split: 10 compute + 2 epilogue warps, as in k_product_t.  Measured alternatives (profiles/r2_summary.md):
-// 8 compute warps run within 2 % of 10 (the arithmetic nearly saturates at two warps per SM sub-partition); four
-// epilogue warps take issue slots and shared-memory bandwidth from the compute warps of every sub-partition (67
-// against 63.6 ms); 13 warps leave 128 registers per thread (four warps on one sub-partition) and spill.
-// The epilogue reads the unit rows with a pipelined reader (nbs_epilogue_c.cuh), C_EPI_ROWS rows per batch: the compute
-// warps wait 0.3 % of their time for a free ring buffer (combine_item: 0.7 %), 62.0 against 62.5 ms, and the kernel
-// needs 152 instead of 168 registers.
-constexpr int C_CWARPS = PROD_CWARPS, C_EWARPS = PROD_EWARPS;
-constexpr int C_EPI_ROWS = 3;
+// Warp split: 12 compute warps (three per SM sub-partition) + 4 epilogue warps = four warp groups of 128 threads.  The
+// CTA is launched with 65536 / 512 = 128 registers per thread; at its first instruction every compute warp group
+// raises its budget to C_REG_COMPUTE and the epilogue warp group lowers its own to C_REG_EPILOGUE (setmaxnreg: 12 x
+// 32 x 144 + 4 x 32 x 80 = 65536, the whole register file of the SM), so the unit code keeps the registers it needs
+// (no spills) while a third compute warp per sub-partition covers more of the latency of a k-step's dependent chain
+// (isolated unit code, nbs_probe_kstep: 288 / 551 cycles per k-step and sub-partition with 12 warps against 304 / 576
+// with 10).  Measured (profiles/r2_summary.md): 10 + 2 warps at 152 registers 62.0 ms; 12 + 4 at 128 registers without
+// setmaxnreg 65.5 (spills); 12 + 4 with 144 / 80 registers 60.1; with units of whole diagrams (build_plan) 58.8.
+// Other budgets: 136 / 104 60.9 - 64.2, 152 / 56 64.5 (the epilogue spills).
+// The epilogue reads the unit rows with a pipelined reader (nbs_epilogue_c.cuh), C_EPI_ROWS rows per batch, one spin
+// component per thread and pass (C_EPI_NM: two components need more than 80 registers).
+constexpr int C_CWARPS = 12, C_EWARPS = 4;
+constexpr int C_REG_COMPUTE = 144, C_REG_EPILOGUE = 80;
+static_assert(C_CWARPS % 4 == 0 && C_EWARPS == 4, "setmaxnreg works on warp groups of four warps");
+static_assert(32 * (C_CWARPS * C_REG_COMPUTE + C_EWARPS * C_REG_EPILOGUE) == 65536, "register budgets must add up to the register file");
+constexpr int C_EPI_ROWS = 3, C_EPI_NM = 1;
 constexpr int C_CTHREADS = C_CWARPS * 32, C_ETHREADS = C_EWARPS * 32, C_THREADS = C_CTHREADS + C_ETHREADS;
 
 struct CProdArgs {
@@ -378,6 +385,7 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
 
     if (tid >= C_CTHREADS) {
         // ---------------- epilogue warps: combine item i while the compute warps run the following items
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C_REG_EPILOGUE));
         const int et = tid - C_CTHREADS;
         for (unsigned it = 0;; ++it) {
             const int b = it % PROD_NBUF;
@@ -385,13 +393,14 @@ __global__ void __launch_bounds__(C_THREADS, 1) k_product_c(const CProdArgs a) {
             const int ip = ctl->meta_pair[b];
             if (ip < 0) break;
             const size_t q = (size_t)ctl->meta_q[b];
-            combine_item_c<C_ETHREADS, C_EPI_ROWS, ALIAS>(a.base, ip, q, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
+            combine_item_c<C_ETHREADS, C_EPI_ROWS, C_EPI_NM, ALIAS>(a.base, ip, q, scr0 + b * scr_stride, et, s_epi, __ldg(a.pair_sign + ip));
             if (et == 0) mbar_arrive(&ctlp->empty[b]); // combine_item ends with a barrier of the epilogue threads
         }
         return;
     }
 
     // ---------------- compute warps
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C_REG_COMPUTE));
     const int lane = tid & 31;
 #ifdef NBS_PROF
     long long pf[PF_N] = {};

@@ -262,8 +262,12 @@ struct Plan {
 // (it carries a u <-> d image to write); a non-NULL vector switches the relation
 //   F[B B' | B3 B4](q)_{a1 a2 a3 a4} = - eta_B eta_B' eta_3 eta_4 F[B B' | B3' B4'](-q)_{a2 a1 a3 a4}      (B' = image of B)
 // on for every sink pair whose channel set is closed under it: such a pair is computed for q <= -q only.
-std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps = 18,
-                       int unit_cost_max = 80, const std::vector<char>* iso_conj = nullptr);
+// unit_split_steps: a diagram with more k-steps is split over several units; unit_cost_max: diagrams are packed into a
+// unit up to this cost (2 per 16x16 k-step, 3 per 64x4 k-step).  Defaults: whole diagrams (K = 144 has 36 k-steps),
+// measured best with 12 compute warps: (36, 120 - 160) 58.8 ms, (18, 80) 60.1, (18, 240) 61.4, (36, 200) 60.8 at 32^3.
+constexpr int UNIT_SPLIT_STEPS_DEFAULT = 36, UNIT_COST_MAX_DEFAULT = 140;
+std::string build_plan(const std::vector<nbs_channel>& channels, Plan& plan, int unit_split_steps = UNIT_SPLIT_STEPS_DEFAULT,
+                       int unit_cost_max = UNIT_COST_MAX_DEFAULT, const std::vector<char>* iso_conj = nullptr);
 
 // Channel relations of the isospin limit (u and d propagators identical): relabelling u <-> d maps every
 // interpolating field of eqs. 2.2-2.3 to +-1 times another one (p <-> n, Sigma+ <-> Sigma-, Xi0 <-> -Xi-, Lambda -> -Lambda,
